@@ -1,0 +1,165 @@
+"""ctypes binding of the CPU oracle (oracle/rt_oracle.cpp).  TEST INFRASTRUCTURE.
+
+Argument marshalling only; all arithmetic is in the C++ file.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+W0 = 1 << 32  # tally quanta per photon
+FATE_ATM_ABS, FATE_SFC_ABS, FATE_TOD_EXIT, FATE_CAPPED = 1, 2, 3, 4
+
+COUNTER_FIELDS = ("n_photons", "n_events", "n_null", "n_rayleigh", "n_hg", "n_atm_abs",
+                  "n_sfc_hits", "n_sfc_abs", "n_toa", "n_capped", "n_cell_steps", "capped_energy")
+
+
+class Counters(C.Structure):
+    _fields_ = [(n, C.c_uint64) for n in COUNTER_FIELDS[:-1]] + [("capped_energy", C.c_int64)]
+
+    def asdict(self):
+        return {n: int(getattr(self, n)) for n in COUNTER_FIELDS}
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        fp = C.POINTER(C.c_float)
+        ip = C.POINTER(C.c_int64)
+        _lib.orc_trace.restype = C.c_int
+        _lib.orc_trace.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float,
+                                   C.c_int, C.c_int, C.c_int, fp, fp, fp, fp, fp, C.c_double, C.c_double,
+                                   C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint32, ip, ip, ip, ip, ip,
+                                   C.POINTER(Counters), C.POINTER(C.c_uint32), C.c_int,
+                                   C.POINTER(C.c_double)]
+        _lib.orc_hardware_threads.restype = C.c_int
+    return _lib
+
+
+def _f32(a):
+    a = np.ascontiguousarray(a, dtype=np.float32)
+    return a, a.ctypes.data_as(C.POINTER(C.c_float))
+
+
+class Tallies:
+    """int64 tallies in the caller-visible layout: atm_abs [nz][ny][nx], the rest [ny][nx]."""
+
+    def __init__(self, nx, ny, nz):
+        self.atm_abs = np.zeros((nz, ny, nx), dtype=np.int64)
+        self.sfc_dir = np.zeros((ny, nx), dtype=np.int64)
+        self.sfc_dif = np.zeros((ny, nx), dtype=np.int64)
+        self.sfc_abs = np.zeros((ny, nx), dtype=np.int64)
+        self.toa_up = np.zeros((ny, nx), dtype=np.int64)
+        self.counters = Counters()
+
+    def closure(self):
+        """Sum of the terminal bins (must equal n_photons * W0 exactly)."""
+        return (int(self.atm_abs.sum()) + int(self.sfc_abs.sum()) + int(self.toa_up.sum())
+                + int(self.counters.capped_energy))
+
+
+def trace(grid, optics, zenith_deg, azimuth_deg, n_photons, first_photon_id=0, seed=1, stream_id=0,
+          precision=64, tallies=None, records=False, n_threads=1):
+    """Run the oracle.  grid = (nx, ny, nz, dx, dy, dz, bx, by, bz); optics = dict with
+    k_ext, k_ext_cloud, ssa, g ([nz][ny][nx] fp32) and sfc_albedo ([ny][nx] fp32).
+    Returns (tallies, records or None, elapsed seconds of the photon loop)."""
+    nx, ny, nz, dx, dy, dz, bx, by, bz = grid
+    k, kp = _f32(optics["k_ext"])
+    kc, kcp = _f32(optics["k_ext_cloud"])
+    w, wp = _f32(optics["ssa"])
+    g, gp = _f32(optics["g"])
+    al, alp = _f32(optics["sfc_albedo"])
+    assert k.size == nx * ny * nz and al.size == nx * ny
+    t = tallies if tallies is not None else Tallies(nx, ny, nz)
+    rec = np.zeros((n_photons, 4), dtype=np.uint32) if records else None
+    ip = C.POINTER(C.c_int64)
+    el = C.c_double(0.0)
+    rc = lib().orc_trace(int(precision), nx, ny, nz, dx, dy, dz, bx, by, bz, kp, kcp, wp, gp, alp,
+                         float(zenith_deg), float(azimuth_deg), int(n_photons), int(first_photon_id),
+                         int(seed), int(stream_id), t.atm_abs.ctypes.data_as(ip),
+                         t.sfc_dir.ctypes.data_as(ip), t.sfc_dif.ctypes.data_as(ip),
+                         t.sfc_abs.ctypes.data_as(ip), t.toa_up.ctypes.data_as(ip), C.byref(t.counters),
+                         rec.ctypes.data_as(C.POINTER(C.c_uint32)) if records else None,
+                         int(n_threads), C.byref(el))
+    if rc != 0:
+        raise ValueError("orc_trace: bad arguments (rc=%d)" % rc)
+    return t, rec, el.value
+
+
+def philox4x32_10(ctr, key):
+    c = (C.c_uint32 * 4)(*ctr)
+    k = (C.c_uint32 * 2)(*key)
+    o = (C.c_uint32 * 4)()
+    lib().orc_philox4x32_10(c, k, o)
+    return tuple(int(x) for x in o)
+
+
+def neg_log_f32(w):
+    w, wp = _f32(w)
+    out = np.empty_like(w)
+    lib().orc_neg_log_f32(wp, out.ctypes.data_as(C.POINTER(C.c_float)), C.c_uint64(w.size))
+    return out
+
+
+def sincos_2pi_f32(u):
+    u, up = _f32(u)
+    s = np.empty_like(u)
+    c = np.empty_like(u)
+    fp = C.POINTER(C.c_float)
+    lib().orc_sincos_2pi_f32(up, s.ctypes.data_as(fp), c.ctypes.data_as(fp), C.c_uint64(u.size))
+    return s, c
+
+
+def _f64(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def sample_hg(g, u, precision=64):
+    u, up = _f64(u)
+    mu = np.empty_like(u)
+    lib().orc_sample_hg(int(precision), C.c_double(g), up, mu.ctypes.data_as(C.POINTER(C.c_double)),
+                        C.c_uint64(u.size))
+    return mu
+
+
+def sample_rayleigh(u, precision=64):
+    u, up = _f64(u)
+    mu = np.empty_like(u)
+    lib().orc_sample_rayleigh(int(precision), up, mu.ctypes.data_as(C.POINTER(C.c_double)),
+                              C.c_uint64(u.size))
+    return mu
+
+
+def rotate(d, mu, u_phi, precision=64):
+    v = (C.c_double * 3)(*d)
+    lib().orc_rotate(int(precision), v, C.c_double(mu), C.c_double(u_phi))
+    return np.array(list(v))
+
+
+def pack_optics_f32(k, kc, w, g):
+    k, kp = _f32(k)
+    kc, kcp = _f32(kc)
+    w, wp = _f32(w)
+    g, gp = _f32(g)
+    out = np.empty((k.size, 4), dtype=np.float32)
+    lib().orc_pack_optics_f32(kp, kcp, wp, gp, out.ctypes.data_as(C.POINTER(C.c_float)),
+                              C.c_uint64(k.size))
+    return out
+
+
+def majorant(nx, ny, nz, bx, by, bz, k_ext):
+    k, kp = _f32(k_ext)
+    out = np.empty(((nz // bz), (ny // by), (nx // bx)), dtype=np.float32)
+    lib().orc_majorant(nx, ny, nz, bx, by, bz, kp, out.ctypes.data_as(C.POINTER(C.c_float)))
+    return out
+
+
+def hardware_threads():
+    return int(lib().orc_hardware_threads())

@@ -1,0 +1,525 @@
+// rt_oracle.cpp — CPU ORACLE for the forward Monte Carlo shortwave photon tracer.
+//
+// TEST INFRASTRUCTURE, NOT PRODUCT.  Only tests/, __graft_entry__.smoke() and
+// bench.py's cpu_baseline / --impl reference legs may build, load or call this
+// file.  The CUDA path (paper_2208_05247_b200/csrc) shares no code with it and
+// never calls it; the two were written separately from the normative text in
+// DESIGN.md §3 ("Stream definition").
+//
+// What it computes (§2.3 "The ray tracer"):
+// photons launched at the domain top along the sun beam, propagated by
+// single-level null-collision tracking on a coarse acceleration grid whose cell
+// value is the highest extinction coefficient inside the cell, local
+// optical properties fetched from the fine grid, Rayleigh / Henyey-
+// Greenstein scattering chosen with probability k_ext,cloud/k_ext,
+// Lambertian surface with local albedo, tallies of surface and
+// domain-top fluxes and 3D absorbed power.  Absorption is ANALOG
+// (BASELINE.json north_star, reading D1): a photon ends in exactly one bin and
+// carries W0 = 2^32 integer quanta, so energy closes exactly in int64.
+//
+// Plain, slow, single-threaded by definition (n_threads > 1 only splits the
+// photon-id range for wall-clock timing; integer tallies make the result
+// identical).  It follows DESIGN.md §3 step by step, in that order and
+// notation, with no blocking, fusion or reordering.
+//
+// Precision.  The tracer is a template on Real:
+//   Real = double : the oracle proper.  fp64 geometry, libm log/sin/cos/cbrt-
+//                   free Rayleigh inversion.  Pinned by tests/test_oracle_*.py
+//                   (Beer-Lambert, closure, limits, symmetry, single scatter,
+//                   Philox known answers, sampler moments).
+//   Real = float  : the same statements in the kernel's precision.  Every
+//                   geometric comparison decides an integer (which cell face,
+//                   which voxel, which event), so for the per-photon identity
+//                   criterion both sides take those decisions in fp32, using
+//                   the fp32 elementary functions that DESIGN.md §3.3 fixes
+//                   operation by operation (log, sincospi).  Every operation is
+//                   an IEEE-754 correctly rounded +,-,*,/,sqrt,fma, so this
+//                   instantiation is bit-reproducible on any conforming machine.
+// Build with -ffp-contract=off (no implicit FMA); fma is written explicitly.
+//
+// Parity unpinned: the discrete cloud-vs-gas choice where cloud and gas share
+// a voxel (Q4 in DESIGN.md §2) is the paper's stated approximation; it
+// is pinned oracle<->GPU only, not against physics.
+
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <thread>
+#include <vector>
+#include <algorithm>
+#include <chrono>
+
+namespace {
+
+// ---------------------------------------------------------------------------
+// §3.1 Philox4x32-10 (Salmon et al., SC'11).  Constants as in the CUDA toolkit
+// header curand_philox4x32_x.h (PHILOX_W32_0/1, PHILOX_M4x32_0/1).
+// ---------------------------------------------------------------------------
+struct U4 { uint32_t x, y, z, w; };
+
+inline U4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                        uint32_t k0, uint32_t k1) {
+  const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
+  const uint32_t W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+  for (int r = 0; r < 10; ++r) {
+    uint64_t p0 = (uint64_t)M0 * c0;
+    uint64_t p1 = (uint64_t)M1 * c2;
+    uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+    uint32_t n1 = (uint32_t)p1;
+    uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+    uint32_t n3 = (uint32_t)p0;
+    c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    k0 += W0; k1 += W1;
+  }
+  return U4{c0, c1, c2, c3};
+}
+
+// §3.2 word -> uniform in [0,1): top 24 bits, exact in fp32 and fp64.
+template <class R> inline R uni24(uint32_t x) { return (R)(x >> 8) * (R)(1.0 / 16777216.0); }
+
+// ---------------------------------------------------------------------------
+// §3.3 fp32 elementary functions fixed operation by operation.
+// ---------------------------------------------------------------------------
+inline float spec_neg_log(float w) {  // -ln(w), w in [2^-24, 1]
+  int32_t ix; std::memcpy(&ix, &w, 4);
+  int32_t E = (ix - 0x3f3504f3) >> 23;         // arithmetic shift (floor)
+  int32_t im = ix - (E << 23);
+  float m; std::memcpy(&m, &im, 4);            // m in [sqrt(1/2), sqrt(2))
+  float f = m - 1.0f;
+  float P = 0x1.645de2p-4f;                    // Horner, degree 6 in f
+  P = std::fmaf(P, f, -0x1.2432aap-3f);
+  P = std::fmaf(P, f, 0x1.317470p-3f);
+  P = std::fmaf(P, f, -0x1.53824cp-3f);
+  P = std::fmaf(P, f, 0x1.98d7f0p-3f);
+  P = std::fmaf(P, f, -0x1.000382p-2f);
+  P = std::fmaf(P, f, 0x1.5556d8p-2f);
+  float f2 = f * f;
+  float r = std::fmaf(f * f2, P, -0.5f * f2);
+  float l1p = f + r;
+  float Ef = (float)E;
+  float res = std::fmaf(Ef, 0x1.62e4p-1f, std::fmaf(Ef, 0x1.7f7d1cp-20f, l1p));
+  return -res;
+}
+
+inline void spec_sincos_2pi(float u, float& sn_out, float& cs_out) {  // angle 2*pi*u, u in [0,1)
+  float t = 2.0f * u;
+  int j = (int)std::fmaf(2.0f, t, 0.5f);       // nearest quarter turn, 0..4
+  float r = t - 0.5f * (float)j;               // exact, in [-1/4, 1/4]
+  float z = r * r;
+  float S = -0x1.2d9302p-1f;
+  S = std::fmaf(S, z, 0x1.465e92p+1f);
+  S = std::fmaf(S, z, -0x1.4abbbap+2f);
+  S = std::fmaf(S, z, 0x1.921fb6p+1f);
+  float sn = r * S;
+  float C = 0x1.d99f54p-3f;
+  C = std::fmaf(C, z, -0x1.55c4eap+0f);
+  C = std::fmaf(C, z, 0x1.03c1dap+2f);
+  C = std::fmaf(C, z, -0x1.3bd3ccp+2f);
+  float cs = std::fmaf(C, z, 1.0f);
+  switch (j & 3) {
+    case 0: sn_out = sn;  cs_out = cs;  break;
+    case 1: sn_out = cs;  cs_out = -sn; break;
+    case 2: sn_out = -sn; cs_out = -cs; break;
+    default: sn_out = -cs; cs_out = sn; break;
+  }
+}
+
+// Real-generic wrappers: double uses the plain library definition.
+template <class R> struct Elem;
+template <> struct Elem<float> {
+  static float neg_log_1m(float u) { return spec_neg_log(1.0f - u); }
+  static void sincos_2pi(float u, float& s, float& c) { spec_sincos_2pi(u, s, c); }
+  static float fma(float a, float b, float c) { return std::fmaf(a, b, c); }
+};
+template <> struct Elem<double> {
+  static double neg_log_1m(double u) { return -std::log(1.0 - u); }
+  static void sincos_2pi(double u, double& s, double& c) {
+    const double two_pi = 6.283185307179586476925286766559;
+    s = std::sin(two_pi * u); c = std::cos(two_pi * u);
+  }
+  static double fma(double a, double b, double c) { return std::fma(a, b, c); }
+};
+
+// ---------------------------------------------------------------------------
+// §3.9 samplers
+// ---------------------------------------------------------------------------
+// Henyey-Greenstein ("Henyey-Greenstein phase function without delta-scaling"):
+// inverse CDF of p(mu) = (1-g^2) / (2 (1 + g^2 - 2 g mu)^(3/2)).
+template <class R> inline R sample_hg(R g, R u) {
+  R mu;
+  if (std::fabs(g) < (R)1e-3) {
+    mu = Elem<R>::fma((R)2, u, (R)-1);
+  } else {
+    R gg = g * g;
+    R den = Elem<R>::fma((R)2 * g, u, (R)1 - g);
+    R q = ((R)1 - gg) / den;
+    R num = Elem<R>::fma(-q, q, (R)1 + gg);
+    mu = num / ((R)2 * g);
+  }
+  return std::min((R)1, std::max((R)-1, mu));
+}
+
+// Rayleigh ("Rayleigh phase function for scattering of gases"):
+// p(mu) = 3/8 (1 + mu^2); CDF(mu) = (mu^3 + 3 mu + 4)/8 = u.  Solve the cubic
+// mu^3 + 3 mu - y = 0, y = 8u - 4, by 4 Newton steps from mu0 = y/4.
+template <class R> inline R sample_rayleigh(R u) {
+  R y = Elem<R>::fma((R)8, u, (R)-4);
+  R mu = (R)0.25 * y;
+  for (int it = 0; it < 4; ++it) {
+    R m2 = mu * mu;
+    R fv = Elem<R>::fma(mu, m2, Elem<R>::fma((R)3, mu, -y));
+    R dv = Elem<R>::fma((R)3, m2, (R)3);
+    mu = mu - fv / dv;
+  }
+  return std::min((R)1, std::max((R)-1, mu));
+}
+
+// Rotate direction (a,b,c) by polar cosine mu and azimuth (cphi,sphi); §3.9.
+template <class R>
+inline void rotate_dir(R& a, R& b, R& c, R mu, R cphi, R sphi) {
+  R s = std::sqrt(std::max((R)0, Elem<R>::fma(-mu, mu, (R)1)));
+  R nx, ny, nz;
+  if (std::fabs(c) < (R)0.99999) {
+    R r = std::sqrt(Elem<R>::fma(-c, c, (R)1));
+    R h = s / r;
+    R ac = a * c, bc = b * c;
+    R t1 = Elem<R>::fma(ac, cphi, -(b * sphi));
+    R t2 = Elem<R>::fma(bc, cphi, a * sphi);
+    nx = Elem<R>::fma(h, t1, a * mu);
+    ny = Elem<R>::fma(h, t2, b * mu);
+    nz = Elem<R>::fma(-(s * r), cphi, c * mu);
+  } else {
+    nx = s * cphi; ny = s * sphi; nz = (c > 0 ? mu : -mu);
+  }
+  R n2 = Elem<R>::fma(nz, nz, Elem<R>::fma(ny, ny, nx * nx));
+  R inv = (R)1 / std::sqrt(n2);
+  a = nx * inv; b = ny * inv; c = nz * inv;
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------
+// C ABI (ctypes).  Counters mirror include/rt.h's rt_counters but are declared
+// here independently.
+// ---------------------------------------------------------------------------
+extern "C" {
+
+struct orc_counters {
+  uint64_t n_photons, n_events, n_null, n_rayleigh, n_hg, n_atm_abs, n_sfc_hits, n_sfc_abs,
+      n_toa, n_capped, n_cell_steps;
+  int64_t capped_energy;
+};
+
+enum { ORC_ATM_ABS = 1, ORC_SFC_ABS = 2, ORC_TOD_EXIT = 3, ORC_CAPPED = 4 };
+
+}  // extern "C"
+
+namespace {
+
+constexpr int64_t W0 = (int64_t)1 << 32;       // tally quanta per photon
+constexpr uint32_t EVENT_CAP = 1u << 20;       // §3.12
+
+struct Problem {
+  int nx, ny, nz, bx, by, bz;
+  float dx, dy, dz;
+  const float *k_ext, *k_cloud, *ssa, *g, *albedo;
+  double zenith_deg, azimuth_deg;
+  uint64_t n_photons, first_id, seed;
+  uint32_t stream_id;
+  int64_t *atm_abs, *sfc_dir, *sfc_dif, *sfc_abs, *toa_up;
+  uint32_t* records;
+};
+
+inline void add64(int64_t* p, int64_t v) { __atomic_fetch_add(p, v, __ATOMIC_RELAXED); }
+
+// §3.1 step 1: per-voxel cumulative coefficients, in Real, in this order.
+template <class R> struct Vox { R c1, c2, c3, g; };
+template <class R>
+inline Vox<R> pack_voxel(float kf, float kcf, float wf, float gf) {
+  R k = (R)kf, kc = (R)kcf, w = (R)wf;
+  Vox<R> v;
+  v.c3 = k;
+  v.c1 = ((R)1 - w) * k;
+  R frac = (k > 0) ? kc / k : (R)0;
+  v.c2 = v.c1 + (w * k) * frac;
+  v.c2 = std::min(v.c2, v.c3);
+  v.c1 = std::min(v.c1, v.c2);
+  v.g = (R)gf;
+  return v;
+}
+
+template <class R>
+void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_begin, uint64_t i_end,
+                 orc_counters& C) {
+  typedef Elem<R> E;
+  const int nx = P.nx, ny = P.ny, nz = P.nz, bx = P.bx, by = P.by, bz = P.bz;
+  const int ncx = nx / bx, ncy = ny / by, ncz = nz / bz;
+  const uint64_t ncol = (uint64_t)nx * ny;
+  const uint64_t n_full = (P.n_photons / ncol) * ncol;
+  const R dx = (R)P.dx, dy = (R)P.dy, dz = (R)P.dz;
+  const R rdx = (R)1 / dx, rdy = (R)1 / dy, rdz = (R)1 / dz;
+  const R Lx = (R)bx * dx, Ly = (R)by * dy, Lz = (R)bz * dz;
+  const R TINY = (R)1e-30f;
+
+  // §3.3 sun direction: computed in double, then converted to Real.
+  const double deg = 3.14159265358979323846 / 180.0;
+  const double th = P.zenith_deg * deg, ph = P.azimuth_deg * deg;
+  const R sun_x = (R)(float)(-std::sin(th) * std::sin(ph));
+  const R sun_y = (R)(float)(-std::sin(th) * std::cos(ph));
+  const R sun_z = (R)(float)(-std::cos(th));
+  const uint32_t k0 = (uint32_t)P.seed, k1 = (uint32_t)(P.seed >> 32);
+
+  for (uint64_t i = i_begin; i < i_end; ++i) {
+    const uint64_t pid = P.first_id + i;
+    const uint32_t p_lo = (uint32_t)pid, p_hi = (uint32_t)(pid >> 32);
+
+    // ---- step 3: launch, event index 0 --------------------------------------
+    U4 X = philox4x32_10(p_lo, p_hi, 0u, P.stream_id, k0, k1);
+    R u0 = uni24<R>(X.x), u1 = uni24<R>(X.y), u2 = uni24<R>(X.z), u3 = uni24<R>(X.w);
+    int ix, iy;
+    if (i < n_full) {
+      uint64_t col = i % ncol;
+      ix = (int)(col % nx); iy = (int)(col / nx);
+    } else {
+      ix = std::min((int)(u2 * (R)nx), nx - 1);
+      iy = std::min((int)(u3 * (R)ny), ny - 1);
+    }
+    int cx = ix / bx, cy = iy / by, cz = ncz - 1;
+    R qx = ((R)(ix % bx) + u0) * dx;
+    R qy = ((R)(iy % by) + u1) * dy;
+    R qz = Lz;
+    R da = sun_x, db = sun_y, dc = sun_z;      // unit direction
+    R va, vb, vc, ia, ib, ic;                  // nudged components and reciprocals
+    auto set_dir = [&]() {
+      va = (std::fabs(da) < TINY) ? TINY : da;
+      vb = (std::fabs(db) < TINY) ? TINY : db;
+      vc = (std::fabs(dc) < TINY) ? TINY : dc;
+      ia = (R)1 / va; ib = (R)1 / vb; ic = (R)1 / vc;
+    };
+    set_dir();
+    bool direct = true;
+    uint32_t e = 1, n_ev = 0, n_sc = 0, n_sfc = 0;
+    int fate = 0; uint32_t term = 0;
+
+    // ---- step 4: draw for event e -------------------------------------------
+    R tau;
+    auto draw = [&]() {
+      X = philox4x32_10(p_lo, p_hi, e, P.stream_id, k0, k1);
+      u0 = uni24<R>(X.x); u1 = uni24<R>(X.y); u2 = uni24<R>(X.z); u3 = uni24<R>(X.w);
+      tau = E::neg_log_1m(u0);
+    };
+    draw();
+    size_t cell = ((size_t)cz * ncy + cy) * ncx + cx;
+    R kh = (R)khat[cell];
+    R rk = (kh > 0) ? (R)1 / kh : (R)0;
+
+    while (fate == 0) {
+      // ---- step 5: distance to the nearest face of the current cell ---------
+      R fx = (va > 0) ? Lx : (R)0, fy = (vb > 0) ? Ly : (R)0, fz = (vc > 0) ? Lz : (R)0;
+      R tx = (fx - qx) * ia, ty = (fy - qy) * ib, tz = (fz - qz) * ic;
+      int axis; R t;
+      if (tx <= ty && tx <= tz) { axis = 0; t = tx; }
+      else if (ty <= tz)        { axis = 1; t = ty; }
+      else                      { axis = 2; t = tz; }
+      R dtau = kh * t;
+      if (kh > 0 && tau <= dtau) {
+        // ---- step 7: tentative collision inside this cell -------------------
+        R s = tau * rk;
+        qx = std::min(Lx, std::max((R)0, E::fma(va, s, qx)));
+        qy = std::min(Ly, std::max((R)0, E::fma(vb, s, qy)));
+        qz = std::min(Lz, std::max((R)0, E::fma(vc, s, qz)));
+        int lx = std::min((int)(qx * rdx), bx - 1);
+        int ly = std::min((int)(qy * rdy), by - 1);
+        int lz = std::min((int)(qz * rdz), bz - 1);
+        size_t vox = ((size_t)(cz * bz + lz) * ny + (cy * by + ly)) * nx + (cx * bx + lx);
+        Vox<R> v = pack_voxel<R>(P.k_ext[vox], P.k_cloud[vox], P.ssa[vox], P.g[vox]);
+        ++n_ev; ++C.n_events;                  // step 6
+        // ---- step 8: classify ----------------------------------------------
+        R xi = u1 * kh;
+        if (xi < v.c1) {
+          add64(&P.atm_abs[vox], W0); ++C.n_atm_abs;
+          fate = ORC_ATM_ABS; term = (uint32_t)vox; break;
+        } else if (xi < v.c2) {                // cloud droplet: Henyey-Greenstein
+          R mu = sample_hg<R>(v.g, u2);
+          R sp, cp; E::sincos_2pi(u3, sp, cp);
+          rotate_dir<R>(da, db, dc, mu, cp, sp); set_dir();
+          direct = false; ++n_sc; ++C.n_hg;
+        } else if (xi < v.c3) {                // gas: Rayleigh
+          R mu = sample_rayleigh<R>(u2);
+          R sp, cp; E::sincos_2pi(u3, sp, cp);
+          rotate_dir<R>(da, db, dc, mu, cp, sp); set_dir();
+          direct = false; ++n_sc; ++C.n_rayleigh;
+        } else {
+          ++C.n_null;                          // null collision: direction unchanged
+        }
+        ++e;
+        if (e > EVENT_CAP) {                   // step 12
+          ++C.n_capped; C.capped_energy += W0; fate = ORC_CAPPED; term = 0; break;
+        }
+        draw();
+      } else {
+        // ---- step 5 (cont.): leave the cell through `axis` -------------------
+        tau = tau - dtau;
+        qx = std::min(Lx, std::max((R)0, E::fma(va, t, qx)));
+        qy = std::min(Ly, std::max((R)0, E::fma(vb, t, qy)));
+        qz = std::min(Lz, std::max((R)0, E::fma(vc, t, qz)));
+        ++C.n_cell_steps;
+        bool at_sfc = false, at_top = false;
+        if (axis == 0) {
+          if (va > 0) { ++cx; if (cx == ncx) cx = 0; qx = (R)0; }
+          else        { --cx; if (cx < 0) cx = ncx - 1; qx = Lx; }
+        } else if (axis == 1) {
+          if (vb > 0) { ++cy; if (cy == ncy) cy = 0; qy = (R)0; }
+          else        { --cy; if (cy < 0) cy = ncy - 1; qy = Ly; }
+        } else {
+          if (vc > 0) { ++cz; qz = (R)0; if (cz == ncz) at_top = true; }
+          else        { --cz; qz = Lz;   if (cz < 0) at_sfc = true; }
+        }
+        if (at_sfc || at_top) {
+          int hx = cx * bx + std::min((int)(qx * rdx), bx - 1);
+          int hy = cy * by + std::min((int)(qy * rdy), by - 1);
+          size_t col = (size_t)hy * nx + hx;
+          if (at_top) {                        // step 11
+            add64(&P.toa_up[col], W0); ++C.n_toa;
+            fate = ORC_TOD_EXIT; term = (uint32_t)col; break;
+          }
+          // ---- step 10: Lambertian surface ---------------------------------
+          ++C.n_sfc_hits; ++n_sfc;
+          add64(direct ? &P.sfc_dir[col] : &P.sfc_dif[col], W0);
+          if (u1 < (R)P.albedo[col]) {
+            R mu = std::sqrt((R)1 - u2), s = std::sqrt(u2);
+            R sp, cp; E::sincos_2pi(u3, sp, cp);
+            da = s * cp; db = s * sp; dc = mu; set_dir();
+            direct = false; cz = 0; qz = (R)0;
+            ++e;
+            if (e > EVENT_CAP) {
+              ++C.n_capped; C.capped_energy += W0; fate = ORC_CAPPED; term = 0; break;
+            }
+            draw();
+          } else {
+            add64(&P.sfc_abs[col], W0); ++C.n_sfc_abs;
+            fate = ORC_SFC_ABS; term = (uint32_t)col; break;
+          }
+        }
+        cell = ((size_t)cz * ncy + cy) * ncx + cx;
+        kh = (R)khat[cell];
+        rk = (kh > 0) ? (R)1 / kh : (R)0;
+      }
+    }
+    ++C.n_photons;
+    if (P.records) {
+      uint32_t* r = P.records + 4 * i;
+      r[0] = (uint32_t)fate | (std::min(n_sfc, 0xFFFFFFu) << 8);
+      r[1] = term; r[2] = n_ev; r[3] = n_sc;
+    }
+  }
+}
+
+// §3.2 majorant: highest extinction coefficient within each acceleration cell.
+std::vector<float> build_majorant(const Problem& P) {
+  const int ncx = P.nx / P.bx, ncy = P.ny / P.by, ncz = P.nz / P.bz;
+  std::vector<float> kh((size_t)ncx * ncy * ncz, 0.0f);
+  for (int z = 0; z < P.nz; ++z)
+    for (int y = 0; y < P.ny; ++y)
+      for (int x = 0; x < P.nx; ++x) {
+        float k = P.k_ext[((size_t)z * P.ny + y) * P.nx + x];
+        float& m = kh[((size_t)(z / P.bz) * ncy + (y / P.by)) * ncx + (x / P.bx)];
+        if (k > m) m = k;
+      }
+  return kh;
+}
+
+}  // namespace
+
+extern "C" {
+
+// Returns 0 on success, -1 on bad arguments.  Tallies and counters are ADDED to.
+// elapsed_s (may be NULL) receives the wall time of the photon loop only.
+int orc_trace(int precision, int nx, int ny, int nz, float dx, float dy, float dz, int bx, int by,
+              int bz, const float* k_ext, const float* k_ext_cloud, const float* ssa, const float* g,
+              const float* sfc_albedo, double zenith_deg, double azimuth_deg, uint64_t n_photons,
+              uint64_t first_photon_id, uint64_t seed, uint32_t stream_id, int64_t* atm_abs,
+              int64_t* sfc_dir, int64_t* sfc_dif, int64_t* sfc_abs, int64_t* toa_up,
+              orc_counters* counters, uint32_t* records, int n_threads, double* elapsed_s) {
+  if (nx <= 0 || ny <= 0 || nz <= 0 || bx <= 0 || by <= 0 || bz <= 0) return -1;
+  if (nx % bx || ny % by || nz % bz) return -1;
+  if (!(zenith_deg >= 0.0 && zenith_deg < 90.0)) return -1;
+  if (precision != 32 && precision != 64) return -1;
+  Problem P{nx, ny, nz, bx, by, bz, dx, dy, dz, k_ext, k_ext_cloud, ssa, g, sfc_albedo,
+            zenith_deg, azimuth_deg, n_photons, first_photon_id, seed, stream_id,
+            atm_abs, sfc_dir, sfc_dif, sfc_abs, toa_up, records};
+  std::vector<float> khat = build_majorant(P);
+  if (n_threads < 1) n_threads = 1;
+  std::vector<orc_counters> cs(n_threads);
+  std::memset(cs.data(), 0, sizeof(orc_counters) * n_threads);
+  auto run = [&](int t) {
+    uint64_t b = n_photons * (uint64_t)t / n_threads, e = n_photons * (uint64_t)(t + 1) / n_threads;
+    if (precision == 64) trace_range<double>(P, khat, b, e, cs[t]);
+    else                 trace_range<float>(P, khat, b, e, cs[t]);
+  };
+  auto t0 = std::chrono::steady_clock::now();
+  if (n_threads == 1) run(0);
+  else {
+    std::vector<std::thread> th;
+    for (int t = 0; t < n_threads; ++t) th.emplace_back(run, t);
+    for (auto& x : th) x.join();
+  }
+  auto t1 = std::chrono::steady_clock::now();
+  if (elapsed_s) *elapsed_s = std::chrono::duration<double>(t1 - t0).count();
+  if (counters) {
+    uint64_t* dst = (uint64_t*)counters;
+    for (int t = 0; t < n_threads; ++t) {
+      const uint64_t* src = (const uint64_t*)&cs[t];
+      for (size_t j = 0; j < sizeof(orc_counters) / 8; ++j) dst[j] += src[j];
+    }
+  }
+  return 0;
+}
+
+// ---- small exports so the pins in tests/ can reach each part by itself ----
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+  U4 r = philox4x32_10(ctr[0], ctr[1], ctr[2], ctr[3], key[0], key[1]);
+  out[0] = r.x; out[1] = r.y; out[2] = r.z; out[3] = r.w;
+}
+void orc_neg_log_f32(const float* w, float* out, uint64_t n) {
+  for (uint64_t i = 0; i < n; ++i) out[i] = spec_neg_log(w[i]);
+}
+void orc_sincos_2pi_f32(const float* u, float* sn, float* cs, uint64_t n) {
+  for (uint64_t i = 0; i < n; ++i) spec_sincos_2pi(u[i], sn[i], cs[i]);
+}
+void orc_sample_hg(int precision, double g, const double* u, double* mu, uint64_t n) {
+  for (uint64_t i = 0; i < n; ++i)
+    mu[i] = precision == 64 ? sample_hg<double>(g, u[i]) : (double)sample_hg<float>((float)g, (float)u[i]);
+}
+void orc_sample_rayleigh(int precision, const double* u, double* mu, uint64_t n) {
+  for (uint64_t i = 0; i < n; ++i)
+    mu[i] = precision == 64 ? sample_rayleigh<double>(u[i]) : (double)sample_rayleigh<float>((float)u[i]);
+}
+// d is 3 doubles in/out; rotation by polar cosine mu and azimuth 2*pi*u_phi.
+void orc_rotate(int precision, double* d, double mu, double u_phi) {
+  if (precision == 64) {
+    double s, c; Elem<double>::sincos_2pi(u_phi, s, c);
+    rotate_dir<double>(d[0], d[1], d[2], mu, c, s);
+  } else {
+    float a = (float)d[0], b = (float)d[1], cc = (float)d[2], s, c;
+    Elem<float>::sincos_2pi((float)u_phi, s, c);
+    rotate_dir<float>(a, b, cc, (float)mu, c, s);
+    d[0] = a; d[1] = b; d[2] = cc;
+  }
+}
+// c is 4 floats out per voxel: c1, c2, c3, g (fp32 packing, step 1).
+void orc_pack_optics_f32(const float* k, const float* kc, const float* w, const float* g, float* c,
+                         uint64_t n) {
+  for (uint64_t i = 0; i < n; ++i) {
+    Vox<float> v = pack_voxel<float>(k[i], kc[i], w[i], g[i]);
+    c[4 * i] = v.c1; c[4 * i + 1] = v.c2; c[4 * i + 2] = v.c3; c[4 * i + 3] = v.g;
+  }
+}
+void orc_majorant(int nx, int ny, int nz, int bx, int by, int bz, const float* k_ext, float* out) {
+  Problem P{}; P.nx = nx; P.ny = ny; P.nz = nz; P.bx = bx; P.by = by; P.bz = bz; P.k_ext = k_ext;
+  std::vector<float> kh = build_majorant(P);
+  std::memcpy(out, kh.data(), kh.size() * sizeof(float));
+}
+int orc_hardware_threads() { return (int)std::thread::hardware_concurrency(); }
+
+}  // extern "C"
