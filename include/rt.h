@@ -1,0 +1,129 @@
+/* rt.h — C ABI of the B200 forward Monte Carlo shortwave photon tracer.
+ *
+ * Operation: PAPER.md §2.3 "The ray tracer" as read in DESIGN.md §2-§3:
+ * photons start at the domain top along the sun beam, fly by single-level
+ * null-collision tracking on a coarse acceleration grid whose cell value is the highest
+ * extinction coefficient inside the cell, fetch local optical properties from the
+ * fine grid, scatter by Rayleigh or Henyey-Greenstein with the cloud/gas split
+ * k_ext,cloud/k_ext, reflect at a Lambertian surface with local albedo and
+ * are tallied as surface flux (direct = never scattered), domain-top upward flux
+ * and 3D absorbed power.  Absorption is analog (BASELINE.json north_star): each
+ * photon carries RT_W0 = 2^32 integer quanta and ends in exactly one bin.
+ *
+ * Every step runs in CUDA kernels for sm_100a; there is no CPU fallback.  All functions
+ * return 0 (RT_OK) or a negative RT_E* code; no exception crosses this boundary;
+ * rt_last_error() gives the text of the last failure on that context.
+ *
+ * Layouts: 3D fields are [z][y][x] with x fastest, z = 0 at the surface; 2D fields are
+ * [y][x].  x = east, y = north.  Lateral boundaries are periodic.
+ */
+#ifndef PAPER_2208_05247_RT_H
+#define PAPER_2208_05247_RT_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RT_OK 0
+#define RT_EINVAL (-1)   /* bad argument (NULL, non-positive size, grid not divisible by block, angle) */
+#define RT_ENOMEM (-2)   /* device allocation failed */
+#define RT_ECUDA (-3)    /* a CUDA call or kernel failed; see rt_last_error */
+#define RT_EOPTICS (-4)  /* rt_set_optics: a field value is outside its physical range */
+#define RT_ESTATE (-5)   /* rt_trace before rt_set_optics */
+
+#define RT_W0 (1ll << 32) /* tally quanta per photon */
+
+/* Photon fates stored in records. */
+#define RT_FATE_ATM_ABS 1
+#define RT_FATE_SFC_ABS 2
+#define RT_FATE_TOD_EXIT 3
+#define RT_FATE_CAPPED 4
+
+typedef struct rt_ctx rt_ctx; /* opaque; owned by the library; one CUDA device per context */
+
+/* Always-on event counters, accumulated across rt_trace calls until rt_reset_tallies.
+ * n_events = tentative collisions (null + real) = n_null + n_rayleigh + n_hg + n_atm_abs:
+ * the "collision events" of BASELINE.json's metric. */
+typedef struct {
+  uint64_t n_photons, n_events, n_null, n_rayleigh, n_hg, n_atm_abs, n_sfc_hits, n_sfc_abs, n_toa,
+      n_capped, n_cell_steps;
+  int64_t capped_energy; /* quanta of photons stopped by the event cap; 0 on all shipped configs */
+} rt_counters;
+
+/* Allocate a context for an nx*ny*nz grid of dx*dy*dz metre voxels with an acceleration grid
+ * of bx*by*bz-voxel blocks ("coarser resolution than the simulation"; Q1).
+ * nx,ny,nz must be multiples of bx,by,bz; bx*by*bz <= 4096.  Allocates packed optics
+ * (16 B/voxel), the majorant grid and zeroed int64 tallies on cuda_device.  *out is owned
+ * by the library until rt_destroy. */
+int rt_create_grid(rt_ctx** out, int nx, int ny, int nz, float dx, float dy, float dz, int bx, int by,
+                   int bz, int cuda_device);
+
+/* Set the optical properties of one spectral point (k_ext, k_ext,cloud, omega0, g as 3D
+ * fields; P:56 local surface albedo).  All five are DEVICE pointers owned by the caller, fp32,
+ * nvox / nvox / nvox / nvox / ncol elements; they are read on `cuda_stream` (a cudaStream_t, NULL =
+ * default stream) and may be freed once the stream has passed this call.  Packs cumulative
+ * coefficients and builds the majorant grid (§3.5).  Validates k_ext >= 0 and
+ * finite, 0 <= k_ext_cloud <= k_ext, 0 <= ssa <= 1, |g| < 1, 0 <= albedo <= 1 on the device;
+ * a violation returns RT_EOPTICS (this call synchronises the stream to learn it). */
+int rt_set_optics(rt_ctx* ctx, const float* k_ext, const float* k_ext_cloud, const float* ssa,
+                  const float* g, const float* sfc_albedo, void* cuda_stream);
+
+/* Trace n_photons photons with global ids first_photon_id .. first_photon_id + n_photons - 1
+ * (DESIGN.md §3.6-3.12).  Sun at zenith_deg in [0, 90) and azimuth_deg clockwise from
+ * north (position of the sun).  Random numbers: Philox4x32-10, key = seed, counter =
+ * (photon id, event index, stream_id).  ADDS to the tallies and counters.  Asynchronous on
+ * `cuda_stream`. */
+int rt_trace(rt_ctx* ctx, double zenith_deg, double azimuth_deg, uint64_t n_photons,
+             uint64_t first_photon_id, uint64_t seed, uint32_t stream_id, void* cuda_stream);
+
+/* As rt_trace, and also writes one 16-byte record per photon to records_out (DEVICE pointer,
+ * 4 uint32 per photon, index = photon id - first_photon_id): word 0 = fate | surface hits << 8,
+ * word 1 = terminal voxel or column index, word 2 = collision events, word 3 = real scatters. */
+int rt_trace_records(rt_ctx* ctx, double zenith_deg, double azimuth_deg, uint64_t n_photons,
+                     uint64_t first_photon_id, uint64_t seed, uint32_t stream_id, void* cuda_stream,
+                     uint32_t* records_out);
+
+/* Synchronise the context's device work and copy tallies out.  Each output may be a host or a
+ * device pointer (detected), or NULL to skip: atm_abs nvox int64 in [z][y][x]; the others ncol
+ * int64 in [y][x]; counters is a HOST pointer or NULL.  Energy closure: sum(atm_abs) +
+ * sum(sfc_abs) + sum(toa_up) + capped_energy == n_photons * RT_W0 exactly. */
+int rt_read_tallies(rt_ctx* ctx, int64_t* atm_abs, int64_t* sfc_dir, int64_t* sfc_dif, int64_t* sfc_abs,
+                    int64_t* toa_up, rt_counters* counters);
+
+/* Zero tallies and counters on `cuda_stream`. */
+int rt_reset_tallies(rt_ctx* ctx, void* cuda_stream);
+
+/* Copy the majorant grid ([cz][cy][cx] fp32, DEVICE or HOST pointer) out; for tests. */
+int rt_read_majorant(rt_ctx* ctx, float* khat_out);
+
+/* Copy the packed per-voxel coefficients (c1,c2,c3,g; 4 fp32 per voxel, [z][y][x]) out; for tests. */
+int rt_read_packed_optics(rt_ctx* ctx, float* packed_out);
+
+/* Random-gather microbenchmark for the roofline denominator: every thread issues
+ * `loads_per_thread` independent 16-byte loads at Philox-random voxel indices of the context's
+ * packed-optics array.  Writes the elapsed milliseconds (CUDA events on `cuda_stream`) to *ms_out and
+ * the number of 16-byte loads issued to *n_loads_out.  Synchronises the stream. */
+int rt_gather_bench(rt_ctx* ctx, uint32_t loads_per_thread, void* cuda_stream, float* ms_out,
+                    uint64_t* n_loads_out);
+
+/* Milliseconds spent in the trace kernel of the most recent rt_trace* call on this context, from
+ * CUDA events recorded on that call's stream around the launch.  Synchronises on the end event. */
+int rt_last_trace_ms(rt_ctx* ctx, float* ms_out);
+
+/* Kernel launches issued by this context so far (the library's own count). */
+uint64_t rt_launch_count(const rt_ctx* ctx);
+
+/* Philox4x32-10 words for n counters (DEVICE pointers: ctr n*4 uint32, out n*4 uint32); for the
+ * bit-for-bit stream test. */
+int rt_philox_words(int cuda_device, const uint32_t* ctr, uint32_t key0, uint32_t key1, uint32_t* out,
+                    uint64_t n);
+
+const char* rt_last_error(const rt_ctx* ctx); /* never NULL; valid until the next call on ctx */
+void rt_destroy(rt_ctx* ctx);                 /* frees all device memory; NULL is a no-op */
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,197 @@
+"""Thin ctypes binding of include/rt.h (librt_b200.so).  Argument marshalling only: every step of
+the method runs in the CUDA kernels behind the C ABI.  PyTorch supplies device memory and streams.
+There is no CPU fallback: a missing library or a failed call raises."""
+import ctypes as C
+import os
+
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "librt_b200.so")
+W0 = 1 << 32
+FATE_ATM_ABS, FATE_SFC_ABS, FATE_TOD_EXIT, FATE_CAPPED = 1, 2, 3, 4
+
+EXPORTS = ("rt_create_grid", "rt_set_optics", "rt_trace", "rt_trace_records", "rt_read_tallies",
+           "rt_reset_tallies", "rt_read_majorant", "rt_read_packed_optics", "rt_gather_bench",
+           "rt_last_trace_ms", "rt_launch_count", "rt_philox_words", "rt_last_error", "rt_destroy")
+
+COUNTER_FIELDS = ("n_photons", "n_events", "n_null", "n_rayleigh", "n_hg", "n_atm_abs", "n_sfc_hits",
+                  "n_sfc_abs", "n_toa", "n_capped", "n_cell_steps", "capped_energy")
+
+
+class RtError(RuntimeError):
+    pass
+
+
+class rt_counters(C.Structure):
+    _fields_ = [(n, C.c_uint64) for n in COUNTER_FIELDS[:-1]] + [("capped_energy", C.c_int64)]
+
+    def asdict(self):
+        return {n: int(getattr(self, n)) for n in COUNTER_FIELDS}
+
+
+_lib = None
+
+
+def lib():
+    """Load librt_b200.so (built by paper_2208_05247_b200.build); raises if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RtError("CUDA library %s is missing: run `python -m paper_2208_05247_b200.build` "
+                      "(there is no CPU fallback)" % LIB_PATH)
+    L = C.CDLL(LIB_PATH)
+    vp, i32, u32, u64, f32, f64 = C.c_void_p, C.c_int, C.c_uint32, C.c_uint64, C.c_float, C.c_double
+    L.rt_create_grid.argtypes = [C.POINTER(vp), i32, i32, i32, f32, f32, f32, i32, i32, i32, i32]
+    L.rt_set_optics.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+    L.rt_trace.argtypes = [vp, f64, f64, u64, u64, u64, u32, vp]
+    L.rt_trace_records.argtypes = [vp, f64, f64, u64, u64, u64, u32, vp, vp]
+    L.rt_read_tallies.argtypes = [vp, vp, vp, vp, vp, vp, C.POINTER(rt_counters)]
+    L.rt_reset_tallies.argtypes = [vp, vp]
+    L.rt_read_majorant.argtypes = [vp, vp]
+    L.rt_read_packed_optics.argtypes = [vp, vp]
+    L.rt_gather_bench.argtypes = [vp, u32, vp, C.POINTER(f32), C.POINTER(u64)]
+    L.rt_last_trace_ms.argtypes = [vp, C.POINTER(f32)]
+    L.rt_launch_count.argtypes = [vp]
+    L.rt_launch_count.restype = u64
+    L.rt_philox_words.argtypes = [i32, vp, u32, u32, vp, u64]
+    L.rt_last_error.argtypes = [vp]
+    L.rt_last_error.restype = C.c_char_p
+    L.rt_destroy.argtypes = [vp]
+    L.rt_destroy.restype = None
+    for name in EXPORTS:
+        if name not in ("rt_launch_count", "rt_last_error", "rt_destroy"):
+            getattr(L, name).restype = i32
+    _lib = L
+    return L
+
+
+def _ptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(None)
+
+
+def _stream(device):
+    return C.c_void_p(torch.cuda.current_stream(device).cuda_stream)
+
+
+class Tallies:
+    """Tallies copied out by rt_read_tallies (torch int64, on the device or pinned host memory)."""
+
+    def __init__(self, atm_abs, sfc_dir, sfc_dif, sfc_abs, toa_up, counters):
+        self.atm_abs, self.sfc_dir, self.sfc_dif, self.sfc_abs, self.toa_up = atm_abs, sfc_dir, sfc_dif, sfc_abs, toa_up
+        self.counters = counters
+
+    def closure(self):
+        return (int(self.atm_abs.sum()) + int(self.sfc_abs.sum()) + int(self.toa_up.sum())
+                + int(self.counters.capped_energy))
+
+
+class Grid:
+    """One rt_ctx: rt_create_grid / rt_set_optics / rt_trace / rt_read_tallies (include/rt.h)."""
+
+    def __init__(self, nx, ny, nz, dx, dy, dz, bx=8, by=8, bz=8, device=0):
+        if not torch.cuda.is_available():
+            raise RtError("no CUDA device: this library has no CPU path")
+        self.L = lib()
+        self.shape = (nz, ny, nx)
+        self.block = (bx, by, bz)
+        self.device = torch.device("cuda", device)
+        self.ctx = C.c_void_p(None)
+        rc = self.L.rt_create_grid(C.byref(self.ctx), nx, ny, nz, dx, dy, dz, bx, by, bz, device)
+        if rc != 0:
+            msg = self.L.rt_last_error(self.ctx).decode() if self.ctx else "bad arguments"
+            if self.ctx:
+                self.L.rt_destroy(self.ctx)
+                self.ctx = C.c_void_p(None)
+            raise RtError("rt_create_grid failed (%d): %s" % (rc, msg))
+
+    def _check(self, rc, name):
+        if rc != 0:
+            raise RtError("%s failed (%d): %s" % (name, rc, self.L.rt_last_error(self.ctx).decode()))
+
+    def _dev32(self, a, n):
+        t = torch.as_tensor(a)
+        if t.dtype != torch.float32 or t.device != self.device or not t.is_contiguous():
+            t = t.to(device=self.device, dtype=torch.float32).contiguous()
+        if t.numel() != n:
+            raise RtError("field has %d elements, expected %d" % (t.numel(), n))
+        return t
+
+    def set_optics(self, k_ext, k_ext_cloud, ssa, g, sfc_albedo):
+        nz, ny, nx = self.shape
+        nvox, ncol = nx * ny * nz, nx * ny
+        ts = [self._dev32(k_ext, nvox), self._dev32(k_ext_cloud, nvox), self._dev32(ssa, nvox),
+              self._dev32(g, nvox), self._dev32(sfc_albedo, ncol)]
+        self._check(self.L.rt_set_optics(self.ctx, *[_ptr(t) for t in ts], _stream(self.device)), "rt_set_optics")
+
+    def trace(self, zenith_deg, azimuth_deg, n_photons, first_photon_id=0, seed=1, stream_id=0, records=False):
+        if records:
+            rec = torch.zeros((max(int(n_photons), 1), 4), dtype=torch.int32, device=self.device)
+            self._check(self.L.rt_trace_records(self.ctx, zenith_deg, azimuth_deg, int(n_photons), int(first_photon_id),
+                                                int(seed), int(stream_id), _stream(self.device), _ptr(rec)),
+                        "rt_trace_records")
+            return rec[:int(n_photons)]
+        self._check(self.L.rt_trace(self.ctx, zenith_deg, azimuth_deg, int(n_photons), int(first_photon_id),
+                                    int(seed), int(stream_id), _stream(self.device)), "rt_trace")
+        return None
+
+    def read_tallies(self, host=True, atm_abs=True):
+        nz, ny, nx = self.shape
+        kw = dict(dtype=torch.int64, device="cpu" if host else self.device)
+        a = torch.empty((nz, ny, nx), **kw) if atm_abs else None
+        cols = [torch.empty((ny, nx), **kw) for _ in range(4)]
+        cnt = rt_counters()
+        self._check(self.L.rt_read_tallies(self.ctx, _ptr(a), *[_ptr(t) for t in cols], C.byref(cnt)), "rt_read_tallies")
+        return Tallies(a, cols[0], cols[1], cols[2], cols[3], cnt)
+
+    def reset_tallies(self):
+        self._check(self.L.rt_reset_tallies(self.ctx, _stream(self.device)), "rt_reset_tallies")
+
+    def read_majorant(self):
+        nz, ny, nx = self.shape
+        bx, by, bz = self.block
+        out = torch.empty((nz // bz, ny // by, nx // bx), dtype=torch.float32)
+        self._check(self.L.rt_read_majorant(self.ctx, _ptr(out)), "rt_read_majorant")
+        return out
+
+    def read_packed_optics(self):
+        nz, ny, nx = self.shape
+        out = torch.empty((nz, ny, nx, 4), dtype=torch.float32)
+        self._check(self.L.rt_read_packed_optics(self.ctx, _ptr(out)), "rt_read_packed_optics")
+        return out
+
+    def gather_bench(self, loads_per_thread=64):
+        ms, n = C.c_float(0), C.c_uint64(0)
+        self._check(self.L.rt_gather_bench(self.ctx, loads_per_thread, _stream(self.device), C.byref(ms), C.byref(n)),
+                    "rt_gather_bench")
+        return ms.value, n.value
+
+    def last_trace_ms(self):
+        ms = C.c_float(0)
+        self._check(self.L.rt_last_trace_ms(self.ctx, C.byref(ms)), "rt_last_trace_ms")
+        return ms.value
+
+    def launch_count(self):
+        return int(self.L.rt_launch_count(self.ctx))
+
+    def close(self):
+        if self.ctx:
+            self.L.rt_destroy(self.ctx)
+            self.ctx = C.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def philox_words(ctr, key, device=0):
+    """Philox4x32-10 words for an (n, 4) int32/uint32 counter tensor on the device."""
+    ctr = ctr.contiguous()
+    out = torch.empty_like(ctr)
+    rc = lib().rt_philox_words(device, _ptr(ctr), key[0], key[1], _ptr(out), ctr.shape[0])
+    if rc != 0:
+        raise RtError("rt_philox_words failed (%d)" % rc)
+    return out

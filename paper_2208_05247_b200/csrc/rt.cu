@@ -1,0 +1,285 @@
+// rt.cu — C ABI of the photon tracer (include/rt.h) over the sm_100a kernels in rt_*.cuh.
+// Host logic only: argument checks, device memory, launches.  No step of the method runs on the CPU.
+#include "../../include/rt.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+
+#include "rt_setup.cuh"
+#include "rt_trace.cuh"
+
+struct rt_ctx {
+  int device = 0;
+  int nx = 0, ny = 0, nz = 0, bx = 0, by = 0, bz = 0, ncx = 0, ncy = 0, ncz = 0;
+  float dx = 0, dy = 0, dz = 0;
+  size_t nvox = 0, ncol = 0, ncell = 0;
+  float4* optics = nullptr;
+  float* khat = nullptr;
+  float* albedo = nullptr;
+  unsigned long long* tallies = nullptr;  // atm_abs | sfc_dir | sfc_dif | sfc_abs | toa_up
+  unsigned long long* counters = nullptr; // C_COUNT words, then the work counter
+  int* bad = nullptr;
+  float* sink = nullptr;
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  bool have_optics = false, have_trace = false;
+  int trace_blocks = 0, trace_blocks_rec = 0, sm_count = 0;
+  uint64_t launches = 0;
+  std::string err;
+};
+
+namespace {
+
+struct DeviceGuard {
+  int prev = -1;
+  explicit DeviceGuard(int dev) { cudaGetDevice(&prev); if (prev != dev) cudaSetDevice(dev); else prev = -1; }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+int fail(rt_ctx* c, int code, const char* what, cudaError_t ce = cudaSuccess) {
+  if (c) {
+    c->err = what;
+    if (ce != cudaSuccess) { c->err += ": "; c->err += cudaGetErrorString(ce); }
+  }
+  return code;
+}
+
+#define RT_CUDA(ctx, call)                                              \
+  do {                                                                  \
+    cudaError_t ce_ = (call);                                           \
+    if (ce_ != cudaSuccess) return fail(ctx, ce_ == cudaErrorMemoryAllocation ? RT_ENOMEM : RT_ECUDA, #call, ce_); \
+  } while (0)
+
+unsigned long long* tally_ptr(rt_ctx* c, int which) {  // 0 atm_abs, 1..4 the column tallies
+  return which == 0 ? c->tallies : c->tallies + c->nvox + (size_t)(which - 1) * c->ncol;
+}
+
+int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photons, uint64_t first_id,
+             uint64_t seed, uint32_t stream_id, void* stream_v, uint32_t* records) {
+  if (!c) return RT_EINVAL;
+  if (!c->have_optics) return fail(c, RT_ESTATE, "rt_trace: call rt_set_optics first");
+  if (!(zenith_deg >= 0.0 && zenith_deg < 90.0) || !std::isfinite(azimuth_deg))
+    return fail(c, RT_EINVAL, "rt_trace: zenith must be in [0, 90) degrees and azimuth finite");
+  DeviceGuard guard(c->device);
+  cudaStream_t st = (cudaStream_t)stream_v;
+  rt::TraceArgs A;
+  A.nx = c->nx; A.ny = c->ny; A.nz = c->nz; A.bx = c->bx; A.by = c->by; A.bz = c->bz;
+  A.ncx = c->ncx; A.ncy = c->ncy; A.ncz = c->ncz;
+  A.dx = c->dx; A.dy = c->dy; A.dz = c->dz;
+  A.rdx = 1.0f / c->dx; A.rdy = 1.0f / c->dy; A.rdz = 1.0f / c->dz;
+  A.Lx = (float)c->bx * c->dx; A.Ly = (float)c->by * c->dy; A.Lz = (float)c->bz * c->dz;
+  // sun direction evaluated in double on the host, rounded once to fp32
+  const double deg = 3.14159265358979323846 / 180.0;
+  const double th = zenith_deg * deg, ph = azimuth_deg * deg;
+  A.sun_x = (float)(-std::sin(th) * std::sin(ph));
+  A.sun_y = (float)(-std::sin(th) * std::cos(ph));
+  A.sun_z = (float)(-std::cos(th));
+  A.optics = c->optics; A.khat = c->khat; A.albedo = c->albedo;
+  A.atm_abs = tally_ptr(c, 0); A.sfc_dir = tally_ptr(c, 1); A.sfc_dif = tally_ptr(c, 2);
+  A.sfc_abs = tally_ptr(c, 3); A.toa_up = tally_ptr(c, 4);
+  A.counters = c->counters; A.next_photon = c->counters + rt::C_COUNT;
+  A.records = records;
+  A.n_photons = n_photons; A.first_id = first_id; A.ncol = c->ncol;
+  A.n_full = (n_photons / c->ncol) * c->ncol;
+  A.key0 = (uint32_t)seed; A.key1 = (uint32_t)(seed >> 32); A.stream_id = stream_id;
+  RT_CUDA(c, cudaMemsetAsync(A.next_photon, 0, sizeof(unsigned long long), st));
+  RT_CUDA(c, cudaEventRecord(c->ev0, st));
+  if (n_photons > 0) {
+    if (records) rt::trace_kernel<true><<<c->trace_blocks_rec, rt::kTraceThreads, 0, st>>>(A);
+    else         rt::trace_kernel<false><<<c->trace_blocks, rt::kTraceThreads, 0, st>>>(A);
+    ++c->launches;
+  }
+  RT_CUDA(c, cudaEventRecord(c->ev1, st));
+  RT_CUDA(c, cudaGetLastError());
+  c->have_trace = true;
+  return RT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int rt_create_grid(rt_ctx** out, int nx, int ny, int nz, float dx, float dy, float dz, int bx, int by,
+                   int bz, int cuda_device) {
+  if (!out) return RT_EINVAL;
+  *out = nullptr;
+  if (nx <= 0 || ny <= 0 || nz <= 0 || bx <= 0 || by <= 0 || bz <= 0) return RT_EINVAL;
+  if (nx % bx || ny % by || nz % bz || (long long)bx * by * bz > 4096) return RT_EINVAL;
+  if (!(dx > 0.0f) || !(dy > 0.0f) || !(dz > 0.0f)) return RT_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || cuda_device < 0 || cuda_device >= ndev) return RT_ECUDA;
+  rt_ctx* c = new rt_ctx();
+  c->device = cuda_device;
+  c->nx = nx; c->ny = ny; c->nz = nz; c->bx = bx; c->by = by; c->bz = bz;
+  c->ncx = nx / bx; c->ncy = ny / by; c->ncz = nz / bz;
+  c->dx = dx; c->dy = dy; c->dz = dz;
+  c->nvox = (size_t)nx * ny * nz; c->ncol = (size_t)nx * ny; c->ncell = (size_t)c->ncx * c->ncy * c->ncz;
+  *out = c;  // returned even on failure so rt_last_error works; caller still calls rt_destroy
+  DeviceGuard guard(cuda_device);
+  const size_t ntally = c->nvox + 4 * c->ncol;
+  RT_CUDA(c, cudaMalloc(&c->optics, c->nvox * sizeof(float4)));
+  RT_CUDA(c, cudaMalloc(&c->khat, c->ncell * sizeof(float)));
+  RT_CUDA(c, cudaMalloc(&c->albedo, c->ncol * sizeof(float)));
+  RT_CUDA(c, cudaMalloc(&c->tallies, ntally * sizeof(unsigned long long)));
+  RT_CUDA(c, cudaMalloc(&c->counters, (rt::C_COUNT + 1) * sizeof(unsigned long long)));
+  RT_CUDA(c, cudaMalloc(&c->bad, sizeof(int)));
+  RT_CUDA(c, cudaMalloc(&c->sink, sizeof(float)));
+  RT_CUDA(c, cudaMemset(c->tallies, 0, ntally * sizeof(unsigned long long)));
+  RT_CUDA(c, cudaMemset(c->counters, 0, (rt::C_COUNT + 1) * sizeof(unsigned long long)));
+  RT_CUDA(c, cudaEventCreate(&c->ev0));
+  RT_CUDA(c, cudaEventCreate(&c->ev1));
+  RT_CUDA(c, cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, cuda_device));
+  int per_sm = 0;
+  RT_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rt::trace_kernel<false>, rt::kTraceThreads, 0));
+  c->trace_blocks = c->sm_count * (per_sm > 0 ? per_sm : 1);
+  RT_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rt::trace_kernel<true>, rt::kTraceThreads, 0));
+  c->trace_blocks_rec = c->sm_count * (per_sm > 0 ? per_sm : 1);
+  return RT_OK;
+}
+
+int rt_set_optics(rt_ctx* c, const float* k_ext, const float* k_ext_cloud, const float* ssa, const float* g,
+                  const float* sfc_albedo, void* cuda_stream) {
+  if (!c) return RT_EINVAL;
+  if (!k_ext || !k_ext_cloud || !ssa || !g || !sfc_albedo) return fail(c, RT_EINVAL, "rt_set_optics: NULL field");
+  DeviceGuard guard(c->device);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  c->have_optics = false;
+  RT_CUDA(c, cudaMemsetAsync(c->bad, 0, sizeof(int), st));
+  RT_CUDA(c, cudaMemsetAsync(c->khat, 0, c->ncell * sizeof(float), st));
+  RT_CUDA(c, cudaMemcpyAsync(c->albedo, sfc_albedo, c->ncol * sizeof(float), cudaMemcpyDeviceToDevice, st));
+  const int blocks = c->sm_count * 8;
+  rt::pack_optics_kernel<<<blocks, 256, 0, st>>>(k_ext, k_ext_cloud, ssa, g, c->optics, (int*)c->khat, c->nx,
+                                                c->ny, c->nz, c->bx, c->by, c->bz, c->bad);
+  rt::check_albedo_kernel<<<c->sm_count, 256, 0, st>>>(c->albedo, c->ncol, c->bad);
+  c->launches += 2;
+  RT_CUDA(c, cudaGetLastError());
+  int bad = 0;
+  RT_CUDA(c, cudaMemcpyAsync(&bad, c->bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+  RT_CUDA(c, cudaStreamSynchronize(st));
+  if (bad) {
+    char msg[160];
+    snprintf(msg, sizeof msg, "rt_set_optics: input out of range (mask 0x%x: 1 k_ext, 2 k_ext_cloud, 4 ssa, 8 g, 16 albedo)", bad);
+    return fail(c, RT_EOPTICS, msg);
+  }
+  c->have_optics = true;
+  return RT_OK;
+}
+
+int rt_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photons, uint64_t first_photon_id,
+             uint64_t seed, uint32_t stream_id, void* cuda_stream) {
+  return do_trace(c, zenith_deg, azimuth_deg, n_photons, first_photon_id, seed, stream_id, cuda_stream, nullptr);
+}
+
+int rt_trace_records(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photons,
+                     uint64_t first_photon_id, uint64_t seed, uint32_t stream_id, void* cuda_stream,
+                     uint32_t* records_out) {
+  if (c && !records_out && n_photons) return fail(c, RT_EINVAL, "rt_trace_records: NULL records_out");
+  return do_trace(c, zenith_deg, azimuth_deg, n_photons, first_photon_id, seed, stream_id, cuda_stream, records_out);
+}
+
+int rt_read_tallies(rt_ctx* c, int64_t* atm_abs, int64_t* sfc_dir, int64_t* sfc_dif, int64_t* sfc_abs,
+                    int64_t* toa_up, rt_counters* counters) {
+  if (!c) return RT_EINVAL;
+  DeviceGuard guard(c->device);
+  RT_CUDA(c, cudaDeviceSynchronize());
+  int64_t* outs[5] = {atm_abs, sfc_dir, sfc_dif, sfc_abs, toa_up};
+  for (int k = 0; k < 5; ++k)
+    if (outs[k])
+      RT_CUDA(c, cudaMemcpy(outs[k], tally_ptr(c, k), (k == 0 ? c->nvox : c->ncol) * sizeof(int64_t), cudaMemcpyDefault));
+  if (counters) {
+    unsigned long long h[rt::C_COUNT];
+    RT_CUDA(c, cudaMemcpy(h, c->counters, sizeof h, cudaMemcpyDeviceToHost));
+    counters->n_null = h[rt::C_NULL]; counters->n_rayleigh = h[rt::C_RAY]; counters->n_hg = h[rt::C_HG];
+    counters->n_atm_abs = h[rt::C_ATM_ABS]; counters->n_sfc_hits = h[rt::C_SFC_HITS];
+    counters->n_sfc_abs = h[rt::C_SFC_ABS]; counters->n_toa = h[rt::C_TOA]; counters->n_capped = h[rt::C_CAPPED];
+    counters->n_cell_steps = h[rt::C_CELLS]; counters->capped_energy = (int64_t)h[rt::C_CAPPED_E];
+    counters->n_events = h[rt::C_NULL] + h[rt::C_RAY] + h[rt::C_HG] + h[rt::C_ATM_ABS];
+    counters->n_photons = h[rt::C_ATM_ABS] + h[rt::C_SFC_ABS] + h[rt::C_TOA] + h[rt::C_CAPPED];
+  }
+  return RT_OK;
+}
+
+int rt_reset_tallies(rt_ctx* c, void* cuda_stream) {
+  if (!c) return RT_EINVAL;
+  DeviceGuard guard(c->device);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  RT_CUDA(c, cudaMemsetAsync(c->tallies, 0, (c->nvox + 4 * c->ncol) * sizeof(unsigned long long), st));
+  RT_CUDA(c, cudaMemsetAsync(c->counters, 0, (rt::C_COUNT + 1) * sizeof(unsigned long long), st));
+  return RT_OK;
+}
+
+int rt_read_majorant(rt_ctx* c, float* khat_out) {
+  if (!c || !khat_out) return RT_EINVAL;
+  DeviceGuard guard(c->device);
+  RT_CUDA(c, cudaDeviceSynchronize());
+  RT_CUDA(c, cudaMemcpy(khat_out, c->khat, c->ncell * sizeof(float), cudaMemcpyDefault));
+  return RT_OK;
+}
+
+int rt_read_packed_optics(rt_ctx* c, float* packed_out) {
+  if (!c || !packed_out) return RT_EINVAL;
+  DeviceGuard guard(c->device);
+  RT_CUDA(c, cudaDeviceSynchronize());
+  RT_CUDA(c, cudaMemcpy(packed_out, c->optics, c->nvox * sizeof(float4), cudaMemcpyDefault));
+  return RT_OK;
+}
+
+int rt_gather_bench(rt_ctx* c, uint32_t loads_per_thread, void* cuda_stream, float* ms_out, uint64_t* n_loads_out) {
+  if (!c || !ms_out || !n_loads_out || loads_per_thread < 8) return RT_EINVAL;
+  DeviceGuard guard(c->device);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const uint32_t iters = loads_per_thread / 8;
+  const int blocks = c->sm_count * 8, threads = 256;
+  cudaEvent_t a, b;
+  RT_CUDA(c, cudaEventCreate(&a));
+  RT_CUDA(c, cudaEventCreate(&b));
+  RT_CUDA(c, cudaEventRecord(a, st));
+  rt::gather_bench_kernel<<<blocks, threads, 0, st>>>(c->optics, (unsigned long long)c->nvox, iters, c->sink);
+  ++c->launches;
+  RT_CUDA(c, cudaEventRecord(b, st));
+  RT_CUDA(c, cudaEventSynchronize(b));
+  RT_CUDA(c, cudaGetLastError());
+  RT_CUDA(c, cudaEventElapsedTime(ms_out, a, b));
+  cudaEventDestroy(a);
+  cudaEventDestroy(b);
+  *n_loads_out = (uint64_t)blocks * threads * iters * 8ull;
+  return RT_OK;
+}
+
+int rt_last_trace_ms(rt_ctx* c, float* ms_out) {
+  if (!c || !ms_out) return RT_EINVAL;
+  if (!c->have_trace) return fail(c, RT_ESTATE, "rt_last_trace_ms: no rt_trace call yet");
+  DeviceGuard guard(c->device);
+  RT_CUDA(c, cudaEventSynchronize(c->ev1));
+  RT_CUDA(c, cudaEventElapsedTime(ms_out, c->ev0, c->ev1));
+  return RT_OK;
+}
+
+uint64_t rt_launch_count(const rt_ctx* c) { return c ? c->launches : 0; }
+
+int rt_philox_words(int cuda_device, const uint32_t* ctr, uint32_t key0, uint32_t key1, uint32_t* out, uint64_t n) {
+  if (!ctr || !out) return RT_EINVAL;
+  DeviceGuard guard(cuda_device);
+  if (n == 0) return RT_OK;
+  rt::philox_words_kernel<<<296, 256>>>((const uint4*)ctr, key0, key1, (uint4*)out, n);
+  if (cudaGetLastError() != cudaSuccess || cudaDeviceSynchronize() != cudaSuccess) return RT_ECUDA;
+  return RT_OK;
+}
+
+const char* rt_last_error(const rt_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+void rt_destroy(rt_ctx* c) {
+  if (!c) return;
+  {
+    DeviceGuard guard(c->device);
+    cudaDeviceSynchronize();
+    cudaFree(c->optics); cudaFree(c->khat); cudaFree(c->albedo); cudaFree(c->tallies);
+    cudaFree(c->counters); cudaFree(c->bad); cudaFree(c->sink);
+    if (c->ev0) cudaEventDestroy(c->ev0);
+    if (c->ev1) cudaEventDestroy(c->ev1);
+  }
+  delete c;
+}
+
+}  // extern "C"

@@ -1,0 +1,93 @@
+// rt_setup.cuh — set-up kernels run by rt_set_optics and the random-gather
+// microbenchmark behind rt_gather_bench.
+#pragma once
+#include "rt_device.cuh"
+
+namespace rt {
+
+// §3.4 pack cumulative coefficients; §3.5 majorant = highest extinction coefficient in each
+// acceleration cell.  One thread per voxel, x fastest, so loads and the float4 store are
+// coalesced.  Non-negative floats order like their bit patterns, so the cell maximum is an
+// integer atomicMax (exact).  `bad` receives a bit mask of violated input ranges.
+__global__ void pack_optics_kernel(const float* __restrict__ k_ext, const float* __restrict__ k_cloud,
+                                   const float* __restrict__ ssa, const float* __restrict__ g,
+                                   float4* __restrict__ optics, int* __restrict__ khat_bits, int nx, int ny,
+                                   int nz, int bx, int by, int bz, int* __restrict__ bad) {
+  const size_t nvox = (size_t)nx * ny * nz;
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  const int ncx = nx / bx, ncy = ny / by;
+  for (size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x; v < nvox; v += stride) {
+    const float k = k_ext[v], kc = k_cloud[v], w = ssa[v], gg = g[v];
+    int flags = 0;
+    if (!(k >= 0.0f) || isinf(k)) flags |= 1;
+    if (!(kc >= 0.0f) || !(kc <= k)) flags |= 2;
+    if (!(w >= 0.0f) || !(w <= 1.0f)) flags |= 4;
+    if (!(fabsf(gg) < 1.0f)) flags |= 8;
+    if (flags) atomicOr(bad, flags);
+    float c3 = k;
+    float c1 = (1.0f - w) * k;
+    const float frac = (k > 0.0f) ? kc / k : 0.0f;
+    float c2 = c1 + (w * k) * frac;
+    c2 = fminf(c2, c3);
+    c1 = fminf(c1, c2);
+    optics[v] = make_float4(c1, c2, c3, gg);
+    const int x = (int)(v % nx), y = (int)((v / nx) % ny), z = (int)(v / ((size_t)nx * ny));
+    const int cell = ((z / bz) * ncy + (y / by)) * ncx + (x / bx);
+    // lanes of a warp that share a cell: reduce before the atomic
+    const unsigned act = __activemask();
+    const unsigned peers = __match_any_sync(act, cell);
+    int m = flags ? 0 : __float_as_int(k);
+    const int leader = __ffs(peers) - 1;
+    for (int off = 16; off > 0; off >>= 1) {
+      const int o = __shfl_down_sync(act, m, off);
+      const unsigned src = (threadIdx.x & 31u) + off;
+      if (src < 32u && ((peers >> src) & 1u)) m = max(m, o);
+    }
+    // shfl_down reduction is only complete when peers are contiguous; contiguous x runs are,
+    // but guard the general case with a per-lane atomic when they are not.
+    const unsigned run = peers >> leader;
+    const bool contiguous = (run & (run + 1u)) == 0u;
+    if (contiguous) {
+      if ((int)(threadIdx.x & 31u) == leader) atomicMax(&khat_bits[cell], m);
+    } else {
+      atomicMax(&khat_bits[cell], flags ? 0 : __float_as_int(k));
+    }
+  }
+}
+
+__global__ void check_albedo_kernel(const float* __restrict__ albedo, size_t ncol, int* __restrict__ bad) {
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < ncol; c += stride) {
+    const float a = albedo[c];
+    if (!(a >= 0.0f) || !(a <= 1.0f)) atomicOr(bad, 16);
+  }
+}
+
+// Random 16-byte gathers over the packed-optics array: 8 independent loads in flight per thread.
+__global__ void gather_bench_kernel(const float4* __restrict__ optics, unsigned long long nvox,
+                                    uint32_t iters, float* __restrict__ sink) {
+  const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
+  float acc = 0.0f;
+  for (uint32_t it = 0; it < iters; ++it) {
+    const uint4 a = philox4x32_10(tid, it, 0u, 0x9a7e12u, 7u, 11u);
+    const uint4 b = philox4x32_10(tid, it, 1u, 0x9a7e12u, 7u, 11u);
+    const uint32_t w[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+    float4 v[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) v[j] = __ldg(&optics[(size_t)(((unsigned long long)w[j] * nvox) >> 32)]);
+#pragma unroll
+    for (int j = 0; j < 8; ++j) acc += v[j].x + v[j].w;
+  }
+  if (acc == -1.2345f) sink[0] = acc;
+}
+
+__global__ void philox_words_kernel(const uint4* __restrict__ ctr, uint32_t k0, uint32_t k1,
+                                    uint4* __restrict__ out, unsigned long long n) {
+  const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+  for (unsigned long long j = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += stride) {
+    const uint4 c = ctr[j];
+    out[j] = philox4x32_10(c.x, c.y, c.z, c.w, k0, k1);
+  }
+}
+
+}  // namespace rt
