@@ -1,0 +1,306 @@
+"""bench.py — throughput of the photon-tracing hot path (BASELINE.json metric) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over the 512x512x128 seeded
+cumulus field (BASELINE.json configs[2]): rt_reset_tallies, rt_set_optics (pack + majorant),
+rt_trace of 2^26 photons, rt_read_tallies (counters + the four column tallies; atm_abs stays on the
+device for the device-timed value, and comes to the host in the e2e leg).  Prints ONE JSON line.
+
+--impl reference times the CPU oracle (oracle/), as it stands, on a bounded sample of the same
+workload on the box's host cores.  It is a deliberately slow checker, not a target.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+WORKLOAD = 3                      # rt_inputs.CONFIGS key: BASELINE.json configs[2], 512x512x128
+METRIC = "photon_paths_per_s"
+UNIT = "paths/s"
+REF_SAMPLE_PHOTONS = 1 << 20      # per --impl reference step: 4 photons per column
+CPU_BASELINE_PHOTONS = 1 << 22    # cpu_baseline leg: 16 photons per column (~20 s on 8 cores)
+SECTOR = 32                       # bytes moved per random 16-byte gather (one DRAM/L2 sector)
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, uuid=None):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        cmd = ["nvidia-smi", "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "200"]
+        if uuid:
+            cmd += ["-i", uuid]
+        try:
+            self.p = subprocess.Popen(cmd, stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, smax, power, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in self.f.read().splitlines():
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); smax.append(float(parts[1])); power.append(float(parts[2]))
+            except ValueError:
+                continue
+            for name, v in zip(names, parts[3:7]):
+                if v.lower() == "active":
+                    reasons.add(name)
+        self.f.close()
+        os.unlink(self.f.name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def run_reference(args):
+    """The oracle on the host cores; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import oracle as O
+    from rt_inputs import CONFIGS, make_optics
+    cfg = CONFIGS[WORKLOAD]
+    opt = make_optics(cfg)
+    cores = O.hardware_threads()
+    n = REF_SAMPLE_PHOTONS
+    times, events = [], 0
+    for step in range(args.warmup + args.steps):
+        t, _, el = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, first_photon_id=step * n,
+                           seed=cfg.seed, precision=64, n_threads=cores)
+        assert t.closure() == n * O.W0
+        if step >= args.warmup:
+            times.append(el)
+            events += t.counters.n_events
+    total = sum(times)
+    value = n * len(times) / total
+    sample = "%d photons per step (%.0f per column) of the %d-photon workload, photon loop only" % (
+        n, n / cfg.ncol, cfg.n_photons)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "collision_events_per_s": events / total,
+        "config": {"workload": cfg.name, "grid": [cfg.nx, cfg.ny, cfg.nz], "photons_per_step": n,
+                   "block": list(cfg.block), "zenith_deg": cfg.zenith_deg, "azimuth_deg": cfg.azimuth_deg},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2208_05247_b200 as rt          # raises if the CUDA library is missing: no CPU fallback
+    from rt_inputs import CONFIGS, make_optics
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def max_over_ranks(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def sum_over_ranks(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        return float(t.item())
+
+    cfg = CONFIGS[WORKLOAD]
+    opt = make_optics(cfg)                       # seeded: every rank builds the same field
+    names = ("k_ext", "k_ext_cloud", "ssa", "g", "sfc_albedo")
+    host = [torch.from_numpy(opt[k]).pin_memory() for k in names]
+    resident = [t.to(dev) for t in host]
+    n = cfg.n_photons                            # per GPU (weak scaling: photon ids are sharded by rank)
+    g = rt.Grid(*cfg.grid, device=local)
+    pinned_cols = rt.Tallies(None, *[torch.empty((cfg.ny, cfg.nx), dtype=torch.int64).pin_memory() for _ in range(4)],
+                             counters=None)
+    pinned_all = rt.Tallies(torch.empty((cfg.nz, cfg.ny, cfg.nx), dtype=torch.int64).pin_memory(),
+                            pinned_cols.sfc_dir, pinned_cols.sfc_dif, pinned_cols.sfc_abs, pinned_cols.toa_up,
+                            counters=None)
+
+    def step(i, fields, out):
+        g.reset_tallies()
+        g.set_optics(*fields)                                    # S0 pack, S1 majorant
+        g.trace(cfg.zenith_deg, cfg.azimuth_deg, n, first_photon_id=(i * world + rank) * n, seed=cfg.seed)  # S2-S10
+        t = g.read_tallies(out=out)                              # S11
+        if t.counters.n_photons != n or t.counters.n_capped != 0:
+            raise SystemExit("bench.py: photon count mismatch (%d of %d, %d capped)" % (
+                t.counters.n_photons, n, t.counters.n_capped))
+        return t, g.last_trace_ms()
+
+    for i in range(args.warmup):
+        step(i, resident, pinned_cols)
+
+    # ---- device-timed region: inputs resident in HBM ---------------------------------------------------
+    uuid = None
+    try:
+        uuid = "GPU-" + str(torch.cuda.get_device_properties(dev).uuid)
+    except Exception:
+        pass
+    sampler = ClockSampler(uuid) if rank == 0 else None
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches0 = g.launch_count()
+    events = sfc_hits = 0
+    trace_ms = []
+    barrier()
+    e0.record()
+    for i in range(args.steps):
+        t, ms = step(args.warmup + i, resident, pinned_cols)
+        events += t.counters.n_events
+        sfc_hits += t.counters.n_sfc_hits
+        trace_ms.append(ms)
+    e1.record()
+    barrier()
+    elapsed_ms = max_over_ranks(e0.elapsed_time(e1))
+    launches = g.launch_count() - launches0
+    clocks = sampler.stop() if sampler else None
+    closure_ok = (int(t.sfc_abs.sum()) + int(t.toa_up.sum()) + t.counters.n_atm_abs * rt.W0 == n * rt.W0)
+
+    total_photons = n * world * args.steps
+    total_events = sum_over_ranks(events)
+    value = total_photons / (elapsed_ms * 1e-3)
+
+    # ---- end-to-end leg: host fields in, all tallies out to the host, every step --------------------------
+    step(0, host, pinned_all)
+    barrier()
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        step(args.warmup + args.steps + i, host, pinned_all)
+    barrier()
+    e2e_s = max_over_ranks(time.perf_counter() - t0)
+    h2d = sum(x.numel() * x.element_size() for x in host)
+    d2h = (cfg.nvox + 4 * cfg.ncol) * 8 + 8 * len(rt.binding.COUNTER_FIELDS)
+
+    # ---- roofline of the dominant kernel (trace_kernel), this rank ---------------------------------------
+    peak, peak_src = _peaks()
+    ms_avg = sum(trace_ms) / len(trace_ms)
+    ev_per_launch = events / args.steps
+    atomics_per_launch = n + sfc_hits / args.steps
+    alg_bytes = SECTOR * ev_per_launch + 2 * SECTOR * atomics_per_launch
+    achieved = alg_bytes / (ms_avg * 1e-3) / 1e9
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "trace_kernel_traffic.json")
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            tj = json.load(f)
+        if tj.get("n_photons") == n and tj.get("workload") == cfg.name:
+            traffic = tj.get("dram_bytes_per_launch")
+    gb_ms, gb_loads = g.gather_bench(64)
+    gather_sectors_per_s = gb_loads / (gb_ms * 1e-3)
+    trace_events_per_s = ev_per_launch / (ms_avg * 1e-3)
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        import oracle as O
+        cores = O.hardware_threads()
+        ot, _, el = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, CPU_BASELINE_PHOTONS, seed=cfg.seed,
+                            precision=64, n_threads=cores)
+        cpu = {"value": CPU_BASELINE_PHOTONS / el, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "collision_events_per_s": ot.counters.n_events / el,
+               "sample": "photon ids [0, %d) (%d per column) of the %d-photon workload, photon loop only" % (
+                   CPU_BASELINE_PHOTONS, CPU_BASELINE_PHOTONS // cfg.ncol, n)}
+
+    print(json.dumps({
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "collision_events_per_s": total_events / (elapsed_ms * 1e-3),
+        "events_per_photon": total_events / total_photons,
+        "trace_kernel": {"ms": ms_avg, "paths_per_s": n / (ms_avg * 1e-3), "events_per_s": trace_events_per_s},
+        "config": {"workload": cfg.name, "grid": [cfg.nx, cfg.ny, cfg.nz], "photons_per_gpu_per_step": n,
+                   "block": list(cfg.block), "zenith_deg": cfg.zenith_deg, "azimuth_deg": cfg.azimuth_deg,
+                   "parallelism": "photon-id ranges per GPU, no collective" if world > 1 else "1 GPU",
+                   "l2": "inputs exceed L2 (512 MiB packed optics + 256 MiB tallies vs 126 MB)",
+                   "step": "reset_tallies + set_optics + trace + read_tallies(column tallies, counters)"},
+        "e2e": {"value": total_photons / e2e_s, "unit": UNIT, "ms_per_step": 1e3 * e2e_s / args.steps,
+                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+        "gpu_launches": launches,
+        "closure_exact": bool(closure_ok),
+        "clocks": clocks,
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": traffic, "kernel": "trace_kernel", "peak_source": peak_src,
+                     "algorithmic_bytes_per_launch": alg_bytes,
+                     "bytes_model": "32 B sector per collision event + 2 x 32 B per tally atomic"},
+        "gather_roofline": {"sectors_per_s": gather_sectors_per_s, "GBps_32B": gather_sectors_per_s * SECTOR / 1e9,
+                            "trace_events_per_s": trace_events_per_s,
+                            "frac": trace_events_per_s / gather_sectors_per_s,
+                            "how": "rt_gather_bench: 8 independent random 16 B loads in flight per thread over the "
+                                   "512 MiB packed-optics array"},
+        "cpu_baseline": cpu,
+    }))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
+    ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing (used under ncu)")
+    args = ap.parse_args()
+    if args.steps < 1 or args.warmup < 0:
+        raise SystemExit("bench.py: --steps >= 1, --warmup >= 0")
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

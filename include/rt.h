@@ -61,9 +61,11 @@ int rt_create_grid(rt_ctx** out, int nx, int ny, int nz, float dx, float dy, flo
                    int bz, int cuda_device);
 
 /* Set the optical properties of one spectral point (k_ext, k_ext,cloud, omega0, g as 3D
- * fields; P:56 local surface albedo).  All five are DEVICE pointers owned by the caller, fp32,
- * nvox / nvox / nvox / nvox / ncol elements; they are read on `cuda_stream` (a cudaStream_t, NULL =
- * default stream) and may be freed once the stream has passed this call.  Packs cumulative
+ * fields; P:56 local surface albedo).  All five are owned by the caller, fp32, nvox / nvox / nvox /
+ * nvox / ncol elements, each a DEVICE pointer (read in place) or a HOST pointer (detected; copied to a
+ * device staging buffer on the stream first -- pinned memory makes that copy asynchronous).  They are
+ * read on `cuda_stream` (a cudaStream_t, NULL = default stream) and may be freed once this call returns
+ * (it synchronises the stream).  Packs cumulative
  * coefficients and builds the majorant grid (§3.5).  Validates k_ext >= 0 and
  * finite, 0 <= k_ext_cloud <= k_ext, 0 <= ssa <= 1, |g| < 1, 0 <= albedo <= 1 on the device;
  * a violation returns RT_EOPTICS (this call synchronises the stream to learn it). */

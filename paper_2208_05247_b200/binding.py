@@ -110,10 +110,13 @@ class Grid:
         if rc != 0:
             raise RtError("%s failed (%d): %s" % (name, rc, self.L.rt_last_error(self.ctx).decode()))
 
-    def _dev32(self, a, n):
+    def _f32(self, a, n):
+        """fp32 contiguous tensor on this device or on the host (the library copies host fields itself)."""
         t = torch.as_tensor(a)
-        if t.dtype != torch.float32 or t.device != self.device or not t.is_contiguous():
-            t = t.to(device=self.device, dtype=torch.float32).contiguous()
+        if t.is_cuda and t.device != self.device:
+            t = t.to(self.device)
+        if t.dtype != torch.float32 or not t.is_contiguous():
+            t = t.to(dtype=torch.float32).contiguous()
         if t.numel() != n:
             raise RtError("field has %d elements, expected %d" % (t.numel(), n))
         return t
@@ -121,8 +124,8 @@ class Grid:
     def set_optics(self, k_ext, k_ext_cloud, ssa, g, sfc_albedo):
         nz, ny, nx = self.shape
         nvox, ncol = nx * ny * nz, nx * ny
-        ts = [self._dev32(k_ext, nvox), self._dev32(k_ext_cloud, nvox), self._dev32(ssa, nvox),
-              self._dev32(g, nvox), self._dev32(sfc_albedo, ncol)]
+        ts = [self._f32(k_ext, nvox), self._f32(k_ext_cloud, nvox), self._f32(ssa, nvox),
+              self._f32(g, nvox), self._f32(sfc_albedo, ncol)]
         self._check(self.L.rt_set_optics(self.ctx, *[_ptr(t) for t in ts], _stream(self.device)), "rt_set_optics")
 
     def trace(self, zenith_deg, azimuth_deg, n_photons, first_photon_id=0, seed=1, stream_id=0, records=False):
@@ -136,11 +139,15 @@ class Grid:
                                     int(seed), int(stream_id), _stream(self.device)), "rt_trace")
         return None
 
-    def read_tallies(self, host=True, atm_abs=True):
+    def read_tallies(self, host=True, atm_abs=True, out=None):
+        """Copy tallies out.  `out` = an earlier Tallies whose (e.g. pinned host) buffers are reused."""
         nz, ny, nx = self.shape
-        kw = dict(dtype=torch.int64, device="cpu" if host else self.device)
-        a = torch.empty((nz, ny, nx), **kw) if atm_abs else None
-        cols = [torch.empty((ny, nx), **kw) for _ in range(4)]
+        if out is not None:
+            a, cols = out.atm_abs, [out.sfc_dir, out.sfc_dif, out.sfc_abs, out.toa_up]
+        else:
+            kw = dict(dtype=torch.int64, device="cpu" if host else self.device)
+            a = torch.empty((nz, ny, nx), **kw) if atm_abs else None
+            cols = [torch.empty((ny, nx), **kw) for _ in range(4)]
         cnt = rt_counters()
         self._check(self.L.rt_read_tallies(self.ctx, _ptr(a), *[_ptr(t) for t in cols], C.byref(cnt)), "rt_read_tallies")
         return Tallies(a, cols[0], cols[1], cols[2], cols[3], cnt)

@@ -22,6 +22,7 @@ struct rt_ctx {
   unsigned long long* counters = nullptr; // C_COUNT words, then the work counter
   int* bad = nullptr;
   float* sink = nullptr;
+  float* stage = nullptr;                 // 4 nvox + ncol floats; only allocated when a caller passes host fields
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   bool have_optics = false, have_trace = false;
   int trace_blocks = 0, trace_blocks_rec = 0, sm_count = 0;
@@ -53,6 +54,23 @@ int fail(rt_ctx* c, int code, const char* what, cudaError_t ce = cudaSuccess) {
 
 unsigned long long* tally_ptr(rt_ctx* c, int which) {  // 0 atm_abs, 1..4 the column tallies
   return which == 0 ? c->tallies : c->tallies + c->nvox + (size_t)(which - 1) * c->ncol;
+}
+
+// rt_set_optics accepts host fields too: they are copied to a device staging buffer on the stream.
+// Returns the device pointer to read from, or nullptr after recording an error.
+const float* stage_input(rt_ctx* c, const float* p, size_t n, size_t slot_offset, cudaStream_t st, int* rc) {
+  cudaPointerAttributes at;
+  cudaError_t ce = cudaPointerGetAttributes(&at, p);
+  if (ce != cudaSuccess) { cudaGetLastError(); at.type = cudaMemoryTypeUnregistered; }
+  if (at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged) return p;
+  if (!c->stage) {
+    ce = cudaMalloc(&c->stage, (4 * c->nvox + c->ncol) * sizeof(float));
+    if (ce != cudaSuccess) { *rc = fail(c, RT_ENOMEM, "rt_set_optics: staging buffer for host fields", ce); return nullptr; }
+  }
+  float* dst = c->stage + slot_offset;
+  ce = cudaMemcpyAsync(dst, p, n * sizeof(float), cudaMemcpyHostToDevice, st);
+  if (ce != cudaSuccess) { *rc = fail(c, RT_ECUDA, "rt_set_optics: host-to-device copy", ce); return nullptr; }
+  return dst;
 }
 
 int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photons, uint64_t first_id,
@@ -145,6 +163,12 @@ int rt_set_optics(rt_ctx* c, const float* k_ext, const float* k_ext_cloud, const
   DeviceGuard guard(c->device);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   c->have_optics = false;
+  int rc = RT_OK;
+  k_ext = stage_input(c, k_ext, c->nvox, 0, st, &rc);                      if (!k_ext) return rc;
+  k_ext_cloud = stage_input(c, k_ext_cloud, c->nvox, c->nvox, st, &rc);    if (!k_ext_cloud) return rc;
+  ssa = stage_input(c, ssa, c->nvox, 2 * c->nvox, st, &rc);                if (!ssa) return rc;
+  g = stage_input(c, g, c->nvox, 3 * c->nvox, st, &rc);                    if (!g) return rc;
+  sfc_albedo = stage_input(c, sfc_albedo, c->ncol, 4 * c->nvox, st, &rc);  if (!sfc_albedo) return rc;
   RT_CUDA(c, cudaMemsetAsync(c->bad, 0, sizeof(int), st));
   RT_CUDA(c, cudaMemsetAsync(c->khat, 0, c->ncell * sizeof(float), st));
   RT_CUDA(c, cudaMemcpyAsync(c->albedo, sfc_albedo, c->ncol * sizeof(float), cudaMemcpyDeviceToDevice, st));
@@ -275,7 +299,7 @@ void rt_destroy(rt_ctx* c) {
     DeviceGuard guard(c->device);
     cudaDeviceSynchronize();
     cudaFree(c->optics); cudaFree(c->khat); cudaFree(c->albedo); cudaFree(c->tallies);
-    cudaFree(c->counters); cudaFree(c->bad); cudaFree(c->sink);
+    cudaFree(c->counters); cudaFree(c->bad); cudaFree(c->sink); cudaFree(c->stage);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
   }
