@@ -155,6 +155,9 @@ def run_ours(args):
         return float(t.item())
 
     cfg = CONFIGS[WORKLOAD]
+    if args.block:
+        from dataclasses import replace
+        cfg = replace(cfg, block=tuple(int(x) for x in args.block.split(",")))
     opt = make_optics(cfg)                       # seeded: every rank builds the same field
     names = ("k_ext", "k_ext_cloud", "ssa", "g", "sfc_albedo")
     host = [torch.from_numpy(opt[k]).pin_memory() for k in names]
@@ -292,6 +295,7 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
+    ap.add_argument("--block", default=None, help="acceleration-grid block bx,by,bz (default: the config's)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing (used under ncu)")
     args = ap.parse_args()
     if args.steps < 1 or args.warmup < 0:

@@ -285,18 +285,31 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
       iy = std::min((int)(u3 * (R)ny), ny - 1);
     }
     int cx = ix / bx, cy = iy / by, cz = ncz - 1;
-    R qx = ((R)(ix % bx) + u0) * dx;
-    R qy = ((R)(iy % by) + u1) * dy;
-    R qz = Lz;
+    // Position inside the current acceleration cell is carried as the REMAINING DISTANCES rx, ry, rz
+    // along the flight direction to the cell's next face on each axis: a cell
+    // crossing subtracts the smallest one from the other two and resets its own to the face spacing
+    // del = L |1/v| exactly, so magnitudes never grow and rounding does not accumulate along a path.
+    // Local coordinates are recovered when needed as q = face - v r.
     R da = sun_x, db = sun_y, dc = sun_z;      // unit direction
     R va, vb, vc, ia, ib, ic;                  // nudged components and reciprocals
+    R delx, dely, delz;                        // distance between successive faces on each axis
+    R rx, ry, rz;                              // remaining distance to the next face on each axis
     auto set_dir = [&]() {
       va = (std::fabs(da) < TINY) ? TINY : da;
       vb = (std::fabs(db) < TINY) ? TINY : db;
       vc = (std::fabs(dc) < TINY) ? TINY : dc;
       ia = (R)1 / va; ib = (R)1 / vb; ic = (R)1 / vc;
+      delx = Lx * std::fabs(ia); dely = Ly * std::fabs(ib); delz = Lz * std::fabs(ic);
+    };
+    auto face = [&](R v, R L) { return (v > 0) ? L : (R)0; };
+    auto place = [&](R qx, R qy, R qz) {        // remaining distances from local coordinates
+      rx = (face(va, Lx) - qx) * ia; ry = (face(vb, Ly) - qy) * ib; rz = (face(vc, Lz) - qz) * ic;
+    };
+    auto local = [&](R v, R r, R L) {           // local coordinate from a remaining distance
+      return std::min(L, std::max((R)0, E::fma(-v, r, face(v, L))));
     };
     set_dir();
+    place(((R)(ix % bx) + u0) * dx, ((R)(iy % by) + u1) * dy, Lz);
     bool direct = true;
     uint32_t e = 1, n_ev = 0, n_sc = 0, n_sfc = 0;
     int fate = 0; uint32_t term = 0;
@@ -314,20 +327,17 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
     R rk = (kh > 0) ? (R)1 / kh : (R)0;
 
     while (fate == 0) {
-      // ---- step 5: distance to the nearest face of the current cell ---------
-      R fx = (va > 0) ? Lx : (R)0, fy = (vb > 0) ? Ly : (R)0, fz = (vc > 0) ? Lz : (R)0;
-      R tx = (fx - qx) * ia, ty = (fy - qy) * ib, tz = (fz - qz) * ic;
+      // ---- step 5: nearest face of the current cell; ties x < y < z -----------
       int axis; R t;
-      if (tx <= ty && tx <= tz) { axis = 0; t = tx; }
-      else if (ty <= tz)        { axis = 1; t = ty; }
-      else                      { axis = 2; t = tz; }
+      if (rx <= ry && rx <= rz) { axis = 0; t = rx; }
+      else if (ry <= rz)        { axis = 1; t = ry; }
+      else                      { axis = 2; t = rz; }
       R dtau = kh * t;
       if (kh > 0 && tau <= dtau) {
         // ---- step 7: tentative collision inside this cell -------------------
         R s = tau * rk;
-        qx = std::min(Lx, std::max((R)0, E::fma(va, s, qx)));
-        qy = std::min(Ly, std::max((R)0, E::fma(vb, s, qy)));
-        qz = std::min(Lz, std::max((R)0, E::fma(vc, s, qz)));
+        rx = std::max((R)0, rx - s); ry = std::max((R)0, ry - s); rz = std::max((R)0, rz - s);
+        R qx = local(va, rx, Lx), qy = local(vb, ry, Ly), qz = local(vc, rz, Lz);
         int lx = std::min((int)(qx * rdx), bx - 1);
         int ly = std::min((int)(qy * rdy), by - 1);
         int lz = std::min((int)(qz * rdz), bz - 1);
@@ -342,12 +352,12 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
         } else if (xi < v.c2) {                // cloud droplet: Henyey-Greenstein
           R mu = sample_hg<R>(v.g, u2);
           R sp, cp; E::sincos_2pi(u3, sp, cp);
-          rotate_dir<R>(da, db, dc, mu, cp, sp); set_dir();
+          rotate_dir<R>(da, db, dc, mu, cp, sp); set_dir(); place(qx, qy, qz);
           direct = false; ++n_sc; ++C.n_hg;
         } else if (xi < v.c3) {                // gas: Rayleigh
           R mu = sample_rayleigh<R>(u2);
           R sp, cp; E::sincos_2pi(u3, sp, cp);
-          rotate_dir<R>(da, db, dc, mu, cp, sp); set_dir();
+          rotate_dir<R>(da, db, dc, mu, cp, sp); set_dir(); place(qx, qy, qz);
           direct = false; ++n_sc; ++C.n_rayleigh;
         } else {
           ++C.n_null;                          // null collision: direction unchanged
@@ -360,22 +370,23 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
       } else {
         // ---- step 5 (cont.): leave the cell through `axis` -------------------
         tau = tau - dtau;
-        qx = std::min(Lx, std::max((R)0, E::fma(va, t, qx)));
-        qy = std::min(Ly, std::max((R)0, E::fma(vb, t, qy)));
-        qz = std::min(Lz, std::max((R)0, E::fma(vc, t, qz)));
         ++C.n_cell_steps;
         bool at_sfc = false, at_top = false;
         if (axis == 0) {
-          if (va > 0) { ++cx; if (cx == ncx) cx = 0; qx = (R)0; }
-          else        { --cx; if (cx < 0) cx = ncx - 1; qx = Lx; }
+          ry = ry - t; rz = rz - t; rx = delx;
+          if (va > 0) { ++cx; if (cx == ncx) cx = 0; }
+          else        { --cx; if (cx < 0) cx = ncx - 1; }
         } else if (axis == 1) {
-          if (vb > 0) { ++cy; if (cy == ncy) cy = 0; qy = (R)0; }
-          else        { --cy; if (cy < 0) cy = ncy - 1; qy = Ly; }
+          rx = rx - t; rz = rz - t; ry = dely;
+          if (vb > 0) { ++cy; if (cy == ncy) cy = 0; }
+          else        { --cy; if (cy < 0) cy = ncy - 1; }
         } else {
-          if (vc > 0) { ++cz; qz = (R)0; if (cz == ncz) at_top = true; }
-          else        { --cz; qz = Lz;   if (cz < 0) at_sfc = true; }
+          rx = rx - t; ry = ry - t; rz = delz;
+          if (vc > 0) { ++cz; if (cz == ncz) at_top = true; }
+          else        { --cz; if (cz < 0) at_sfc = true; }
         }
         if (at_sfc || at_top) {
+          R qx = local(va, rx, Lx), qy = local(vb, ry, Ly);
           int hx = cx * bx + std::min((int)(qx * rdx), bx - 1);
           int hy = cy * by + std::min((int)(qy * rdy), by - 1);
           size_t col = (size_t)hy * nx + hx;
@@ -390,7 +401,7 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
             R mu = std::sqrt((R)1 - u2), s = std::sqrt(u2);
             R sp, cp; E::sincos_2pi(u3, sp, cp);
             da = s * cp; db = s * sp; dc = mu; set_dir();
-            direct = false; cz = 0; qz = (R)0;
+            direct = false; cz = 0; place(qx, qy, (R)0);
             ++e;
             if (e > EVENT_CAP) {
               ++C.n_capped; C.capped_energy += W0; fate = ORC_CAPPED; term = 0; break;

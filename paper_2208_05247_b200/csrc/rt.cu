@@ -93,6 +93,8 @@ int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photon
   A.sun_x = (float)(-std::sin(th) * std::sin(ph));
   A.sun_y = (float)(-std::sin(th) * std::cos(ph));
   A.sun_z = (float)(-std::cos(th));
+  auto inv = [](float d) { return 1.0f / (std::fabs(d) < rt::kTiny ? rt::kTiny : d); };  // IEEE fp32, as set_inverse
+  A.sun_ix = inv(A.sun_x); A.sun_iy = inv(A.sun_y); A.sun_iz = inv(A.sun_z);
   A.optics = c->optics; A.khat = c->khat; A.albedo = c->albedo;
   A.atm_abs = tally_ptr(c, 0); A.sfc_dir = tally_ptr(c, 1); A.sfc_dif = tally_ptr(c, 2);
   A.sfc_abs = tally_ptr(c, 3); A.toa_up = tally_ptr(c, 4);

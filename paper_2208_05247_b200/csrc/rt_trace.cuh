@@ -1,7 +1,21 @@
 // rt_trace.cuh — the persistent photon-tracing kernel.
-// One thread carries one photon at a time; a warp draws photon ids in chunks from a global
-// counter and refills idle lanes with ballot/popc so lanes stay busy through the long tail of
-// in-cloud photons (BASELINE.json north_star: "compacted and regenerated persistently").
+//
+// One thread carries one photon at a time.  A photon is a small state machine:
+//   TRAVERSE  next thing to do is a step of the walk over acceleration cells (§3.7),
+//   COLLIDE   a tentative collision lies inside the current cell: fetch the voxel, classify (§3.8),
+//   SCATTER   a real scattering event was chosen: sample the angle and rotate (§3.9),
+//   DEAD      the lane is idle and waits for a new photon.
+// The phases have very different costs (a cell step is ~60 instructions, a collision with its Philox
+// draw and logarithm ~300, a scatter with its divisions and square roots ~200), and a scatter is chosen
+// by only ~7 % of the events: letting each lane take "its" branch every iteration runs the scatter code
+// in 84 % of the iterations with 2 of 32 lanes active (ncu, profiles/r1_baseline_*: 14.4 active threads
+// per instruction overall).  Instead the warp VOTES each iteration (ballot/popc) on one phase to run;
+// COLLIDE and TRAVERSE both end by probing the current cell for the next event, so a lane stays in its
+// state while it keeps colliding (in cloud) or keeps crossing (in clear air); SCATTER and the refill of
+// DEAD lanes run when enough lanes wait for them.  Dead lanes are refilled in batches from a
+// warp-private pool of photon ids taken in chunks from a global counter (BASELINE.json north_star:
+// "compacted and regenerated persistently with warp-level ballot/shuffle").  The per-photon sequence of
+// arithmetic operations is unchanged by the scheduling, so results do not depend on it.
 #pragma once
 #include "rt_device.cuh"
 
@@ -12,14 +26,28 @@ constexpr uint32_t kEventCap = 1u << 20;        // §3.12
 constexpr float kTiny = 1e-30f;                 // direction components are nudged away from 0
 constexpr int kTraceThreads = 256;
 constexpr int kChunk = 128;                     // photon ids a warp takes per global atomic
+#ifndef RT_REGEN_BATCH
+#define RT_REGEN_BATCH 6
+#endif
+#ifndef RT_SCATTER_BATCH
+#define RT_SCATTER_BATCH 6
+#endif
+#ifndef RT_TRAVERSE_WEIGHT
+#define RT_TRAVERSE_WEIGHT 2
+#endif
+constexpr int kRegenBatch = RT_REGEN_BATCH;       // refill when this many lanes are idle (or nothing else to do)
+constexpr int kScatterBatch = RT_SCATTER_BATCH;   // run SCATTER when this many lanes wait for it (or nothing else)
+constexpr int kTraverseWeight = RT_TRAVERSE_WEIGHT;  // TRAVERSE (cheap) runs when nT * weight >= nC
 
 enum Counter { C_NULL = 0, C_RAY, C_HG, C_ATM_ABS, C_SFC_HITS, C_SFC_ABS, C_TOA, C_CAPPED, C_CELLS,
                C_CAPPED_E, C_COUNT };
 
+enum : uint32_t { ST_DEAD = 0, ST_TRAVERSE = 1, ST_COLLIDE = 2, ST_SCATTER = 3 };
+
 struct TraceArgs {
   int nx, ny, nz, bx, by, bz, ncx, ncy, ncz;
   float dx, dy, dz, rdx, rdy, rdz, Lx, Ly, Lz;
-  float sun_x, sun_y, sun_z;
+  float sun_x, sun_y, sun_z, sun_ix, sun_iy, sun_iz;  // beam direction and 1/nudge(component), host-computed
   const float4* __restrict__ optics;   // [z][y][x] (c1, c2, c3, g)
   const float* __restrict__ khat;      // [cz][cy][cx]
   const float* __restrict__ albedo;    // [y][x]
@@ -39,6 +67,15 @@ __device__ __forceinline__ void tally_add(unsigned mask, unsigned long long* p) 
     atomicAdd(p, kW0 * (unsigned long long)__popc(peers));
 }
 
+__device__ __forceinline__ float nudge(float d) { return fabsf(d) < kTiny ? kTiny : d; }
+
+__device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+  return v;
+}
+
+
 template <bool kRecords>
 __global__ void __launch_bounds__(kTraceThreads) trace_kernel(const TraceArgs A) {
   __shared__ unsigned long long s_cnt[C_COUNT];
@@ -48,29 +85,73 @@ __global__ void __launch_bounds__(kTraceThreads) trace_kernel(const TraceArgs A)
   const unsigned lane = threadIdx.x & 31u;
   const unsigned lt_mask = (1u << lane) - 1u;
   unsigned long long pool_next = 0, pool_end = 0;  // warp-uniform chunk of photon indices
-  bool alive = false, exhausted = false;
+  bool exhausted = false;                          // warp-uniform: the global counter has run out
 
   // photon state
+  uint32_t st = ST_DEAD;
   unsigned long long i = 0;
   uint32_t p_lo = 0, p_hi = 0, e = 0;
   int cx = 0, cy = 0, cz = 0;
   float qx = 0, qy = 0, qz = 0, da = 0, db = 0, dc = -1, ia = 0, ib = 0, ic = 0;
-  float tau = 0, kh = 0, u1 = 0, u2 = 0, u3 = 0;
+  float tau = 0, kh = 0, u1 = 0;
+  float t = 0;                      // TRAVERSE: distance to the face the photon leaves the cell through
+  int axis = 3;                     // ... and that face's axis (3 = none: probe only, after a scatter)
+  uint32_t w2 = 0, w3 = 0;          // words 2, 3 of the current event's draw
+  uint32_t sw2 = 0, sw3 = 0;        // ... of the event that chose SCATTER (its draw is already replaced)
+  float sg = 0;                     // asymmetry parameter for the pending scatter; 2 = Rayleigh
   bool direct = true;
-  uint32_t n_ev = 0, n_sc = 0, n_hg = 0, n_sfc = 0, n_cells = 0;
+  bool fresh = false;               // just launched: in COLLIDE only to take its first draw
+  // event counts: running totals of this thread; a photon's own counts are differences (records)
+  uint32_t t_ev = 0, t_sc = 0, t_hg = 0, t_sfc = 0, t_cells = 0;
+  uint32_t b_ev = 0, b_sc = 0, b_sfc = 0;  // totals when the current photon was launched (records only)
+
+  auto draw = [&]() {
+    const uint4 X = philox4x32_10(p_lo, p_hi, e, A.stream_id, A.key0, A.key1);
+    tau = neg_log(1.0f - u24(X.x)); u1 = u24(X.y); w2 = X.z; w3 = X.w;
+  };
+  auto set_inverse = [&]() { ia = 1.0f / nudge(da); ib = 1.0f / nudge(db); ic = 1.0f / nudge(dc); };
+  // §3.7 first half: distance to the nearest face of the current cell (ties x < y < z) and whether the
+  // tentative collision falls before it.  Sets the lane's next state.
+  auto probe = [&]() {
+    const float tx = ((ia > 0.0f ? A.Lx : 0.0f) - qx) * ia;   // sign(ia) == sign(nudged component)
+    const float ty = ((ib > 0.0f ? A.Ly : 0.0f) - qy) * ib;
+    const float tz = ((ic > 0.0f ? A.Lz : 0.0f) - qz) * ic;
+    if (tx <= ty && tx <= tz) { axis = 0; t = tx; }
+    else if (ty <= tz)        { axis = 1; t = ty; }
+    else                      { axis = 2; t = tz; }
+    st = (kh > 0.0f && tau <= kh * t) ? ST_COLLIDE : ST_TRAVERSE;
+  };
+  auto flush_thread_counters = [&]() {
+    unsigned long long v;
+    v = warp_sum(t_sc - t_hg);  if (lane == 0 && v) atomicAdd(&s_cnt[C_RAY], v);
+    v = warp_sum(t_hg);         if (lane == 0 && v) atomicAdd(&s_cnt[C_HG], v);
+    v = warp_sum(t_sfc);        if (lane == 0 && v) atomicAdd(&s_cnt[C_SFC_HITS], v);
+    v = warp_sum(t_cells);      if (lane == 0 && v) atomicAdd(&s_cnt[C_CELLS], v);
+    // null = events - scatters - absorptions; absorptions are counted at the photon's end, so park the
+    // (events - scatters) part here and subtract C_ATM_ABS when the block folds its counters
+    v = warp_sum(t_ev - t_sc);  if (lane == 0 && v) atomicAdd(&s_cnt[C_NULL], v);
+  };
 
   for (;;) {
-    // ---- regeneration: refill idle lanes (converged) --------------------------------------
-    const unsigned need = __ballot_sync(0xffffffffu, !alive && !exhausted);
-    if (need) {
-      // hand out what the warp's pool has, then take one fresh chunk if lanes are still waiting
-      unsigned waiting = need;
+    const unsigned bT = __ballot_sync(0xffffffffu, st == ST_TRAVERSE);
+    const unsigned bC = __ballot_sync(0xffffffffu, st == ST_COLLIDE);
+    const unsigned bS = __ballot_sync(0xffffffffu, st == ST_SCATTER);
+    const unsigned live = bT | bC | bS;
+    int fate = 0;
+    uint32_t term = 0;
+    unsigned long long* tally_a = nullptr;  // arrival / terminal bin
+    unsigned long long* tally_b = nullptr;  // surface absorption after an arrival tally
+
+    if (!exhausted && (__popc(~live) >= kRegenBatch || !live)) {
+      // ---- regeneration: hand photon ids to the idle lanes -------------------------------------
+      unsigned waiting = ~live;
+      bool got = false;
 #pragma unroll 1
       for (int pass = 0; pass < 2 && waiting; ++pass) {
         const unsigned long long have = pool_end - pool_next;
         const unsigned rank = __popc(waiting & lt_mask);
         const bool mine = ((waiting >> lane) & 1u) && (unsigned long long)rank < have;
-        if (mine) { i = pool_next + rank; alive = true; }
+        if (mine) { i = pool_next + rank; got = true; }
         const unsigned took = __ballot_sync(0xffffffffu, mine);
         pool_next += __popc(took);
         waiting &= ~took;
@@ -83,18 +164,23 @@ __global__ void __launch_bounds__(kTraceThreads) trace_kernel(const TraceArgs A)
           if (pool_next > pool_end) pool_next = pool_end;
         }
       }
-      if ((waiting >> lane) & 1u) exhausted = true;
-
-      if (((need & ~waiting) >> lane) & 1u) {
-        // ---- §3.6 launch, event index 0 -----------------------------------------------------
+      if (waiting) exhausted = true;
+      if (__any_sync(0xffffffffu, t_ev > (1u << 30) || t_cells > (1u << 30))) {
+        flush_thread_counters();                   // keep the 32-bit running totals far from overflow
+        if (kRecords) { b_ev -= t_ev; b_sc -= t_sc; b_sfc -= t_sfc; }
+        t_ev = t_sc = t_hg = t_sfc = t_cells = 0;
+      }
+      if (got) {
+        // ---- §3.6 launch, event index 0 ------------------------------------------------------
         const unsigned long long pid = A.first_id + i;
         p_lo = (uint32_t)pid; p_hi = (uint32_t)(pid >> 32);
-        uint4 X = philox4x32_10(p_lo, p_hi, 0u, A.stream_id, A.key0, A.key1);
+        const uint4 X = philox4x32_10(p_lo, p_hi, 0u, A.stream_id, A.key0, A.key1);
         int ix, iy;
         if (i < A.n_full) {
-          const unsigned long long col = i % A.ncol;
-          ix = (int)(col % (unsigned long long)A.nx);
-          iy = (int)(col / (unsigned long long)A.nx);
+          // column = i mod ncol; 32-bit arithmetic whenever the index allows it
+          const uint32_t col = (i >> 32) ? (uint32_t)(i % A.ncol) : (uint32_t)i % (uint32_t)A.ncol;
+          ix = (int)(col % (uint32_t)A.nx);
+          iy = (int)(col / (uint32_t)A.nx);
         } else {
           ix = min((int)(u24(X.z) * (float)A.nx), A.nx - 1);
           iy = min((int)(u24(X.w) * (float)A.ny), A.ny - 1);
@@ -104,150 +190,158 @@ __global__ void __launch_bounds__(kTraceThreads) trace_kernel(const TraceArgs A)
         qy = ((float)(iy % A.by) + u24(X.y)) * A.dy;
         qz = A.Lz;
         da = A.sun_x; db = A.sun_y; dc = A.sun_z;
-        ia = 1.0f / (fabsf(da) < kTiny ? kTiny : da);
-        ib = 1.0f / (fabsf(db) < kTiny ? kTiny : db);
-        ic = 1.0f / (fabsf(dc) < kTiny ? kTiny : dc);
+        ia = A.sun_ix; ib = A.sun_iy; ic = A.sun_iz;
         direct = true;
-        e = 1; n_ev = n_sc = n_hg = n_sfc = n_cells = 0;
-        X = philox4x32_10(p_lo, p_hi, e, A.stream_id, A.key0, A.key1);
-        tau = neg_log(1.0f - u24(X.x)); u1 = u24(X.y); u2 = u24(X.z); u3 = u24(X.w);
+        e = 0;
+        if (kRecords) { b_ev = t_ev; b_sc = t_sc; b_sfc = t_sfc; }
         kh = __ldg(&A.khat[((size_t)cz * A.ncy + cy) * A.ncx + cx]);
+        fresh = true;                                // COLLIDE's tail draws event 1 and probes the cell
+        st = ST_COLLIDE;
       }
+      continue;
     }
-    if (!__any_sync(0xffffffffu, alive)) break;
+    if (!live) break;
 
-    // ---- one step of the photon: a cell crossing or a tentative collision ------------------
-    int fate = 0;
-    uint32_t term = 0;
-    unsigned long long* tally_a = nullptr;  // arrival / terminal bin
-    unsigned long long* tally_b = nullptr;  // surface absorption after an arrival tally
-    if (alive) {
-      const float va = fabsf(da) < kTiny ? kTiny : da;
-      const float vb = fabsf(db) < kTiny ? kTiny : db;
-      const float vc = fabsf(dc) < kTiny ? kTiny : dc;
-      // §3.7 distance to the nearest face of the current cell; ties x < y < z
-      const float tx = ((va > 0.0f ? A.Lx : 0.0f) - qx) * ia;
-      const float ty = ((vb > 0.0f ? A.Ly : 0.0f) - qy) * ib;
-      const float tz = ((vc > 0.0f ? A.Lz : 0.0f) - qz) * ic;
-      int axis; float t;
-      if (tx <= ty && tx <= tz) { axis = 0; t = tx; }
-      else if (ty <= tz)        { axis = 1; t = ty; }
-      else                      { axis = 2; t = tz; }
-      const float dtau = kh * t;
-      bool redraw = false;
-      if (kh > 0.0f && tau <= dtau) {
-        // §3.8 tentative collision inside this cell
-        const float s = tau * (1.0f / kh);
-        qx = fminf(A.Lx, fmaxf(0.0f, fmaf(va, s, qx)));
-        qy = fminf(A.Ly, fmaxf(0.0f, fmaf(vb, s, qy)));
-        qz = fminf(A.Lz, fmaxf(0.0f, fmaf(vc, s, qz)));
-        const int lx = min((int)(qx * A.rdx), A.bx - 1);
-        const int ly = min((int)(qy * A.rdy), A.by - 1);
-        const int lz = min((int)(qz * A.rdz), A.bz - 1);
-        const size_t vox = ((size_t)(cz * A.bz + lz) * A.ny + (cy * A.by + ly)) * A.nx + (cx * A.bx + lx);
-        const float4 v = __ldg(&A.optics[vox]);
-        ++n_ev;
-        const float xi = u1 * kh;
-        if (xi < v.x) {                         // absorbed by the gas / droplet
-          tally_a = A.atm_abs + vox;
-          fate = 1; term = (uint32_t)vox;
-        } else if (xi < v.z) {                  // real scattering
-          float mu;
-          if (xi < v.y) { mu = sample_hg(v.w, u2); ++n_hg; }
-          else          { mu = sample_rayleigh(u2); }
-          float sp, cp;
-          sincos_2pi(u3, sp, cp);
-          rotate_dir(da, db, dc, mu, cp, sp);
-          ia = 1.0f / (fabsf(da) < kTiny ? kTiny : da);
-          ib = 1.0f / (fabsf(db) < kTiny ? kTiny : db);
-          ic = 1.0f / (fabsf(dc) < kTiny ? kTiny : dc);
-          direct = false; ++n_sc;
-        }
-        if (fate == 0) redraw = true;
-      } else {
-        // §3.7 leave the cell through `axis`, carrying the residual optical depth
-        tau = tau - dtau;
-        qx = fminf(A.Lx, fmaxf(0.0f, fmaf(va, t, qx)));
-        qy = fminf(A.Ly, fmaxf(0.0f, fmaf(vb, t, qy)));
-        qz = fminf(A.Lz, fmaxf(0.0f, fmaf(vc, t, qz)));
-        ++n_cells;
+    const int nT = __popc(bT), nC = __popc(bC), nS = __popc(bS);
+    if (nS >= kScatterBatch || !(bT | bC)) {
+      // ---- SCATTER: phase-function angle, rotation (§3.9) ------------------------------------------
+      if (st == ST_SCATTER) {
+        float mu;
+        if (sg < 1.5f) { mu = sample_hg(sg, u24(sw2)); ++t_hg; }
+        else           { mu = sample_rayleigh(u24(sw2)); }
+        float sp, cp;
+        sincos_2pi(u24(sw3), sp, cp);
+        rotate_dir(da, db, dc, mu, cp, sp);
+        set_inverse();
+        direct = false; ++t_sc;
+        probe();
+      }
+    } else if (nT * kTraverseWeight >= nC) {
+      // ---- TRAVERSE: leave the cell through `axis`, carrying the residual optical depth (§3.7) ------
+      if (st == ST_TRAVERSE) {
+        tau = tau - kh * t;
+        qx = fminf(A.Lx, fmaxf(0.0f, fmaf(nudge(da), t, qx)));
+        qy = fminf(A.Ly, fmaxf(0.0f, fmaf(nudge(db), t, qy)));
+        qz = fminf(A.Lz, fmaxf(0.0f, fmaf(nudge(dc), t, qz)));
+        ++t_cells;
         bool at_sfc = false, at_top = false;
         if (axis == 0) {
-          if (va > 0.0f) { ++cx; if (cx == A.ncx) cx = 0; qx = 0.0f; }
+          if (ia > 0.0f) { ++cx; if (cx == A.ncx) cx = 0; qx = 0.0f; }
           else           { --cx; if (cx < 0) cx = A.ncx - 1; qx = A.Lx; }
         } else if (axis == 1) {
-          if (vb > 0.0f) { ++cy; if (cy == A.ncy) cy = 0; qy = 0.0f; }
+          if (ib > 0.0f) { ++cy; if (cy == A.ncy) cy = 0; qy = 0.0f; }
           else           { --cy; if (cy < 0) cy = A.ncy - 1; qy = A.Ly; }
         } else {
-          if (vc > 0.0f) { ++cz; qz = 0.0f; at_top = (cz == A.ncz); }
+          if (ic > 0.0f) { ++cz; qz = 0.0f; at_top = (cz == A.ncz); }
           else           { --cz; qz = A.Lz; at_sfc = (cz < 0); }
         }
         if (at_sfc || at_top) {
           const int hx = cx * A.bx + min((int)(qx * A.rdx), A.bx - 1);
           const int hy = cy * A.by + min((int)(qy * A.rdy), A.by - 1);
           const size_t col = (size_t)hy * A.nx + hx;
-          if (at_top) {                         // §3.11 leaves through the domain top
+          if (at_top) {                          // §3.11 leaves through the domain top
             tally_a = A.toa_up + col;
             fate = 3; term = (uint32_t)col;
-          } else {                              // §3.10 Lambertian surface
-            ++n_sfc;
+          } else {                               // §3.10 Lambertian surface
+            ++t_sfc;
             tally_a = (direct ? A.sfc_dir : A.sfc_dif) + col;
             if (u1 < __ldg(&A.albedo[col])) {
+              const float u2 = u24(w2);
               const float mu = sqrtf(1.0f - u2), s = sqrtf(u2);
               float sp, cp;
-              sincos_2pi(u3, sp, cp);
+              sincos_2pi(u24(w3), sp, cp);
               da = s * cp; db = s * sp; dc = mu;
-              ia = 1.0f / (fabsf(da) < kTiny ? kTiny : da);
-              ib = 1.0f / (fabsf(db) < kTiny ? kTiny : db);
-              ic = 1.0f / (fabsf(dc) < kTiny ? kTiny : dc);
+              set_inverse();
               direct = false; cz = 0; qz = 0.0f;
-              redraw = true;
+              ++e;
+              if (e > kEventCap) { fate = 4; term = 0; }   // §3.12
+              else draw();
             } else {
               tally_b = A.sfc_abs + col;
               fate = 2; term = (uint32_t)col;
             }
           }
         }
-        if (fate == 0) kh = __ldg(&A.khat[((size_t)cz * A.ncy + cy) * A.ncx + cx]);
-      }
-      if (redraw) {
-        ++e;
-        if (e > kEventCap) {                    // §3.12
-          fate = 4; term = 0;
+        if (fate == 0) {
+          kh = __ldg(&A.khat[((size_t)cz * A.ncy + cy) * A.ncx + cx]);
+          probe();
         } else {
-          const uint4 X = philox4x32_10(p_lo, p_hi, e, A.stream_id, A.key0, A.key1);
-          tau = neg_log(1.0f - u24(X.x)); u1 = u24(X.y); u2 = u24(X.z); u3 = u24(X.w);
+          st = ST_DEAD;
+        }
+      }
+    } else {
+      // ---- COLLIDE: fetch the voxel, classify, draw the next event (§3.8) --------------------------
+      if (st == ST_COLLIDE) {
+        bool go_on = true;                         // the photon continues with a new draw
+        if (!fresh) {
+          const float s = tau * (1.0f / kh);
+          qx = fminf(A.Lx, fmaxf(0.0f, fmaf(nudge(da), s, qx)));
+          qy = fminf(A.Ly, fmaxf(0.0f, fmaf(nudge(db), s, qy)));
+          qz = fminf(A.Lz, fmaxf(0.0f, fmaf(nudge(dc), s, qz)));
+          const int lx = min((int)(qx * A.rdx), A.bx - 1);
+          const int ly = min((int)(qy * A.rdy), A.by - 1);
+          const int lz = min((int)(qz * A.rdz), A.bz - 1);
+          const size_t vox = ((size_t)(cz * A.bz + lz) * A.ny + (cy * A.by + ly)) * A.nx + (cx * A.bx + lx);
+          const float4 v = __ldg(&A.optics[vox]);
+          ++t_ev;
+          const float xi = u1 * kh;
+          st = ST_TRAVERSE;
+          if (xi < v.x) {                           // absorbed by the gas / droplet
+            tally_a = A.atm_abs + vox;
+            fate = 1; term = (uint32_t)vox;
+            st = ST_DEAD; go_on = false;
+          } else if (xi < v.z) {                    // real scattering: angle and rotation in SCATTER
+            st = ST_SCATTER;
+            sg = (xi < v.y) ? v.w : 2.0f;
+            sw2 = w2; sw3 = w3;
+          }
+        }
+        fresh = false;
+        if (go_on) {
+          ++e;
+          if (e > kEventCap) {                      // §3.12 (the capped event itself is still counted)
+            if (st == ST_SCATTER) { ++t_sc; if (sg < 1.5f) ++t_hg; }
+            fate = 4; term = 0; st = ST_DEAD;
+          } else {
+            draw();
+            if (st != ST_SCATTER) probe();          // a scattered photon probes with its new direction
+          }
         }
       }
     }
 
-    // ---- tallies (converged): warp-aggregated 64-bit integer atomics ----------------------------
+    // ---- tallies (converged): warp-aggregated 64-bit integer atomics -----------------------------
     const unsigned ma = __ballot_sync(0xffffffffu, tally_a != nullptr);
     if (ma) {
       if (tally_a) tally_add(ma, tally_a);
       const unsigned mb = __ballot_sync(0xffffffffu, tally_b != nullptr);
       if (mb && tally_b) tally_add(mb, tally_b);
     }
-    if (fate != 0) {
-      // photon finished: fold its event counts into the block counters, write its record
-      const uint32_t n_abs = (fate == 1) ? 1u : 0u;
-      atomicAdd(&s_cnt[C_NULL], (unsigned long long)(n_ev - n_sc - n_abs));
-      atomicAdd(&s_cnt[C_RAY], (unsigned long long)(n_sc - n_hg));
-      atomicAdd(&s_cnt[C_HG], (unsigned long long)n_hg);
-      atomicAdd(&s_cnt[C_SFC_HITS], (unsigned long long)n_sfc);
-      atomicAdd(&s_cnt[C_CELLS], (unsigned long long)n_cells);
-      atomicAdd(&s_cnt[fate == 1 ? C_ATM_ABS : fate == 2 ? C_SFC_ABS : fate == 3 ? C_TOA : C_CAPPED], 1ull);
-      if (fate == 4) atomicAdd(&s_cnt[C_CAPPED_E], kW0);
-      if (kRecords) {
+    if (__any_sync(0xffffffffu, fate != 0)) {
+      // photons finished: count their fates per warp, write their records
+      const unsigned f1 = __ballot_sync(0xffffffffu, fate == 1), f2 = __ballot_sync(0xffffffffu, fate == 2);
+      const unsigned f3 = __ballot_sync(0xffffffffu, fate == 3), f4 = __ballot_sync(0xffffffffu, fate == 4);
+      if (lane == 0) {
+        if (f1) atomicAdd(&s_cnt[C_ATM_ABS], (unsigned long long)__popc(f1));
+        if (f2) atomicAdd(&s_cnt[C_SFC_ABS], (unsigned long long)__popc(f2));
+        if (f3) atomicAdd(&s_cnt[C_TOA], (unsigned long long)__popc(f3));
+        if (f4) {
+          atomicAdd(&s_cnt[C_CAPPED], (unsigned long long)__popc(f4));
+          atomicAdd(&s_cnt[C_CAPPED_E], kW0 * (unsigned long long)__popc(f4));
+        }
+      }
+      if (kRecords && fate != 0) {
         uint4 r;
-        r.x = (uint32_t)fate | (min(n_sfc, 0xFFFFFFu) << 8);
-        r.y = term; r.z = n_ev; r.w = n_sc;
+        r.x = (uint32_t)fate | (min(t_sfc - b_sfc, 0xFFFFFFu) << 8);
+        r.y = term; r.z = t_ev - b_ev; r.w = t_sc - b_sc;
         reinterpret_cast<uint4*>(A.records)[i] = r;
       }
-      alive = false;
     }
   }
 
+  flush_thread_counters();
+  __syncthreads();
+  if (threadIdx.x == 0) s_cnt[C_NULL] -= s_cnt[C_ATM_ABS];   // events - scatters - absorptions
   __syncthreads();
   if (threadIdx.x < C_COUNT && s_cnt[threadIdx.x] != 0ull)
     atomicAdd(&A.counters[threadIdx.x], s_cnt[threadIdx.x]);
