@@ -1,21 +1,21 @@
 // rt_trace.cuh — the persistent photon-tracing kernel.
 //
-// One thread carries one photon at a time.  A photon is a small state machine:
-//   TRAVERSE  next thing to do is a step of the walk over acceleration cells (§3.7),
-//   COLLIDE   a tentative collision lies inside the current cell: fetch the voxel, classify (§3.8),
-//   SCATTER   a real scattering event was chosen: sample the angle and rotate (§3.9),
-//   DEAD      the lane is idle and waits for a new photon.
-// The phases have very different costs (a cell step is ~60 instructions, a collision with its Philox
-// draw and logarithm ~300, a scatter with its divisions and square roots ~200), and a scatter is chosen
-// by only ~7 % of the events: letting each lane take "its" branch every iteration runs the scatter code
-// in 84 % of the iterations with 2 of 32 lanes active (ncu, profiles/r1_baseline_*: 14.4 active threads
-// per instruction overall).  Instead the warp VOTES each iteration (ballot/popc) on one phase to run;
-// COLLIDE and TRAVERSE both end by probing the current cell for the next event, so a lane stays in its
-// state while it keeps colliding (in cloud) or keeps crossing (in clear air); SCATTER and the refill of
-// DEAD lanes run when enough lanes wait for them.  Dead lanes are refilled in batches from a
-// warp-private pool of photon ids taken in chunks from a global counter (BASELINE.json north_star:
-// "compacted and regenerated persistently with warp-level ballot/shuffle").  The per-photon sequence of
-// arithmetic operations is unchanged by the scheduling, so results do not depend on it.
+// One thread carries one photon at a time.  Its position inside the current acceleration cell is held
+// as the remaining distances (rx, ry, rz) along the flight direction to the cell's next face on each
+// axis: a cell crossing is ~25 instructions (smallest of three, two subtractions, one
+// reset to the face spacing, index step, one 4-byte load of the majorant), a null collision updates the
+// three distances and nothing else.  With cheap crossings a fine acceleration grid (2^3 voxels per
+// cell) pays: 38 tentative collisions and 168 crossings per photon on the 512x512x128 cumulus field
+// instead of 202 and 42 with 8^3 cells.
+//
+// Divergence.  MOVE (cross or collide) is what every live lane does each iteration.  A real scatter
+// (phase-function inversion, rotation, three IEEE divisions: ~200 instructions) is chosen by few lanes
+// per iteration; run inline it executed in 84 % of the iterations with 2 of 32 lanes active (ncu,
+// profiles/r1_baseline_*).  So a lane that chose to scatter parks in SCATTER and the warp runs that
+// phase when kScatterBatch lanes wait (ballot/popc vote); DEAD lanes are refilled kRegenBatch at a time
+// from a warp-private pool of photon ids taken in chunks from a global counter (BASELINE.json
+// north_star: "compacted and regenerated persistently with warp-level ballot/shuffle").  A photon's own
+// sequence of arithmetic operations does not depend on the scheduling, so neither do the results.
 #pragma once
 #include "rt_device.cuh"
 
@@ -26,23 +26,22 @@ constexpr uint32_t kEventCap = 1u << 20;        // §3.12
 constexpr float kTiny = 1e-30f;                 // direction components are nudged away from 0
 constexpr int kTraceThreads = 256;
 constexpr int kChunk = 128;                     // photon ids a warp takes per global atomic
+#ifndef RT_MIN_BLOCKS
+#define RT_MIN_BLOCKS 3
+#endif
 #ifndef RT_REGEN_BATCH
 #define RT_REGEN_BATCH 6
 #endif
 #ifndef RT_SCATTER_BATCH
 #define RT_SCATTER_BATCH 6
 #endif
-#ifndef RT_TRAVERSE_WEIGHT
-#define RT_TRAVERSE_WEIGHT 2
-#endif
 constexpr int kRegenBatch = RT_REGEN_BATCH;       // refill when this many lanes are idle (or nothing else to do)
 constexpr int kScatterBatch = RT_SCATTER_BATCH;   // run SCATTER when this many lanes wait for it (or nothing else)
-constexpr int kTraverseWeight = RT_TRAVERSE_WEIGHT;  // TRAVERSE (cheap) runs when nT * weight >= nC
 
 enum Counter { C_NULL = 0, C_RAY, C_HG, C_ATM_ABS, C_SFC_HITS, C_SFC_ABS, C_TOA, C_CAPPED, C_CELLS,
                C_CAPPED_E, C_COUNT };
 
-enum : uint32_t { ST_DEAD = 0, ST_TRAVERSE = 1, ST_COLLIDE = 2, ST_SCATTER = 3 };
+enum : uint32_t { ST_DEAD = 0, ST_MOVE = 1, ST_SCATTER = 2 };
 
 struct TraceArgs {
   int nx, ny, nz, bx, by, bz, ncx, ncy, ncz;
@@ -76,8 +75,9 @@ __device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
 }
 
 
+
 template <bool kRecords>
-__global__ void __launch_bounds__(kTraceThreads) trace_kernel(const TraceArgs A) {
+__global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(const TraceArgs A) {
   __shared__ unsigned long long s_cnt[C_COUNT];
   if (threadIdx.x < C_COUNT) s_cnt[threadIdx.x] = 0ull;
   __syncthreads();
@@ -90,36 +90,38 @@ __global__ void __launch_bounds__(kTraceThreads) trace_kernel(const TraceArgs A)
   // photon state
   uint32_t st = ST_DEAD;
   unsigned long long i = 0;
-  uint32_t p_lo = 0, p_hi = 0, e = 0;
+  uint32_t e = 0;
   int cx = 0, cy = 0, cz = 0;
-  float qx = 0, qy = 0, qz = 0, da = 0, db = 0, dc = -1, ia = 0, ib = 0, ic = 0;
+  float da = 0, db = 0, dc = -1;          // unit direction
+  float rx = 0, ry = 0, rz = 0;           // remaining distance to the cell's next face on each axis
+  float delx = 0, dely = 0, delz = 0;     // distance between successive faces on each axis
   float tau = 0, kh = 0, u1 = 0;
-  float t = 0;                      // TRAVERSE: distance to the face the photon leaves the cell through
-  int axis = 3;                     // ... and that face's axis (3 = none: probe only, after a scatter)
-  uint32_t w2 = 0, w3 = 0;          // words 2, 3 of the current event's draw
-  uint32_t sw2 = 0, sw3 = 0;        // ... of the event that chose SCATTER (its draw is already replaced)
-  float sg = 0;                     // asymmetry parameter for the pending scatter; 2 = Rayleigh
+  uint32_t w2 = 0, w3 = 0;                // words 2, 3 of the current event's draw
+  uint32_t sw2 = 0, sw3 = 0;              // ... of the event that chose SCATTER (its draw is already replaced)
+  float sg = 0;                           // asymmetry parameter for the pending scatter; 2 = Rayleigh
   bool direct = true;
-  bool fresh = false;               // just launched: in COLLIDE only to take its first draw
   // event counts: running totals of this thread; a photon's own counts are differences (records)
   uint32_t t_ev = 0, t_sc = 0, t_hg = 0, t_sfc = 0, t_cells = 0;
   uint32_t b_ev = 0, b_sc = 0, b_sfc = 0;  // totals when the current photon was launched (records only)
 
   auto draw = [&]() {
-    const uint4 X = philox4x32_10(p_lo, p_hi, e, A.stream_id, A.key0, A.key1);
+    const unsigned long long pid = A.first_id + i;
+    const uint4 X = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), e, A.stream_id, A.key0, A.key1);
     tau = neg_log(1.0f - u24(X.x)); u1 = u24(X.y); w2 = X.z; w3 = X.w;
   };
-  auto set_inverse = [&]() { ia = 1.0f / nudge(da); ib = 1.0f / nudge(db); ic = 1.0f / nudge(dc); };
-  // §3.7 first half: distance to the nearest face of the current cell (ties x < y < z) and whether the
-  // tentative collision falls before it.  Sets the lane's next state.
-  auto probe = [&]() {
-    const float tx = ((ia > 0.0f ? A.Lx : 0.0f) - qx) * ia;   // sign(ia) == sign(nudged component)
-    const float ty = ((ib > 0.0f ? A.Ly : 0.0f) - qy) * ib;
-    const float tz = ((ic > 0.0f ? A.Lz : 0.0f) - qz) * ic;
-    if (tx <= ty && tx <= tz) { axis = 0; t = tx; }
-    else if (ty <= tz)        { axis = 1; t = ty; }
-    else                      { axis = 2; t = tz; }
-    st = (kh > 0.0f && tau <= kh * t) ? ST_COLLIDE : ST_TRAVERSE;
+  // local coordinate from a remaining distance: q = face - v r, face = L if v > 0 else 0
+  auto local = [&](float d, float r, float L) {
+    const float v = nudge(d);
+    return fminf(L, fmaxf(0.0f, fmaf(-v, r, v > 0.0f ? L : 0.0f)));
+  };
+  // after a change of direction at local position (qx, qy, qz): reciprocals, face spacings, distances
+  auto place = [&](float qx, float qy, float qz) {
+    const float va = nudge(da), vb = nudge(db), vc = nudge(dc);
+    const float ia = 1.0f / va, ib = 1.0f / vb, ic = 1.0f / vc;
+    delx = A.Lx * fabsf(ia); dely = A.Ly * fabsf(ib); delz = A.Lz * fabsf(ic);
+    rx = ((va > 0.0f ? A.Lx : 0.0f) - qx) * ia;
+    ry = ((vb > 0.0f ? A.Ly : 0.0f) - qy) * ib;
+    rz = ((vc > 0.0f ? A.Lz : 0.0f) - qz) * ic;
   };
   auto flush_thread_counters = [&]() {
     unsigned long long v;
@@ -133,10 +135,9 @@ __global__ void __launch_bounds__(kTraceThreads) trace_kernel(const TraceArgs A)
   };
 
   for (;;) {
-    const unsigned bT = __ballot_sync(0xffffffffu, st == ST_TRAVERSE);
-    const unsigned bC = __ballot_sync(0xffffffffu, st == ST_COLLIDE);
+    const unsigned bM = __ballot_sync(0xffffffffu, st == ST_MOVE);
     const unsigned bS = __ballot_sync(0xffffffffu, st == ST_SCATTER);
-    const unsigned live = bT | bC | bS;
+    const unsigned live = bM | bS;
     int fate = 0;
     uint32_t term = 0;
     unsigned long long* tally_a = nullptr;  // arrival / terminal bin
@@ -173,8 +174,7 @@ __global__ void __launch_bounds__(kTraceThreads) trace_kernel(const TraceArgs A)
       if (got) {
         // ---- §3.6 launch, event index 0 ------------------------------------------------------
         const unsigned long long pid = A.first_id + i;
-        p_lo = (uint32_t)pid; p_hi = (uint32_t)(pid >> 32);
-        const uint4 X = philox4x32_10(p_lo, p_hi, 0u, A.stream_id, A.key0, A.key1);
+        const uint4 X = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), 0u, A.stream_id, A.key0, A.key1);
         int ix, iy;
         if (i < A.n_full) {
           // column = i mod ncol; 32-bit arithmetic whenever the index allows it
@@ -186,73 +186,110 @@ __global__ void __launch_bounds__(kTraceThreads) trace_kernel(const TraceArgs A)
           iy = min((int)(u24(X.w) * (float)A.ny), A.ny - 1);
         }
         cx = ix / A.bx; cy = iy / A.by; cz = A.ncz - 1;
-        qx = ((float)(ix % A.bx) + u24(X.x)) * A.dx;
-        qy = ((float)(iy % A.by) + u24(X.y)) * A.dy;
-        qz = A.Lz;
         da = A.sun_x; db = A.sun_y; dc = A.sun_z;
-        ia = A.sun_ix; ib = A.sun_iy; ic = A.sun_iz;
+        // place() with the beam's host-computed reciprocals (same IEEE operations)
+        delx = A.Lx * fabsf(A.sun_ix); dely = A.Ly * fabsf(A.sun_iy); delz = A.Lz * fabsf(A.sun_iz);
+        rx = ((A.sun_ix > 0.0f ? A.Lx : 0.0f) - ((float)(ix % A.bx) + u24(X.x)) * A.dx) * A.sun_ix;
+        ry = ((A.sun_iy > 0.0f ? A.Ly : 0.0f) - ((float)(iy % A.by) + u24(X.y)) * A.dy) * A.sun_iy;
+        rz = ((A.sun_iz > 0.0f ? A.Lz : 0.0f) - A.Lz) * A.sun_iz;
         direct = true;
-        e = 0;
+        e = 1;
         if (kRecords) { b_ev = t_ev; b_sc = t_sc; b_sfc = t_sfc; }
+        draw();
         kh = __ldg(&A.khat[((size_t)cz * A.ncy + cy) * A.ncx + cx]);
-        fresh = true;                                // COLLIDE's tail draws event 1 and probes the cell
-        st = ST_COLLIDE;
+        st = ST_MOVE;
       }
       continue;
     }
     if (!live) break;
 
-    const int nT = __popc(bT), nC = __popc(bC), nS = __popc(bS);
-    if (nS >= kScatterBatch || !(bT | bC)) {
-      // ---- SCATTER: phase-function angle, rotation (§3.9) ------------------------------------------
+    if (__popc(bS) >= kScatterBatch || !bM) {
+      // ---- SCATTER: phase-function angle, rotation, new distances to the faces (§3.9) --------------
       if (st == ST_SCATTER) {
+        const float qx = local(da, rx, A.Lx), qy = local(db, ry, A.Ly), qz = local(dc, rz, A.Lz);
         float mu;
         if (sg < 1.5f) { mu = sample_hg(sg, u24(sw2)); ++t_hg; }
         else           { mu = sample_rayleigh(u24(sw2)); }
         float sp, cp;
         sincos_2pi(u24(sw3), sp, cp);
         rotate_dir(da, db, dc, mu, cp, sp);
-        set_inverse();
+        place(qx, qy, qz);
         direct = false; ++t_sc;
-        probe();
+        st = ST_MOVE;
       }
-    } else if (nT * kTraverseWeight >= nC) {
-      // ---- TRAVERSE: leave the cell through `axis`, carrying the residual optical depth (§3.7) ------
-      if (st == ST_TRAVERSE) {
-        tau = tau - kh * t;
-        qx = fminf(A.Lx, fmaxf(0.0f, fmaf(nudge(da), t, qx)));
-        qy = fminf(A.Ly, fmaxf(0.0f, fmaf(nudge(db), t, qy)));
-        qz = fminf(A.Lz, fmaxf(0.0f, fmaf(nudge(dc), t, qz)));
+    } else if (st == ST_MOVE) {
+      // ---- MOVE: nearest face of the current cell (ties x < y < z), then collide or cross (§3.7) ----
+      int axis; float t;
+      if (rx <= ry && rx <= rz) { axis = 0; t = rx; }
+      else if (ry <= rz)        { axis = 1; t = ry; }
+      else                      { axis = 2; t = rz; }
+      const float dtau = kh * t;
+      if (kh > 0.0f && tau <= dtau) {
+        // §3.8 tentative collision inside this cell: fetch the voxel, classify, draw the next event
+        const float s = tau * (1.0f / kh);
+        rx = fmaxf(0.0f, rx - s); ry = fmaxf(0.0f, ry - s); rz = fmaxf(0.0f, rz - s);
+        const float qx = local(da, rx, A.Lx), qy = local(db, ry, A.Ly), qz = local(dc, rz, A.Lz);
+        const int lx = min((int)(qx * A.rdx), A.bx - 1);
+        const int ly = min((int)(qy * A.rdy), A.by - 1);
+        const int lz = min((int)(qz * A.rdz), A.bz - 1);
+        const size_t vox = ((size_t)(cz * A.bz + lz) * A.ny + (cy * A.by + ly)) * A.nx + (cx * A.bx + lx);
+        const float4 v = __ldg(&A.optics[vox]);
+        ++t_ev;
+        const float xi = u1 * kh;
+        if (xi < v.x) {                             // absorbed by the gas / droplet
+          tally_a = A.atm_abs + vox;
+          fate = 1; term = (uint32_t)vox;
+        } else {
+          if (xi < v.z) {                           // real scattering: angle and rotation in SCATTER
+            st = ST_SCATTER;
+            sg = (xi < v.y) ? v.w : 2.0f;
+            sw2 = w2; sw3 = w3;
+          }
+          ++e;
+          if (e > kEventCap) {                      // §3.12 (the capped event itself is still counted)
+            if (st == ST_SCATTER) { ++t_sc; if (sg < 1.5f) ++t_hg; }
+            fate = 4; term = 0;
+          } else {
+            draw();
+          }
+        }
+      } else {
+        // §3.7 leave the cell through `axis`, carrying the residual optical depth
+        tau = tau - dtau;
         ++t_cells;
         bool at_sfc = false, at_top = false;
         if (axis == 0) {
-          if (ia > 0.0f) { ++cx; if (cx == A.ncx) cx = 0; qx = 0.0f; }
-          else           { --cx; if (cx < 0) cx = A.ncx - 1; qx = A.Lx; }
+          ry = ry - t; rz = rz - t; rx = delx;
+          if (nudge(da) > 0.0f) { ++cx; if (cx == A.ncx) cx = 0; }
+          else                  { --cx; if (cx < 0) cx = A.ncx - 1; }
         } else if (axis == 1) {
-          if (ib > 0.0f) { ++cy; if (cy == A.ncy) cy = 0; qy = 0.0f; }
-          else           { --cy; if (cy < 0) cy = A.ncy - 1; qy = A.Ly; }
+          rx = rx - t; rz = rz - t; ry = dely;
+          if (nudge(db) > 0.0f) { ++cy; if (cy == A.ncy) cy = 0; }
+          else                  { --cy; if (cy < 0) cy = A.ncy - 1; }
         } else {
-          if (ic > 0.0f) { ++cz; qz = 0.0f; at_top = (cz == A.ncz); }
-          else           { --cz; qz = A.Lz; at_sfc = (cz < 0); }
+          rx = rx - t; ry = ry - t; rz = delz;
+          if (nudge(dc) > 0.0f) { ++cz; at_top = (cz == A.ncz); }
+          else                  { --cz; at_sfc = (cz < 0); }
         }
         if (at_sfc || at_top) {
+          const float qx = local(da, rx, A.Lx), qy = local(db, ry, A.Ly);
           const int hx = cx * A.bx + min((int)(qx * A.rdx), A.bx - 1);
           const int hy = cy * A.by + min((int)(qy * A.rdy), A.by - 1);
           const size_t col = (size_t)hy * A.nx + hx;
-          if (at_top) {                          // §3.11 leaves through the domain top
+          if (at_top) {                             // §3.11 leaves through the domain top
             tally_a = A.toa_up + col;
             fate = 3; term = (uint32_t)col;
-          } else {                               // §3.10 Lambertian surface
+          } else {                                  // §3.10 Lambertian surface
             ++t_sfc;
             tally_a = (direct ? A.sfc_dir : A.sfc_dif) + col;
             if (u1 < __ldg(&A.albedo[col])) {
               const float u2 = u24(w2);
-              const float mu = sqrtf(1.0f - u2), s = sqrtf(u2);
+              const float mu = sqrtf(1.0f - u2), sn = sqrtf(u2);
               float sp, cp;
               sincos_2pi(u24(w3), sp, cp);
-              da = s * cp; db = s * sp; dc = mu;
-              set_inverse();
-              direct = false; cz = 0; qz = 0.0f;
+              da = sn * cp; db = sn * sp; dc = mu;
+              direct = false; cz = 0;
+              place(qx, qy, 0.0f);
               ++e;
               if (e > kEventCap) { fate = 4; term = 0; }   // §3.12
               else draw();
@@ -262,52 +299,9 @@ __global__ void __launch_bounds__(kTraceThreads) trace_kernel(const TraceArgs A)
             }
           }
         }
-        if (fate == 0) {
-          kh = __ldg(&A.khat[((size_t)cz * A.ncy + cy) * A.ncx + cx]);
-          probe();
-        } else {
-          st = ST_DEAD;
-        }
+        if (fate == 0) kh = __ldg(&A.khat[((size_t)cz * A.ncy + cy) * A.ncx + cx]);
       }
-    } else {
-      // ---- COLLIDE: fetch the voxel, classify, draw the next event (§3.8) --------------------------
-      if (st == ST_COLLIDE) {
-        bool go_on = true;                         // the photon continues with a new draw
-        if (!fresh) {
-          const float s = tau * (1.0f / kh);
-          qx = fminf(A.Lx, fmaxf(0.0f, fmaf(nudge(da), s, qx)));
-          qy = fminf(A.Ly, fmaxf(0.0f, fmaf(nudge(db), s, qy)));
-          qz = fminf(A.Lz, fmaxf(0.0f, fmaf(nudge(dc), s, qz)));
-          const int lx = min((int)(qx * A.rdx), A.bx - 1);
-          const int ly = min((int)(qy * A.rdy), A.by - 1);
-          const int lz = min((int)(qz * A.rdz), A.bz - 1);
-          const size_t vox = ((size_t)(cz * A.bz + lz) * A.ny + (cy * A.by + ly)) * A.nx + (cx * A.bx + lx);
-          const float4 v = __ldg(&A.optics[vox]);
-          ++t_ev;
-          const float xi = u1 * kh;
-          st = ST_TRAVERSE;
-          if (xi < v.x) {                           // absorbed by the gas / droplet
-            tally_a = A.atm_abs + vox;
-            fate = 1; term = (uint32_t)vox;
-            st = ST_DEAD; go_on = false;
-          } else if (xi < v.z) {                    // real scattering: angle and rotation in SCATTER
-            st = ST_SCATTER;
-            sg = (xi < v.y) ? v.w : 2.0f;
-            sw2 = w2; sw3 = w3;
-          }
-        }
-        fresh = false;
-        if (go_on) {
-          ++e;
-          if (e > kEventCap) {                      // §3.12 (the capped event itself is still counted)
-            if (st == ST_SCATTER) { ++t_sc; if (sg < 1.5f) ++t_hg; }
-            fate = 4; term = 0; st = ST_DEAD;
-          } else {
-            draw();
-            if (st != ST_SCATTER) probe();          // a scattered photon probes with its new direction
-          }
-        }
-      }
+      if (fate != 0) st = ST_DEAD;
     }
 
     // ---- tallies (converged): warp-aggregated 64-bit integer atomics -----------------------------
