@@ -106,8 +106,14 @@ int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photon
   RT_CUDA(c, cudaMemsetAsync(A.next_photon, 0, sizeof(unsigned long long), st));
   RT_CUDA(c, cudaEventRecord(c->ev0, st));
   if (n_photons > 0) {
-    if (records) rt::trace_kernel<true><<<c->trace_blocks_rec, rt::kTraceThreads, 0, st>>>(A);
-    else         rt::trace_kernel<false><<<c->trace_blocks, rt::kTraceThreads, 0, st>>>(A);
+    const bool pow2 = !(c->ncx & (c->ncx - 1)) && !(c->ncy & (c->ncy - 1));
+    if (records) {
+      if (pow2) rt::trace_kernel<true, true><<<c->trace_blocks_rec, rt::kTraceThreads, 0, st>>>(A);
+      else      rt::trace_kernel<true, false><<<c->trace_blocks_rec, rt::kTraceThreads, 0, st>>>(A);
+    } else {
+      if (pow2) rt::trace_kernel<false, true><<<c->trace_blocks, rt::kTraceThreads, 0, st>>>(A);
+      else      rt::trace_kernel<false, false><<<c->trace_blocks, rt::kTraceThreads, 0, st>>>(A);
+    }
     ++c->launches;
   }
   RT_CUDA(c, cudaEventRecord(c->ev1, st));
@@ -151,9 +157,15 @@ int rt_create_grid(rt_ctx** out, int nx, int ny, int nz, float dx, float dy, flo
   RT_CUDA(c, cudaEventCreate(&c->ev1));
   RT_CUDA(c, cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, cuda_device));
   int per_sm = 0;
-  RT_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rt::trace_kernel<false>, rt::kTraceThreads, 0));
+  // persistent grid: resident blocks per SM (the smaller of the two wrap variants) x SM count
+  int per_sm2 = 0;
+  RT_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rt::trace_kernel<false, false>, rt::kTraceThreads, 0));
+  RT_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm2, rt::trace_kernel<false, true>, rt::kTraceThreads, 0));
+  per_sm = per_sm < per_sm2 ? per_sm : per_sm2;
   c->trace_blocks = c->sm_count * (per_sm > 0 ? per_sm : 1);
-  RT_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rt::trace_kernel<true>, rt::kTraceThreads, 0));
+  RT_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rt::trace_kernel<true, false>, rt::kTraceThreads, 0));
+  RT_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm2, rt::trace_kernel<true, true>, rt::kTraceThreads, 0));
+  per_sm = per_sm < per_sm2 ? per_sm : per_sm2;
   c->trace_blocks_rec = c->sm_count * (per_sm > 0 ? per_sm : 1);
   return RT_OK;
 }

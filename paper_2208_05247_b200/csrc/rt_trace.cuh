@@ -8,14 +8,17 @@
 // cell) pays: 38 tentative collisions and 168 crossings per photon on the 512x512x128 cumulus field
 // instead of 202 and 42 with 8^3 cells.
 //
-// Divergence.  MOVE (cross or collide) is what every live lane does each iteration.  A real scatter
-// (phase-function inversion, rotation, three IEEE divisions: ~200 instructions) is chosen by few lanes
-// per iteration; run inline it executed in 84 % of the iterations with 2 of 32 lanes active (ncu,
-// profiles/r1_baseline_*).  So a lane that chose to scatter parks in SCATTER and the warp runs that
-// phase when kScatterBatch lanes wait (ballot/popc vote); DEAD lanes are refilled kRegenBatch at a time
-// from a warp-private pool of photon ids taken in chunks from a global counter (BASELINE.json
-// north_star: "compacted and regenerated persistently with warp-level ballot/shuffle").  A photon's own
-// sequence of arithmetic operations does not depend on the scheduling, so neither do the results.
+// Divergence.  The cheap step, MOVE (find the nearest face; cross it, or notice that the tentative
+// collision comes first), is what live lanes do by default.  The expensive steps are each wanted by few
+// lanes per iteration -- a collision (voxel gather, classification, Philox draw, logarithm: ~180
+// instructions) by ~5 of 32, a real scatter (phase-function inversion, rotation, three IEEE divisions:
+// ~250) by ~2, a surface or domain-top arrival by fewer -- and run inline they executed with 2-6 lanes
+// active (ncu, profiles/r1_*: 11-14 active threads per instruction overall).  So a lane that needs one
+// PARKS in COLLIDE, SCATTER or BOUNDARY, and the warp votes (ballot/popc) to run that phase once enough
+// lanes wait for it; DEAD lanes are refilled kRegenBatch at a time from a warp-private pool of photon
+// ids taken in chunks from a global counter (BASELINE.json north_star: "compacted and regenerated
+// persistently with warp-level ballot/shuffle").  A photon's own sequence of arithmetic operations does
+// not depend on the scheduling, so neither do the results.
 #pragma once
 #include "rt_device.cuh"
 
@@ -33,15 +36,27 @@ constexpr int kChunk = 128;                     // photon ids a warp takes per g
 #define RT_REGEN_BATCH 6
 #endif
 #ifndef RT_SCATTER_BATCH
-#define RT_SCATTER_BATCH 6
+#define RT_SCATTER_BATCH 8
+#endif
+#ifndef RT_COLLIDE_BATCH
+#define RT_COLLIDE_BATCH 8
+#endif
+#ifndef RT_MOVE_STEPS
+#define RT_MOVE_STEPS 3
+#endif
+#ifndef RT_BOUNDARY_BATCH
+#define RT_BOUNDARY_BATCH 4
 #endif
 constexpr int kRegenBatch = RT_REGEN_BATCH;       // refill when this many lanes are idle (or nothing else to do)
-constexpr int kScatterBatch = RT_SCATTER_BATCH;   // run SCATTER when this many lanes wait for it (or nothing else)
+constexpr int kScatterBatch = RT_SCATTER_BATCH;   // run SCATTER when this many lanes wait for it (or nothing moves)
+constexpr int kCollideBatch = RT_COLLIDE_BATCH;   // ... COLLIDE
+constexpr int kBoundaryBatch = RT_BOUNDARY_BATCH; // ... BOUNDARY
+constexpr int kMoveSteps = RT_MOVE_STEPS;         // MOVE steps between two votes
 
 enum Counter { C_NULL = 0, C_RAY, C_HG, C_ATM_ABS, C_SFC_HITS, C_SFC_ABS, C_TOA, C_CAPPED, C_CELLS,
                C_CAPPED_E, C_COUNT };
 
-enum : uint32_t { ST_DEAD = 0, ST_MOVE = 1, ST_SCATTER = 2 };
+enum : uint32_t { ST_DEAD = 0, ST_MOVE = 1, ST_COLLIDE = 2, ST_SCATTER = 3, ST_BOUNDARY = 4 };
 
 struct TraceArgs {
   int nx, ny, nz, bx, by, bz, ncx, ncy, ncz;
@@ -76,7 +91,8 @@ __device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
 
 
 
-template <bool kRecords>
+// kPow2: the acceleration grid's x and y extents are powers of two, so the periodic wrap is a mask.
+template <bool kRecords, bool kPow2>
 __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(const TraceArgs A) {
   __shared__ unsigned long long s_cnt[C_COUNT];
   if (threadIdx.x < C_COUNT) s_cnt[threadIdx.x] = 0ull;
@@ -134,18 +150,16 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
     v = warp_sum(t_ev - t_sc);  if (lane == 0 && v) atomicAdd(&s_cnt[C_NULL], v);
   };
 
-  for (;;) {
-    const unsigned bM = __ballot_sync(0xffffffffu, st == ST_MOVE);
-    const unsigned bS = __ballot_sync(0xffffffffu, st == ST_SCATTER);
-    const unsigned live = bM | bS;
-    int fate = 0;
-    uint32_t term = 0;
-    unsigned long long* tally_a = nullptr;  // arrival / terminal bin
-    unsigned long long* tally_b = nullptr;  // surface absorption after an arrival tally
 
-    if (!exhausted && (__popc(~live) >= kRegenBatch || !live)) {
+  for (;;) {
+    // the vote: one warp-wide integer add counts the lanes in each of the five states (6 bits each)
+    const unsigned votes = __reduce_add_sync(0xffffffffu, 1u << (6u * st));
+    const int nD = votes & 63u, nM = (votes >> 6) & 63u, nC = (votes >> 12) & 63u, nS = (votes >> 18) & 63u,
+              nB = (votes >> 24) & 63u;
+
+    if (!exhausted && (nD >= kRegenBatch || nD == 32)) {
       // ---- regeneration: hand photon ids to the idle lanes -------------------------------------
-      unsigned waiting = ~live;
+      unsigned waiting = __ballot_sync(0xffffffffu, st == ST_DEAD);
       bool got = false;
 #pragma unroll 1
       for (int pass = 0; pass < 2 && waiting; ++pass) {
@@ -201,9 +215,50 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
       }
       continue;
     }
-    if (!live) break;
+    if (nD == 32) break;
 
-    if (__popc(bS) >= kScatterBatch || !bM) {
+    const bool stuck = (nM == 0);                  // nothing can move: run the fullest parked phase
+    if (!stuck && nC < kCollideBatch && nS < kScatterBatch && nB < kBoundaryBatch) {
+      // ---- MOVE: nearest face of the current cell (ties x < y < z), then cross or park (§3.7) -------
+#pragma unroll
+      for (int rep = 0; rep < kMoveSteps; ++rep)
+      if (st == ST_MOVE) {
+        const bool ax0 = (rx <= ry) && (rx <= rz);
+        const bool ax1 = !ax0 && (ry <= rz);
+        const bool ax2 = !ax0 && !ax1;
+        const float t = ax0 ? rx : (ax1 ? ry : rz);
+        const float dtau = kh * t;
+        if (kh > 0.0f && tau <= dtau) {
+          st = ST_COLLIDE;                           // the tentative collision comes first
+        } else {
+          // leave the cell through that face, carrying the residual optical depth
+          tau = tau - dtau;
+          ++t_cells;
+          rx = ax0 ? delx : rx - t;
+          ry = ax1 ? dely : ry - t;
+          rz = ax2 ? delz : rz - t;
+          // step the cell index; x and y wrap (periodic).  d > -tiny is "the nudged component is positive"
+          if (kPow2) {
+            if (ax0) cx = (cx + ((da > -kTiny) ? 1 : -1)) & (A.ncx - 1);
+            if (ax1) cy = (cy + ((db > -kTiny) ? 1 : -1)) & (A.ncy - 1);
+          } else {
+            if (ax0) { cx += (da > -kTiny) ? 1 : -1; cx = (cx == A.ncx) ? 0 : cx; cx = (cx < 0) ? A.ncx - 1 : cx; }
+            if (ax1) { cy += (db > -kTiny) ? 1 : -1; cy = (cy == A.ncy) ? 0 : cy; cy = (cy < 0) ? A.ncy - 1 : cy; }
+          }
+          if (ax2) cz += (dc > -kTiny) ? 1 : -1;
+          if ((unsigned)cz >= (unsigned)A.ncz) st = ST_BOUNDARY;   // surface (cz = -1) or domain top
+          else kh = __ldg(&A.khat[((size_t)cz * A.ncy + cy) * A.ncx + cx]);
+        }
+      }
+      continue;
+    }
+
+    // which parked phase: one that reached its batch size, or (nothing moves) the fullest one
+    int phase;
+    if (stuck) phase = (nC >= nS && nC >= nB) ? ST_COLLIDE : (nS >= nB ? ST_SCATTER : ST_BOUNDARY);
+    else       phase = (nC >= kCollideBatch) ? ST_COLLIDE : (nS >= kScatterBatch ? ST_SCATTER : ST_BOUNDARY);
+
+    if (phase == ST_SCATTER) {
       // ---- SCATTER: phase-function angle, rotation, new distances to the faces (§3.9) --------------
       if (st == ST_SCATTER) {
         const float qx = local(da, rx, A.Lx), qy = local(db, ry, A.Ly), qz = local(dc, rz, A.Lz);
@@ -217,15 +272,16 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
         direct = false; ++t_sc;
         st = ST_MOVE;
       }
-    } else if (st == ST_MOVE) {
-      // ---- MOVE: nearest face of the current cell (ties x < y < z), then collide or cross (§3.7) ----
-      int axis; float t;
-      if (rx <= ry && rx <= rz) { axis = 0; t = rx; }
-      else if (ry <= rz)        { axis = 1; t = ry; }
-      else                      { axis = 2; t = rz; }
-      const float dtau = kh * t;
-      if (kh > 0.0f && tau <= dtau) {
-        // §3.8 tentative collision inside this cell: fetch the voxel, classify, draw the next event
+      continue;
+    }
+
+    int fate = 0;
+    uint32_t term = 0;
+    unsigned long long* tally_a = nullptr;  // arrival / terminal bin
+    unsigned long long* tally_b = nullptr;  // surface absorption after an arrival tally
+    if (phase == ST_COLLIDE) {
+      // ---- COLLIDE: fetch the voxel, classify, draw the next event (§3.8) --------------------------
+      if (st == ST_COLLIDE) {
         const float s = tau * (1.0f / kh);
         rx = fmaxf(0.0f, rx - s); ry = fmaxf(0.0f, ry - s); rz = fmaxf(0.0f, rz - s);
         const float qx = local(da, rx, A.Lx), qy = local(db, ry, A.Ly), qz = local(dc, rz, A.Lz);
@@ -236,6 +292,7 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
         const float4 v = __ldg(&A.optics[vox]);
         ++t_ev;
         const float xi = u1 * kh;
+        st = ST_MOVE;
         if (xi < v.x) {                             // absorbed by the gas / droplet
           tally_a = A.atm_abs + vox;
           fate = 1; term = (uint32_t)vox;
@@ -253,56 +310,43 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
             draw();
           }
         }
-      } else {
-        // §3.7 leave the cell through `axis`, carrying the residual optical depth
-        tau = tau - dtau;
-        ++t_cells;
-        bool at_sfc = false, at_top = false;
-        if (axis == 0) {
-          ry = ry - t; rz = rz - t; rx = delx;
-          if (nudge(da) > 0.0f) { ++cx; if (cx == A.ncx) cx = 0; }
-          else                  { --cx; if (cx < 0) cx = A.ncx - 1; }
-        } else if (axis == 1) {
-          rx = rx - t; rz = rz - t; ry = dely;
-          if (nudge(db) > 0.0f) { ++cy; if (cy == A.ncy) cy = 0; }
-          else                  { --cy; if (cy < 0) cy = A.ncy - 1; }
-        } else {
-          rx = rx - t; ry = ry - t; rz = delz;
-          if (nudge(dc) > 0.0f) { ++cz; at_top = (cz == A.ncz); }
-          else                  { --cz; at_sfc = (cz < 0); }
-        }
-        if (at_sfc || at_top) {
-          const float qx = local(da, rx, A.Lx), qy = local(db, ry, A.Ly);
-          const int hx = cx * A.bx + min((int)(qx * A.rdx), A.bx - 1);
-          const int hy = cy * A.by + min((int)(qy * A.rdy), A.by - 1);
-          const size_t col = (size_t)hy * A.nx + hx;
-          if (at_top) {                             // §3.11 leaves through the domain top
-            tally_a = A.toa_up + col;
-            fate = 3; term = (uint32_t)col;
-          } else {                                  // §3.10 Lambertian surface
-            ++t_sfc;
-            tally_a = (direct ? A.sfc_dir : A.sfc_dif) + col;
-            if (u1 < __ldg(&A.albedo[col])) {
-              const float u2 = u24(w2);
-              const float mu = sqrtf(1.0f - u2), sn = sqrtf(u2);
-              float sp, cp;
-              sincos_2pi(u24(w3), sp, cp);
-              da = sn * cp; db = sn * sp; dc = mu;
-              direct = false; cz = 0;
-              place(qx, qy, 0.0f);
-              ++e;
-              if (e > kEventCap) { fate = 4; term = 0; }   // §3.12
-              else draw();
-            } else {
-              tally_b = A.sfc_abs + col;
-              fate = 2; term = (uint32_t)col;
+      }
+    } else {
+      // ---- BOUNDARY: arrival at the surface (§3.10) or exit through the domain top (§3.11) ----------
+      if (st == ST_BOUNDARY) {
+        const float qx = local(da, rx, A.Lx), qy = local(db, ry, A.Ly);
+        const int hx = cx * A.bx + min((int)(qx * A.rdx), A.bx - 1);
+        const int hy = cy * A.by + min((int)(qy * A.rdy), A.by - 1);
+        const size_t col = (size_t)hy * A.nx + hx;
+        if (cz >= 0) {                              // left through the domain top
+          tally_a = A.toa_up + col;
+          fate = 3; term = (uint32_t)col;
+        } else {                                    // Lambertian surface
+          ++t_sfc;
+          tally_a = (direct ? A.sfc_dir : A.sfc_dif) + col;
+          if (u1 < __ldg(&A.albedo[col])) {
+            const float u2 = u24(w2);
+            const float mu = sqrtf(1.0f - u2), sn = sqrtf(u2);
+            float sp, cp;
+            sincos_2pi(u24(w3), sp, cp);
+            da = sn * cp; db = sn * sp; dc = mu;
+            direct = false; cz = 0;
+            place(qx, qy, 0.0f);
+            ++e;
+            if (e > kEventCap) { fate = 4; term = 0; }   // §3.12
+            else {
+              draw();
+              kh = __ldg(&A.khat[((size_t)cz * A.ncy + cy) * A.ncx + cx]);
+              st = ST_MOVE;
             }
+          } else {
+            tally_b = A.sfc_abs + col;
+            fate = 2; term = (uint32_t)col;
           }
         }
-        if (fate == 0) kh = __ldg(&A.khat[((size_t)cz * A.ncy + cy) * A.ncx + cx]);
       }
-      if (fate != 0) st = ST_DEAD;
     }
+    if (fate != 0) st = ST_DEAD;
 
     // ---- tallies (converged): warp-aggregated 64-bit integer atomics -----------------------------
     const unsigned ma = __ballot_sync(0xffffffffu, tally_a != nullptr);
