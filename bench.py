@@ -123,6 +123,7 @@ def run_ours(args):
     import torch
     import torch.distributed as dist
     import paper_2208_05247_b200 as rt          # raises if the CUDA library is missing: no CPU fallback
+    from paper_2208_05247_b200.shard import weak_range
     from rt_inputs import CONFIGS, make_optics
 
     rank = int(os.environ.get("RANK", "0"))
@@ -173,7 +174,7 @@ def run_ours(args):
     def step(i, fields, out):
         g.reset_tallies()
         g.set_optics(*fields)                                    # S0 pack, S1 majorant
-        g.trace(cfg.zenith_deg, cfg.azimuth_deg, n, first_photon_id=(i * world + rank) * n, seed=cfg.seed)  # S2-S10
+        g.trace(cfg.zenith_deg, cfg.azimuth_deg, n, first_photon_id=weak_range(rank, world, i, n)[0], seed=cfg.seed)  # S2-S10
         t = g.read_tallies(out=out)                              # S11
         if t.counters.n_photons != n or t.counters.n_capped != 0:
             raise SystemExit("bench.py: photon count mismatch (%d of %d, %d capped)" % (

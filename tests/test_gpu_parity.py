@@ -126,6 +126,41 @@ def test_config2_sample():
     assert nb > 0 and rms < 0.02, (rms, nb)
 
 
+def test_config3_bench_configuration_sample():
+    """BASELINE.json configs[2] (512x512x128, the field bench.py times), same 2^3-voxel acceleration cells and
+    launch configuration: photon ids [0, 2^19) (two full passes over the columns) against the oracle in
+    kernel precision, record by record and tally by tally; then the full 2^26-photon launch checked through
+    properties that hold at any size (exact closure, counters consistent, no capped photon) and through
+    the sampled ids, whose records must not depend on how many other photons share the launch."""
+    rt = _rt()
+    cfg = CONFIGS[3]
+    opt = make_optics(cfg)
+    n = 1 << 19
+    g = rt.Grid(*cfg.grid, device=0)
+    g.set_optics(opt["k_ext"], opt["k_ext_cloud"], opt["ssa"], opt["g"], opt["sfc_albedo"])
+    rec = g.trace(cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed, records=True).cpu().numpy().view(np.uint32)
+    t = g.read_tallies()
+    o32, rec32, _ = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed, precision=32,
+                            records=True, n_threads=8)
+    assert np.array_equal(rec, rec32)
+    for name in ("atm_abs", "sfc_dir", "sfc_dif", "sfc_abs", "toa_up"):
+        assert np.array_equal(getattr(t, name).numpy(), getattr(o32, name)), name
+    assert t.counters.asdict() == o32.counters.asdict()
+    # the full launch bench.py times
+    g.reset_tallies()
+    N = cfg.n_photons
+    recN = g.trace(cfg.zenith_deg, cfg.azimuth_deg, N, seed=cfg.seed, records=True)
+    tN = g.read_tallies()
+    assert tN.closure() == N * rt.W0 and tN.counters.n_photons == N and tN.counters.n_capped == 0
+    c = tN.counters
+    assert c.n_events == c.n_null + c.n_rayleigh + c.n_hg + c.n_atm_abs
+    assert c.n_sfc_hits >= c.n_sfc_abs and int(tN.sfc_dir.sum() + tN.sfc_dif.sum()) == c.n_sfc_hits * rt.W0
+    assert int(tN.atm_abs.sum()) == c.n_atm_abs * rt.W0 and int(tN.toa_up.sum()) == c.n_toa * rt.W0
+    # ids below ncol * floor(N / ncol) launch from column id mod ncol in both runs: same records
+    assert np.array_equal(recN[:n].cpu().numpy().view(np.uint32), rec32)
+    g.close()
+
+
 def test_ragged_photon_count_and_offsets():
     """n not a multiple of ncol (remainder pass), non-zero first id and stream id, 33 photons, 0 photons."""
     rt = _rt()
