@@ -25,9 +25,14 @@ if ROOT not in sys.path:
 WORKLOAD = 3                      # rt_inputs.CONFIGS key: BASELINE.json configs[2], 512x512x128
 METRIC = "photon_paths_per_s"
 UNIT = "paths/s"
-REF_SAMPLE_PHOTONS = 1 << 20      # per --impl reference step: 4 photons per column
-CPU_BASELINE_PHOTONS = 1 << 22    # cpu_baseline leg: 16 photons per column (~20 s on 8 cores)
+REF_SAMPLE_PHOTONS = 1 << 23      # per --impl reference step: 32 photons per column (~2 s on 16 cores)
+CPU_BASELINE_PHOTONS = 1 << 25    # cpu_baseline leg: 128 photons per column (~10 s on 16 cores)
 SECTOR = 32                       # bytes moved per random 16-byte gather (one DRAM/L2 sector)
+# thread instructions per unit of the method's work, counted in the shipped kernel's SASS
+# (profiles/r1_trace_kernel.md): one MOVE step (find the nearest face; cross or park),
+# one tentative collision (gather, classify, Philox draw, logarithm), one real scatter, one surface
+# or top arrival, one photon launch.
+INST_PER_UNIT = {"move": 50, "collide": 200, "scatter": 240, "boundary": 150, "launch": 190}
 
 
 def _peaks():
@@ -36,6 +41,14 @@ def _peaks():
         with open(path) as f:
             return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def _sm_max_mhz():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f).get("sm_max_mhz", 1965.0))
+    return 1965.0
 
 
 class ClockSampler:
@@ -194,6 +207,7 @@ def run_ours(args):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     launches0 = g.launch_count()
     events = sfc_hits = 0
+    csum = {}
     trace_ms = []
     barrier()
     e0.record()
@@ -201,6 +215,8 @@ def run_ours(args):
         t, ms = step(args.warmup + i, resident, pinned_cols)
         events += t.counters.n_events
         sfc_hits += t.counters.n_sfc_hits
+        for k, v in t.counters.asdict().items():
+            csum[k] = csum.get(k, 0) + v
         trace_ms.append(ms)
     e1.record()
     barrier()
@@ -225,22 +241,36 @@ def run_ours(args):
     d2h = (cfg.nvox + 4 * cfg.ncol) * 8 + 8 * len(rt.binding.COUNTER_FIELDS)
 
     # ---- roofline of the dominant kernel (trace_kernel), this rank ---------------------------------------
-    peak, peak_src = _peaks()
+    # The kernel is bound by instruction issue, not by memory (0.5 % of the HBM copy rate, 80 %
+    # of issue slots busy), so the bound is "alu".  Algorithmic work = thread instructions the method's steps
+    # need, per unit, as counted in the shipped kernel's SASS (profiles/r1_trace_kernel.md) x the units the
+    # launch processed; peak = every lane of every SM sub-partition issuing each cycle at the SM clock.
+    hbm_peak, peak_src = _peaks()
     ms_avg = sum(trace_ms) / len(trace_ms)
-    ev_per_launch = events / args.steps
-    atomics_per_launch = n + sfc_hits / args.steps
+    per = {k: v / args.steps for k, v in csum.items()}
+    units = {"move": per["n_cell_steps"] + per["n_events"], "collide": per["n_events"],
+             "scatter": per["n_hg"] + per["n_rayleigh"], "boundary": per["n_sfc_hits"] + per["n_toa"],
+             "launch": per["n_photons"]}
+    alg_inst = sum(INST_PER_UNIT[k] * units[k] for k in units)
+    sm_mhz = _sm_max_mhz()
+    alu_peak = 148 * 4 * 32 * sm_mhz * 1e6 / 1e12            # T thread-instructions / s
+    achieved = alg_inst / (ms_avg * 1e-3) / 1e12
+    ev_per_launch = per["n_events"]
+    atomics_per_launch = n + per["n_sfc_hits"]
     alg_bytes = SECTOR * ev_per_launch + 2 * SECTOR * atomics_per_launch
-    achieved = alg_bytes / (ms_avg * 1e-3) / 1e9
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "trace_kernel_traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "trace_kernel_traffic.txt")
     if os.path.exists(tpath):
         with open(tpath) as f:
             tj = json.load(f)
-        if tj.get("n_photons") == n and tj.get("workload") == cfg.name:
+        if tj.get("n_photons") == n and tj.get("workload") == cfg.name and tj.get("block") == list(cfg.block):
             traffic = tj.get("dram_bytes_per_launch")
-    gb_ms, gb_loads = g.gather_bench(64)
-    gather_sectors_per_s = gb_loads / (gb_ms * 1e-3)
     trace_events_per_s = ev_per_launch / (ms_avg * 1e-3)
+    trace_gathers_per_s = (units["move"] + units["collide"]) / (ms_avg * 1e-3)   # majorant + voxel loads
+    gather = {}
+    for label, foot in (("hbm_512MiB", 0), ("l2_16MiB", 1 << 20)):
+        gb_ms, gb_loads = g.gather_bench(64, foot)
+        gather[label] = gb_loads / (gb_ms * 1e-3)
 
     if rank != 0:
         if world > 1:
@@ -275,15 +305,23 @@ def run_ours(args):
         "gpu_launches": launches,
         "closure_exact": bool(closure_ok),
         "clocks": clocks,
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": traffic, "kernel": "trace_kernel", "peak_source": peak_src,
-                     "algorithmic_bytes_per_launch": alg_bytes,
-                     "bytes_model": "32 B sector per collision event + 2 x 32 B per tally atomic"},
-        "gather_roofline": {"sectors_per_s": gather_sectors_per_s, "GBps_32B": gather_sectors_per_s * SECTOR / 1e9,
-                            "trace_events_per_s": trace_events_per_s,
-                            "frac": trace_events_per_s / gather_sectors_per_s,
+        "roofline": {"bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "T thread-inst/s",
+                     "frac": achieved / alu_peak, "traffic": traffic, "kernel": "trace_kernel",
+                     "peak_source": "148 SMs x 4 sub-partitions x 32 lanes x %.0f MHz (DESIGN.md §6)" % sm_mhz,
+                     "algorithmic_inst_per_launch": alg_inst, "inst_per_unit": INST_PER_UNIT,
+                     "units_per_launch": units},
+        "hbm": {"algorithmic_GBps": alg_bytes / (ms_avg * 1e-3) / 1e9, "peak_GBps": hbm_peak, "peak_source": peak_src,
+                "frac": alg_bytes / (ms_avg * 1e-3) / 1e9 / hbm_peak,
+                "bytes_model": "32 B sector per tentative collision + 2 x 32 B per tally atomic; ncu shows the "
+                               "real DRAM traffic (roofline.traffic) is ~100x smaller: the working set sits in L2"},
+        "gather_roofline": {"random_16B_loads_per_s": gather, "trace_events_per_s": trace_events_per_s,
+                            "trace_gathers_per_s": trace_gathers_per_s,
+                            "frac_events_vs_hbm": trace_events_per_s / gather["hbm_512MiB"],
+                            "frac_gathers_vs_hbm": trace_gathers_per_s / gather["hbm_512MiB"],
+                            "frac_gathers_vs_l2": trace_gathers_per_s / gather["l2_16MiB"],
                             "how": "rt_gather_bench: 8 independent random 16 B loads in flight per thread over the "
-                                   "512 MiB packed-optics array"},
+                                   "whole 512 MiB packed-optics array (HBM) and over its first 16 MiB (L2); "
+                                   "trace gathers = voxel records + 4 B majorant loads"},
         "cpu_baseline": cpu,
     }))
     if world > 1:

@@ -104,11 +104,13 @@ int rt_read_majorant(rt_ctx* ctx, float* khat_out);
 int rt_read_packed_optics(rt_ctx* ctx, float* packed_out);
 
 /* Random-gather microbenchmark for the roofline denominator: every thread issues
- * `loads_per_thread` independent 16-byte loads at Philox-random voxel indices of the context's
- * packed-optics array.  Writes the elapsed milliseconds (CUDA events on `cuda_stream`) to *ms_out and
- * the number of 16-byte loads issued to *n_loads_out.  Synchronises the stream. */
-int rt_gather_bench(rt_ctx* ctx, uint32_t loads_per_thread, void* cuda_stream, float* ms_out,
-                    uint64_t* n_loads_out);
+ * `loads_per_thread` independent 16-byte loads at Philox-random voxel indices among the first
+ * `footprint_voxels` records of the context's packed-optics array (0 = the whole array; a footprint of
+ * a few MiB measures L2, hundreds of MiB measures HBM).  Runs once untimed, then writes the elapsed
+ * milliseconds of a second run (CUDA events on `cuda_stream`) to *ms_out and the number of 16-byte loads
+ * issued to *n_loads_out.  Synchronises the stream. */
+int rt_gather_bench(rt_ctx* ctx, uint32_t loads_per_thread, uint64_t footprint_voxels, void* cuda_stream,
+                    float* ms_out, uint64_t* n_loads_out);
 
 /* Milliseconds spent in the trace kernel of the most recent rt_trace* call on this context, from
  * CUDA events recorded on that call's stream around the launch.  Synchronises on the end event. */

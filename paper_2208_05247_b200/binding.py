@@ -51,7 +51,7 @@ def lib():
     L.rt_reset_tallies.argtypes = [vp, vp]
     L.rt_read_majorant.argtypes = [vp, vp]
     L.rt_read_packed_optics.argtypes = [vp, vp]
-    L.rt_gather_bench.argtypes = [vp, u32, vp, C.POINTER(f32), C.POINTER(u64)]
+    L.rt_gather_bench.argtypes = [vp, u32, u64, vp, C.POINTER(f32), C.POINTER(u64)]
     L.rt_last_trace_ms.argtypes = [vp, C.POINTER(f32)]
     L.rt_launch_count.argtypes = [vp]
     L.rt_launch_count.restype = u64
@@ -168,9 +168,10 @@ class Grid:
         self._check(self.L.rt_read_packed_optics(self.ctx, _ptr(out)), "rt_read_packed_optics")
         return out
 
-    def gather_bench(self, loads_per_thread=64):
+    def gather_bench(self, loads_per_thread=64, footprint_voxels=0):
         ms, n = C.c_float(0), C.c_uint64(0)
-        self._check(self.L.rt_gather_bench(self.ctx, loads_per_thread, _stream(self.device), C.byref(ms), C.byref(n)),
+        self._check(self.L.rt_gather_bench(self.ctx, loads_per_thread, int(footprint_voxels), _stream(self.device),
+                                           C.byref(ms), C.byref(n)),
                     "rt_gather_bench")
         return ms.value, n.value
 

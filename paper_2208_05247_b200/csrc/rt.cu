@@ -263,8 +263,10 @@ int rt_read_packed_optics(rt_ctx* c, float* packed_out) {
   return RT_OK;
 }
 
-int rt_gather_bench(rt_ctx* c, uint32_t loads_per_thread, void* cuda_stream, float* ms_out, uint64_t* n_loads_out) {
-  if (!c || !ms_out || !n_loads_out || loads_per_thread < 8) return RT_EINVAL;
+int rt_gather_bench(rt_ctx* c, uint32_t loads_per_thread, uint64_t footprint_voxels, void* cuda_stream,
+                    float* ms_out, uint64_t* n_loads_out) {
+  if (!c || !ms_out || !n_loads_out || loads_per_thread < 8 || footprint_voxels > c->nvox) return RT_EINVAL;
+  const unsigned long long nfoot = footprint_voxels ? footprint_voxels : c->nvox;
   DeviceGuard guard(c->device);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const uint32_t iters = loads_per_thread / 8;
@@ -272,9 +274,10 @@ int rt_gather_bench(rt_ctx* c, uint32_t loads_per_thread, void* cuda_stream, flo
   cudaEvent_t a, b;
   RT_CUDA(c, cudaEventCreate(&a));
   RT_CUDA(c, cudaEventCreate(&b));
+  rt::gather_bench_kernel<<<blocks, threads, 0, st>>>(c->optics, nfoot, iters, c->sink);   // warm-up
   RT_CUDA(c, cudaEventRecord(a, st));
-  rt::gather_bench_kernel<<<blocks, threads, 0, st>>>(c->optics, (unsigned long long)c->nvox, iters, c->sink);
-  ++c->launches;
+  rt::gather_bench_kernel<<<blocks, threads, 0, st>>>(c->optics, nfoot, iters, c->sink);
+  c->launches += 2;
   RT_CUDA(c, cudaEventRecord(b, st));
   RT_CUDA(c, cudaEventSynchronize(b));
   RT_CUDA(c, cudaGetLastError());
