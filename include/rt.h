@@ -54,7 +54,7 @@ typedef struct {
 
 /* Allocate a context for an nx*ny*nz grid of dx*dy*dz metre voxels with an acceleration grid
  * of bx*by*bz-voxel blocks ("coarser resolution than the simulation"; Q1).
- * nx,ny,nz must be multiples of bx,by,bz; bx*by*bz <= 4096.  Allocates packed optics
+ * nx,ny,nz must be multiples of bx,by,bz; bx*by*bz <= 4096; nx*ny*nz < 2^32.  Allocates packed optics
  * (16 B/voxel), the majorant grid and zeroed int64 tallies on cuda_device.  *out is owned
  * by the library until rt_destroy. */
 int rt_create_grid(rt_ctx** out, int nx, int ny, int nz, float dx, float dy, float dz, int bx, int by,

@@ -102,7 +102,7 @@ int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photon
   A.records = records;
   A.n_photons = n_photons; A.first_id = first_id; A.ncol = c->ncol;
   A.n_full = (n_photons / c->ncol) * c->ncol;
-  A.key0 = (uint32_t)seed; A.key1 = (uint32_t)(seed >> 32); A.stream_id = stream_id;
+  A.keys = rt::philox_round_keys((uint32_t)seed, (uint32_t)(seed >> 32)); A.stream_id = stream_id;
   RT_CUDA(c, cudaMemsetAsync(A.next_photon, 0, sizeof(unsigned long long), st));
   RT_CUDA(c, cudaEventRecord(c->ev0, st));
   if (n_photons > 0) {
@@ -133,6 +133,7 @@ int rt_create_grid(rt_ctx** out, int nx, int ny, int nz, float dx, float dy, flo
   if (nx <= 0 || ny <= 0 || nz <= 0 || bx <= 0 || by <= 0 || bz <= 0) return RT_EINVAL;
   if (nx % bx || ny % by || nz % bz || (long long)bx * by * bz > 4096) return RT_EINVAL;
   if (!(dx > 0.0f) || !(dy > 0.0f) || !(dz > 0.0f)) return RT_EINVAL;
+  if ((unsigned long long)nx * ny * nz >= (1ull << 32)) return RT_EINVAL;   // voxel indices are 32-bit in the kernels
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || cuda_device < 0 || cuda_device >= ndev) return RT_ECUDA;
   rt_ctx* c = new rt_ctx();

@@ -71,7 +71,8 @@ struct TraceArgs {
   unsigned long long* next_photon;     // work counter, zeroed before launch
   uint32_t* records;                   // 4 words per photon or nullptr
   unsigned long long n_photons, first_id, n_full, ncol;
-  uint32_t key0, key1, stream_id;
+  PhiloxKeys keys;                     // round keys of the Philox key (seed)
+  uint32_t stream_id;
 };
 
 // Add kW0 to *p once per distinct address among the lanes of `mask` (warp-aggregated tally).
@@ -122,7 +123,7 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
 
   auto draw = [&]() {
     const unsigned long long pid = A.first_id + i;
-    const uint4 X = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), e, A.stream_id, A.key0, A.key1);
+    const uint4 X = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), e, A.stream_id, A.keys);
     tau = neg_log(1.0f - u24(X.x)); u1 = u24(X.y); w2 = X.z; w3 = X.w;
   };
   // local coordinate from a remaining distance: q = face - v r, face = L if v > 0 else 0
@@ -188,7 +189,7 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
       if (got) {
         // ---- §3.6 launch, event index 0 ------------------------------------------------------
         const unsigned long long pid = A.first_id + i;
-        const uint4 X = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), 0u, A.stream_id, A.key0, A.key1);
+        const uint4 X = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), 0u, A.stream_id, A.keys);
         int ix, iy;
         if (i < A.n_full) {
           // column = i mod ncol; 32-bit arithmetic whenever the index allows it
@@ -210,7 +211,7 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
         e = 1;
         if (kRecords) { b_ev = t_ev; b_sc = t_sc; b_sfc = t_sfc; }
         draw();
-        kh = __ldg(&A.khat[((size_t)cz * A.ncy + cy) * A.ncx + cx]);
+        kh = __ldg(A.khat + (((unsigned)cz * (unsigned)A.ncy + (unsigned)cy) * (unsigned)A.ncx + (unsigned)cx));
         st = ST_MOVE;
       }
       continue;
@@ -247,7 +248,7 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
           }
           if (ax2) cz += (dc > -kTiny) ? 1 : -1;
           if ((unsigned)cz >= (unsigned)A.ncz) st = ST_BOUNDARY;   // surface (cz = -1) or domain top
-          else kh = __ldg(&A.khat[((size_t)cz * A.ncy + cy) * A.ncx + cx]);
+          else kh = __ldg(A.khat + (((unsigned)cz * (unsigned)A.ncy + (unsigned)cy) * (unsigned)A.ncx + (unsigned)cx));
         }
       }
       continue;
@@ -288,7 +289,9 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
         const int lx = min((int)(qx * A.rdx), A.bx - 1);
         const int ly = min((int)(qy * A.rdy), A.by - 1);
         const int lz = min((int)(qz * A.rdz), A.bz - 1);
-        const size_t vox = ((size_t)(cz * A.bz + lz) * A.ny + (cy * A.by + ly)) * A.nx + (cx * A.bx + lx);
+        // 32-bit indices: rt_create_grid refuses grids of 2^32 voxels or more
+        const unsigned vox = ((unsigned)(cz * A.bz + lz) * (unsigned)A.ny + (unsigned)(cy * A.by + ly)) * (unsigned)A.nx
+                             + (unsigned)(cx * A.bx + lx);
         const float4 v = __ldg(&A.optics[vox]);
         ++t_ev;
         const float xi = u1 * kh;
@@ -317,7 +320,7 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
         const float qx = local(da, rx, A.Lx), qy = local(db, ry, A.Ly);
         const int hx = cx * A.bx + min((int)(qx * A.rdx), A.bx - 1);
         const int hy = cy * A.by + min((int)(qy * A.rdy), A.by - 1);
-        const size_t col = (size_t)hy * A.nx + hx;
+        const unsigned col = (unsigned)hy * (unsigned)A.nx + (unsigned)hx;
         if (cz >= 0) {                              // left through the domain top
           tally_a = A.toa_up + col;
           fate = 3; term = (uint32_t)col;
@@ -336,7 +339,7 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
             if (e > kEventCap) { fate = 4; term = 0; }   // §3.12
             else {
               draw();
-              kh = __ldg(&A.khat[((size_t)cz * A.ncy + cy) * A.ncx + cx]);
+              kh = __ldg(A.khat + (((unsigned)cz * (unsigned)A.ncy + (unsigned)cy) * (unsigned)A.ncx + (unsigned)cx));
               st = ST_MOVE;
             }
           } else {
