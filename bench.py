@@ -22,7 +22,8 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-WORKLOAD = 3                      # rt_inputs.CONFIGS key: BASELINE.json configs[2], 512x512x128
+WORKLOAD = 3                      # default rt_inputs.CONFIGS key: BASELINE.json configs[2], 512x512x128 (the
+                                  # configuration the metric is quoted on); --workload N times another config
 METRIC = "photon_paths_per_s"
 UNIT = "paths/s"
 REF_SAMPLE_PHOTONS = 1 << 23      # per --impl reference step: 32 photons per column (~2 s on 16 cores)
@@ -103,7 +104,7 @@ def run_reference(args):
         return
     import oracle as O
     from rt_inputs import CONFIGS, make_optics
-    cfg = CONFIGS[WORKLOAD]
+    cfg = CONFIGS[args.workload if args.workload != 4 else 3]   # the spectral sweep's field is config 3's
     opt = make_optics(cfg)
     cores = O.hardware_threads()
     n = REF_SAMPLE_PHOTONS
@@ -168,31 +169,52 @@ def run_ours(args):
         dist.all_reduce(t, op=dist.ReduceOp.SUM)
         return float(t.item())
 
-    cfg = CONFIGS[WORKLOAD]
+    cfg = CONFIGS[args.workload]
     if args.block:
         from dataclasses import replace
         cfg = replace(cfg, block=tuple(int(x) for x in args.block.split(",")))
     opt = make_optics(cfg)                       # seeded: every rank builds the same field
     names = ("k_ext", "k_ext_cloud", "ssa", "g", "sfc_albedo")
-    host = [torch.from_numpy(opt[k]).pin_memory() for k in names]
-    resident = [t.to(dev) for t in host]
+    spectral = args.workload == 4
+    host = [torch.from_numpy(opt[k]).pin_memory() for k in names] if not spectral else None
     n = cfg.n_photons                            # per GPU (weak scaling: photon ids are sharded by rank)
     g = rt.Grid(*cfg.grid, device=local)
     pinned_cols = rt.Tallies(None, *[torch.empty((cfg.ny, cfg.nx), dtype=torch.int64).pin_memory() for _ in range(4)],
                              counters=None)
-    pinned_all = rt.Tallies(torch.empty((cfg.nz, cfg.ny, cfg.nx), dtype=torch.int64).pin_memory(),
-                            pinned_cols.sfc_dir, pinned_cols.sfc_dif, pinned_cols.sfc_abs, pinned_cols.toa_up,
-                            counters=None)
+    if spectral:
+        # BASELINE.json configs[3]: 112 spectral points, each its own optics on the same cloud field, photons
+        # split by irradiance weight; all 112 field sets resident in HBM (43 GB of the 180 GB) before timing
+        from rt_inputs import make_optics_torch, spectral_points, split_photons
+        from paper_2208_05247_b200.sweeps import spectral_sweep
+        pts = spectral_points(112)
+        counts = split_photons(n, [p["weight"] for p in pts])
+        resident = [[make_optics_torch(cfg, p, device=dev)[k] for k in names] for p in pts]
+        pinned_all = None
+    else:
+        resident = [t.to(dev) for t in host]
+        pinned_all = rt.Tallies(torch.empty((cfg.nz, cfg.ny, cfg.nx), dtype=torch.int64).pin_memory(),
+                                pinned_cols.sfc_dir, pinned_cols.sfc_dif, pinned_cols.sfc_abs, pinned_cols.toa_up,
+                                counters=None)
+    point_ms = []
 
     def step(i, fields, out):
         g.reset_tallies()
-        g.set_optics(*fields)                                    # S0 pack, S1 majorant
-        g.trace(cfg.zenith_deg, cfg.azimuth_deg, n, first_photon_id=weak_range(rank, world, i, n)[0], seed=cfg.seed)  # S2-S10
+        first = weak_range(rank, world, i, n)[0]
+        if spectral:
+            tm = []
+            spectral_sweep(g, lambda j: fields[j], counts, cfg.zenith_deg, cfg.azimuth_deg, seed=cfg.seed,
+                           first_photon_id=first, timings=tm)    # 112 x (S0, S1, S2-S10)
+            ms = sum(x[1] for x in tm)
+            point_ms[:] = tm
+        else:
+            g.set_optics(*fields)                                    # S0 pack, S1 majorant
+            g.trace(cfg.zenith_deg, cfg.azimuth_deg, n, first_photon_id=first, seed=cfg.seed)  # S2-S10
+            ms = None
         t = g.read_tallies(out=out)                              # S11
         if t.counters.n_photons != n or t.counters.n_capped != 0:
             raise SystemExit("bench.py: photon count mismatch (%d of %d, %d capped)" % (
                 t.counters.n_photons, n, t.counters.n_capped))
-        return t, g.last_trace_ms()
+        return t, (g.last_trace_ms() if ms is None else ms)
 
     for i in range(args.warmup):
         step(i, resident, pinned_cols)
@@ -230,15 +252,19 @@ def run_ours(args):
     value = total_photons / (elapsed_ms * 1e-3)
 
     # ---- end-to-end leg: host fields in, all tallies out to the host, every step --------------------------
-    step(0, host, pinned_all)
-    barrier()
-    t0 = time.perf_counter()
-    for i in range(args.steps):
-        step(args.warmup + args.steps + i, host, pinned_all)
-    barrier()
-    e2e_s = max_over_ranks(time.perf_counter() - t0)
-    h2d = sum(x.numel() * x.element_size() for x in host)
-    d2h = (cfg.nvox + 4 * cfg.ncol) * 8 + 8 * len(rt.binding.COUNTER_FIELDS)
+    e2e = None
+    if not spectral:
+        step(0, host, pinned_all)
+        barrier()
+        t0 = time.perf_counter()
+        for i in range(args.steps):
+            step(args.warmup + args.steps + i, host, pinned_all)
+        barrier()
+        e2e_s = max_over_ranks(time.perf_counter() - t0)
+        h2d = sum(x.numel() * x.element_size() for x in host)
+        d2h = (cfg.nvox + 4 * cfg.ncol) * 8 + 8 * len(rt.binding.COUNTER_FIELDS)
+        e2e = {"value": total_photons / e2e_s, "unit": UNIT, "ms_per_step": 1e3 * e2e_s / args.steps,
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h}
 
     # ---- roofline of the dominant kernel (trace_kernel), this rank ---------------------------------------
     # The kernel is bound by instruction issue, not by memory (0.5 % of the HBM copy rate, 80 %
@@ -268,7 +294,7 @@ def run_ours(args):
     trace_events_per_s = ev_per_launch / (ms_avg * 1e-3)
     trace_gathers_per_s = (units["move"] + units["collide"]) / (ms_avg * 1e-3)   # majorant + voxel loads
     gather = {}
-    for label, foot in (("hbm_512MiB", 0), ("l2_16MiB", 1 << 20)):
+    for label, foot in (("hbm_512MiB", 0), ("l2_16MiB", min(1 << 20, cfg.nvox))):   # labels name config 3's sizes
         gb_ms, gb_loads = g.gather_bench(64, foot)
         gather[label] = gb_loads / (gb_ms * 1e-3)
 
@@ -298,10 +324,13 @@ def run_ours(args):
         "config": {"workload": cfg.name, "grid": [cfg.nx, cfg.ny, cfg.nz], "photons_per_gpu_per_step": n,
                    "block": list(cfg.block), "zenith_deg": cfg.zenith_deg, "azimuth_deg": cfg.azimuth_deg,
                    "parallelism": "photon-id ranges per GPU, no collective" if world > 1 else "1 GPU",
-                   "l2": "inputs exceed L2 (512 MiB packed optics + 256 MiB tallies vs 126 MB)",
-                   "step": "reset_tallies + set_optics + trace + read_tallies(column tallies, counters)"},
-        "e2e": {"value": total_photons / e2e_s, "unit": UNIT, "ms_per_step": 1e3 * e2e_s / args.steps,
-                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+                   "l2": ("inputs exceed L2 (%d MiB packed optics + %d MiB tallies vs 126 MB)" % (
+                       cfg.nvox * 16 >> 20, cfg.nvox * 8 >> 20)) if cfg.nvox * 24 > (126 << 20) else
+                         "inputs fit L2; every step traces new photon ids",
+                   "step": ("reset_tallies + 112 x (set_optics + trace, stream_id = point) + read_tallies"
+                            if spectral else
+                            "reset_tallies + set_optics + trace + read_tallies(column tallies, counters)")},
+        "e2e": e2e,
         "gpu_launches": launches,
         "closure_exact": bool(closure_ok),
         "clocks": clocks,
@@ -334,6 +363,8 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
+    ap.add_argument("--workload", type=int, choices=(1, 2, 3, 4, 5), default=WORKLOAD,
+                    help="BASELINE.json configs[N-1]; the default (3) is the configuration the metric is quoted on")
     ap.add_argument("--block", default=None, help="acceleration-grid block bx,by,bz (default: the config's)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing (used under ncu)")
     args = ap.parse_args()

@@ -199,3 +199,36 @@ def plane_parallel(nx, ny, nz, dx, dy, dz, k_ext, ssa, g=0.0, cloud_frac=0.0, al
 
 def with_photons(cfg: Config, n):
     return replace(cfg, n_photons=int(n))
+
+
+def make_optics_torch(cfg: Config, spectral=None, device="cuda"):
+    """make_optics() assembled on a torch device (same IEEE fp64 operations in the same order, then one
+    rounding to fp32), for sweeps that re-set the optics many times (config 4).  The cloud field comes from
+    the numpy generator and is cached on the device."""
+    import torch
+    make_optics(cfg) if spectral is None else None        # fills the host cloud cache if needed
+    key = (cfg.nx, cfg.ny, cfg.nz, cfg.dx, cfg.dy, cfg.dz, cfg.n_blobs, cfg.name.startswith("tiny_box"))
+    if key not in _cloud_cache:
+        make_optics(cfg)
+    dkey = key + (str(device),)
+    if dkey not in _cloud_cache_dev:
+        _cloud_cache_dev.clear()
+        _cloud_cache_dev[dkey] = torch.from_numpy(_cloud_cache[key]).to(device)
+    kc = _cloud_cache_dev[dkey]
+    p = spectral or {"k_abs0": cfg.k_abs0, "k_ray0": cfg.k_ray0, "cloud_ssa": cfg.cloud_ssa, "cloud_g": cfg.cloud_g}
+    zc = (np.arange(cfg.nz) + 0.5) * cfg.dz
+    prof = np.ones(cfg.nz) if cfg.name.startswith("tiny_box") else np.exp(-zc / SCALE_HEIGHT)
+    k_abs = torch.from_numpy(p["k_abs0"] * prof).to(device)[:, None, None]
+    k_ray = torch.from_numpy(p["k_ray0"] * prof).to(device)[:, None, None]
+    k_ext = k_abs + k_ray + kc
+    ssa = (k_ray + p["cloud_ssa"] * kc) / k_ext
+    return {
+        "k_ext": k_ext.float(),
+        "k_ext_cloud": kc.float(),
+        "ssa": ssa.float(),
+        "g": torch.full(kc.shape, p["cloud_g"], dtype=torch.float32, device=device),
+        "sfc_albedo": torch.full((cfg.ny, cfg.nx), cfg.sfc_albedo, dtype=torch.float32, device=device),
+    }
+
+
+_cloud_cache_dev = {}

@@ -1,0 +1,111 @@
+"""BASELINE.json configs[3] (spectral sweep, 112 points on the 512x512x128 field) and configs[4] (convergence
+sweep on 1024x1024x192) on the GPU, through the C ABI, against the oracle.
+
+Whole sweeps are checked by what holds at any size (closure bit-exact in fixed point, counter identities,
+no capped photon, the paper's N^-1/2 noise law); sampled launches are compared with the oracle in
+kernel precision record by record and tally by tally."""
+import numpy as np
+import pytest
+import torch
+
+import oracle as O
+from rt_inputs import CONFIGS, make_optics, make_optics_torch, spectral_points, split_photons
+
+pytestmark = pytest.mark.gpu
+
+NAMES = ("k_ext", "k_ext_cloud", "ssa", "g", "sfc_albedo")
+TALLIES = ("atm_abs", "sfc_dir", "sfc_dif", "sfc_abs", "toa_up")
+
+
+def _rt():
+    import paper_2208_05247_b200 as rt
+    return rt
+
+
+def test_config4_spectral_sweep():
+    rt = _rt()
+    from paper_2208_05247_b200.sweeps import spectral_sweep
+    cfg = CONFIGS[4]
+    pts = spectral_points(112)
+    counts = split_photons(cfg.n_photons, [p["weight"] for p in pts])
+    assert sum(counts) == cfg.n_photons and len(counts) == 112 and min(counts) > 0
+    g = rt.Grid(*cfg.grid, device=0)
+
+    # the device-side field assembly hands the library the same fp32 arrays as the host recipe
+    sample = (0, 37, 111)
+    host_opt = {}
+    for j in sample:
+        host_opt[j] = make_optics(cfg, pts[j])
+        dev = make_optics_torch(cfg, pts[j])
+        for k in NAMES:
+            assert np.array_equal(dev[k].cpu().numpy().view(np.uint32), host_opt[j][k].view(np.uint32)), (j, k)
+
+    # sampled points: 2^17 photons each (not a multiple of ncol: all launch from random columns),
+    # stream_id = j, against the oracle in kernel precision
+    n = 1 << 17
+    for j in sample:
+        opt = host_opt[j]
+        g.reset_tallies()
+        g.set_optics(*[opt[k] for k in NAMES])
+        rec = g.trace(cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed, stream_id=j, records=True)
+        t = g.read_tallies()
+        o32, rec32, _ = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed, stream_id=j,
+                                precision=32, records=True, n_threads=8)
+        assert np.array_equal(rec.cpu().numpy().view(np.uint32), rec32), j
+        for name in TALLIES:
+            assert np.array_equal(getattr(t, name).numpy(), getattr(o32, name)), (j, name)
+        assert t.counters.asdict() == o32.counters.asdict()
+    del host_opt
+
+    # the whole sweep: 112 x (rt_set_optics + rt_trace), tallies accumulated over the points
+    g.reset_tallies()
+    total = spectral_sweep(g, lambda j: [make_optics_torch(cfg, pts[j])[k] for k in NAMES], counts,
+                           cfg.zenith_deg, cfg.azimuth_deg, seed=cfg.seed)
+    t = g.read_tallies()
+    c = t.counters
+    assert total == cfg.n_photons and c.n_photons == total and c.n_capped == 0
+    assert t.closure() == total * rt.W0
+    assert c.n_events == c.n_null + c.n_rayleigh + c.n_hg + c.n_atm_abs
+    assert int(t.sfc_dir.sum() + t.sfc_dif.sum()) == c.n_sfc_hits * rt.W0
+    assert int(t.atm_abs.sum()) == c.n_atm_abs * rt.W0 and int(t.toa_up.sum()) == c.n_toa * rt.W0
+    # a sweep in which many points absorb strongly: broadband absorption well above the single-point config 3
+    assert 0.05 < c.n_atm_abs / total < 0.9
+    g.close()
+
+
+def test_config5_convergence_sweep():
+    rt = _rt()
+    from paper_2208_05247_b200.sweeps import convergence_sweep
+    cfg = CONFIGS[5]
+    opt = make_optics(cfg)
+    g = rt.Grid(*cfg.grid, device=0)
+    g.set_optics(*[opt[k] for k in NAMES])
+
+    # 1 photon per column (2^20 photons, one full pass) against the oracle in kernel precision
+    n = cfg.ncol
+    rec = g.trace(cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed, records=True).cpu().numpy().view(np.uint32)
+    t = g.read_tallies()
+    o32, rec32, _ = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed, precision=32,
+                            records=True, n_threads=8)
+    assert np.array_equal(rec, rec32)
+    for name in TALLIES:
+        assert np.array_equal(getattr(t, name).numpy(), getattr(o32, name)), name
+    assert t.counters.asdict() == o32.counters.asdict()
+    del t, o32, rec, rec32
+
+    per_column = (1, 4, 16, 64, 256)
+    rows, ref = convergence_sweep(g, cfg.ncol, per_column, cfg.zenith_deg, cfg.azimuth_deg, seed=cfg.seed,
+                                  sfc_block=(16, 16), vox_block=(16, 32, 32), min_hits=500)
+    print(rows)                                   # shown with pytest -s: the sweep table of DESIGN.md §6
+    g.close()
+    assert [r["photons_per_column"] for r in rows] == list(per_column)
+    for r in rows:
+        assert r["closure_exact"] and r["n_capped"] == 0
+        assert r["sfc_blocks"] >= 1000 and r["heating_blocks"] >= 100
+    # the noise falls as N^-1/2.  With an independent 256-per-column reference the expected RMS
+    # difference is c sqrt(1/N + 1/256): c is the same at every N (15 % covers its own sampling error and
+    # the non-Poisson part of the surface tally, whose direct beam is stratified by column)
+    for key in ("rms_noise_sfc", "rms_noise_heating"):
+        c = [r[key] / np.sqrt(1.0 / r["photons_per_column"] + 1.0 / ref["photons_per_column"]) for r in rows]
+        assert max(c) / min(c) < 1.15, (key, c)
+        assert rows[0][key] > 4 * rows[3][key]        # 64x the photons: ~ sqrt((1+1/256)/(1/64+1/256)) = 7.2
