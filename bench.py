@@ -111,7 +111,7 @@ def run_reference(args):
     times, events = [], 0
     for step in range(args.warmup + args.steps):
         t, _, el = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, first_photon_id=step * n,
-                           seed=cfg.seed, precision=64, n_threads=cores)
+                           seed=cfg.seed, precision=64, n_threads=cores, **cfg.accel)
         assert t.closure() == n * O.W0
         if step >= args.warmup:
             times.append(el)
@@ -173,12 +173,15 @@ def run_ours(args):
     if args.block:
         from dataclasses import replace
         cfg = replace(cfg, block=tuple(int(x) for x in args.block.split(",")))
+    if args.merge:
+        from dataclasses import replace
+        cfg = replace(cfg, merge=tuple(int(x) for x in args.merge.split(",")))
     opt = make_optics(cfg)                       # seeded: every rank builds the same field
     names = ("k_ext", "k_ext_cloud", "ssa", "g", "sfc_albedo")
     spectral = args.workload == 4
     host = [torch.from_numpy(opt[k]).pin_memory() for k in names] if not spectral else None
     n = cfg.n_photons                            # per GPU (weak scaling: photon ids are sharded by rank)
-    g = rt.Grid(*cfg.grid, device=local)
+    g = rt.Grid(*cfg.grid, device=local, **cfg.accel)
     pinned_cols = rt.Tallies(None, *[torch.empty((cfg.ny, cfg.nx), dtype=torch.int64).pin_memory() for _ in range(4)],
                              counters=None)
     if spectral:
@@ -308,7 +311,7 @@ def run_ours(args):
         import oracle as O
         cores = O.hardware_threads()
         ot, _, el = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, CPU_BASELINE_PHOTONS, seed=cfg.seed,
-                            precision=64, n_threads=cores)
+                            precision=64, n_threads=cores, **cfg.accel)
         cpu = {"value": CPU_BASELINE_PHOTONS / el, "unit": UNIT, "cores": cores, "kind": "oracle",
                "collision_events_per_s": ot.counters.n_events / el,
                "sample": "photon ids [0, %d) (%d per column) of the %d-photon workload, photon loop only" % (
@@ -322,7 +325,8 @@ def run_ours(args):
         "events_per_photon": total_events / total_photons,
         "trace_kernel": {"ms": ms_avg, "paths_per_s": n / (ms_avg * 1e-3), "events_per_s": trace_events_per_s},
         "config": {"workload": cfg.name, "grid": [cfg.nx, cfg.ny, cfg.nz], "photons_per_gpu_per_step": n,
-                   "block": list(cfg.block), "zenith_deg": cfg.zenith_deg, "azimuth_deg": cfg.azimuth_deg,
+                   "block": list(cfg.block), "merge": list(cfg.merge), "merge_ratio": cfg.merge_ratio,
+                   "zenith_deg": cfg.zenith_deg, "azimuth_deg": cfg.azimuth_deg,
                    "parallelism": "photon-id ranges per GPU, no collective" if world > 1 else "1 GPU",
                    "l2": ("inputs exceed L2 (%d MiB packed optics + %d MiB tallies vs 126 MB)" % (
                        cfg.nvox * 16 >> 20, cfg.nvox * 8 >> 20)) if cfg.nvox * 24 > (126 << 20) else
@@ -366,6 +370,7 @@ def main():
     ap.add_argument("--workload", type=int, choices=(1, 2, 3, 4, 5), default=WORKLOAD,
                     help="BASELINE.json configs[N-1]; the default (3) is the configuration the metric is quoted on")
     ap.add_argument("--block", default=None, help="acceleration-grid block bx,by,bz (default: the config's)")
+    ap.add_argument("--merge", default=None, help="merged-cell factors mx,my,mz (default: the config's; 1,1,1 = off)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing (used under ncu)")
     args = ap.parse_args()
     if args.steps < 1 or args.warmup < 0:

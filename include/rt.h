@@ -48,7 +48,7 @@ typedef struct rt_ctx rt_ctx; /* opaque; owned by the library; one CUDA device p
  * the "collision events" of BASELINE.json's metric. */
 typedef struct {
   uint64_t n_photons, n_events, n_null, n_rayleigh, n_hg, n_atm_abs, n_sfc_hits, n_sfc_abs, n_toa,
-      n_capped, n_cell_steps;
+      n_capped, n_cell_steps, n_relevel;
   int64_t capped_energy; /* quanta of photons stopped by the event cap; 0 on all shipped configs */
 } rt_counters;
 
@@ -94,10 +94,22 @@ int rt_trace_records(rt_ctx* ctx, double zenith_deg, double azimuth_deg, uint64_
 int rt_read_tallies(rt_ctx* ctx, int64_t* atm_abs, int64_t* sfc_dir, int64_t* sfc_dif, int64_t* sfc_abs,
                     int64_t* toa_up, rt_counters* counters);
 
+/* Merged acceleration cells (P:54 leaves the acceleration grid's resolution open).
+ * Blocks of mx*my*mz acceleration cells in which the extinction is nearly uniform (max k_ext <=
+ * merge_ratio * min k_ext over the block's voxels) are traversed as ONE cell with the block's maximum as
+ * majorant: clear air above, below and between the clouds costs one step per block instead of one per
+ * cell.  Any majorant >= k_ext gives the same expectations, so only the sample paths change.
+ * mx, my, mz: powers of two dividing the acceleration grid's extents; 1,1,1 (the default after
+ * rt_create_grid) = single-level grid.  merge_ratio >= 1.  Takes effect at the next rt_set_optics;
+ * a context that already holds optics must be given them again before the next rt_trace
+ * (RT_ESTATE otherwise).  Errors: RT_EINVAL. */
+int rt_set_merge(rt_ctx* ctx, int mx, int my, int mz, float merge_ratio);
+
 /* Zero tallies and counters on `cuda_stream`. */
 int rt_reset_tallies(rt_ctx* ctx, void* cuda_stream);
 
-/* Copy the majorant grid ([cz][cy][cx] fp32, DEVICE or HOST pointer) out; for tests. */
+/* Copy the majorant grid ([cz][cy][cx] fp32, DEVICE or HOST pointer) out; for tests.  Cells of a merged
+ * block hold -(block maximum) (sign bit set), the others their own maximum. */
 int rt_read_majorant(rt_ctx* ctx, float* khat_out);
 
 /* Copy the packed per-voxel coefficients (c1,c2,c3,g; 4 fp32 per voxel, [z][y][x]) out; for tests. */

@@ -13,7 +13,7 @@ W0 = 1 << 32  # tally quanta per photon
 FATE_ATM_ABS, FATE_SFC_ABS, FATE_TOD_EXIT, FATE_CAPPED = 1, 2, 3, 4
 
 COUNTER_FIELDS = ("n_photons", "n_events", "n_null", "n_rayleigh", "n_hg", "n_atm_abs",
-                  "n_sfc_hits", "n_sfc_abs", "n_toa", "n_capped", "n_cell_steps", "capped_energy")
+                  "n_sfc_hits", "n_sfc_abs", "n_toa", "n_capped", "n_cell_steps", "n_relevel", "capped_energy")
 
 
 class Counters(C.Structure):
@@ -34,7 +34,8 @@ def lib():
         ip = C.POINTER(C.c_int64)
         _lib.orc_trace.restype = C.c_int
         _lib.orc_trace.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float,
-                                   C.c_int, C.c_int, C.c_int, fp, fp, fp, fp, fp, C.c_double, C.c_double,
+                                   C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_float,
+                                   fp, fp, fp, fp, fp, C.c_double, C.c_double,
                                    C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint32, ip, ip, ip, ip, ip,
                                    C.POINTER(Counters), C.POINTER(C.c_uint32), C.c_int,
                                    C.POINTER(C.c_double)]
@@ -65,9 +66,10 @@ class Tallies:
 
 
 def trace(grid, optics, zenith_deg, azimuth_deg, n_photons, first_photon_id=0, seed=1, stream_id=0,
-          precision=64, tallies=None, records=False, n_threads=1):
+          precision=64, tallies=None, records=False, n_threads=1, merge=(1, 1, 1), merge_ratio=1.25):
     """Run the oracle.  grid = (nx, ny, nz, dx, dy, dz, bx, by, bz); optics = dict with
-    k_ext, k_ext_cloud, ssa, g ([nz][ny][nx] fp32) and sfc_albedo ([ny][nx] fp32).
+    k_ext, k_ext_cloud, ssa, g ([nz][ny][nx] fp32) and sfc_albedo ([ny][nx] fp32); merge = merged-cell
+    factors ((1, 1, 1) = single-level acceleration grid).
     Returns (tallies, records or None, elapsed seconds of the photon loop)."""
     nx, ny, nz, dx, dy, dz, bx, by, bz = grid
     k, kp = _f32(optics["k_ext"])
@@ -80,7 +82,8 @@ def trace(grid, optics, zenith_deg, azimuth_deg, n_photons, first_photon_id=0, s
     rec = np.zeros((n_photons, 4), dtype=np.uint32) if records else None
     ip = C.POINTER(C.c_int64)
     el = C.c_double(0.0)
-    rc = lib().orc_trace(int(precision), nx, ny, nz, dx, dy, dz, bx, by, bz, kp, kcp, wp, gp, alp,
+    rc = lib().orc_trace(int(precision), nx, ny, nz, dx, dy, dz, bx, by, bz, int(merge[0]), int(merge[1]),
+                         int(merge[2]), float(merge_ratio), kp, kcp, wp, gp, alp,
                          float(zenith_deg), float(azimuth_deg), int(n_photons), int(first_photon_id),
                          int(seed), int(stream_id), t.atm_abs.ctypes.data_as(ip),
                          t.sfc_dir.ctypes.data_as(ip), t.sfc_dif.ctypes.data_as(ip),
@@ -154,10 +157,12 @@ def pack_optics_f32(k, kc, w, g):
     return out
 
 
-def majorant(nx, ny, nz, bx, by, bz, k_ext):
+def majorant(nx, ny, nz, bx, by, bz, k_ext, merge=(1, 1, 1), merge_ratio=1.25):
+    """Majorant table [ncz][ncy][ncx]; cells of merged blocks hold -(block maximum)."""
     k, kp = _f32(k_ext)
     out = np.empty(((nz // bz), (ny // by), (nx // bx)), dtype=np.float32)
-    lib().orc_majorant(nx, ny, nz, bx, by, bz, kp, out.ctypes.data_as(C.POINTER(C.c_float)))
+    lib().orc_majorant(nx, ny, nz, bx, by, bz, int(merge[0]), int(merge[1]), int(merge[2]),
+                       C.c_float(merge_ratio), kp, out.ctypes.data_as(C.POINTER(C.c_float)))
     return out
 
 

@@ -206,7 +206,7 @@ extern "C" {
 
 struct orc_counters {
   uint64_t n_photons, n_events, n_null, n_rayleigh, n_hg, n_atm_abs, n_sfc_hits, n_sfc_abs,
-      n_toa, n_capped, n_cell_steps;
+      n_toa, n_capped, n_cell_steps, n_relevel;
   int64_t capped_energy;
 };
 
@@ -221,6 +221,8 @@ constexpr uint32_t EVENT_CAP = 1u << 20;       // §3.12
 
 struct Problem {
   int nx, ny, nz, bx, by, bz;
+  int mx, my, mz;            // §3.5b: merged cells of mx x my x mz acceleration cells (1,1,1 = none)
+  float merge_ratio;         // §3.5b: merged iff max c3 <= merge_ratio * min c3 over the merged cell's voxels
   float dx, dy, dz;
   const float *k_ext, *k_cloud, *ssa, *g, *albedo;
   double zenith_deg, azimuth_deg;
@@ -258,7 +260,11 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
   const uint64_t n_full = (P.n_photons / ncol) * ncol;
   const R dx = (R)P.dx, dy = (R)P.dy, dz = (R)P.dz;
   const R rdx = (R)1 / dx, rdy = (R)1 / dy, rdz = (R)1 / dz;
-  const R Lx = (R)bx * dx, Ly = (R)by * dy, Lz = (R)bz * dz;
+  // §3.5b/§3.7: cell extents at level 0 (one acceleration cell) and level 1 (a merged cell)
+  const int mxyz[3] = {P.mx, P.my, P.mz};
+  const R Lv[2][3] = {{(R)bx * dx, (R)by * dy, (R)bz * dz},
+                      {(R)(P.mx * bx) * dx, (R)(P.my * by) * dy, (R)(P.mz * bz) * dz}};
+  const int ncs[3] = {ncx, ncy, ncz};
   const R TINY = (R)1e-30f;
 
   // §3.3 sun direction: computed in double, then converted to Real.
@@ -284,32 +290,46 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
       ix = std::min((int)(u2 * (R)nx), nx - 1);
       iy = std::min((int)(u3 * (R)ny), ny - 1);
     }
-    int cx = ix / bx, cy = iy / by, cz = ncz - 1;
-    // Position inside the current acceleration cell is carried as the REMAINING DISTANCES rx, ry, rz
-    // along the flight direction to the cell's next face on each axis: a cell
-    // crossing subtracts the smallest one from the other two and resets its own to the face spacing
-    // del = L |1/v| exactly, so magnitudes never grow and rounding does not accumulate along a path.
-    // Local coordinates are recovered when needed as q = face - v r.
-    R da = sun_x, db = sun_y, dc = sun_z;      // unit direction
-    R va, vb, vc, ia, ib, ic;                  // nudged components and reciprocals
-    R delx, dely, delz;                        // distance between successive faces on each axis
-    R rx, ry, rz;                              // remaining distance to the next face on each axis
+    int c[3] = {ix / bx, iy / by, ncz - 1};    // acceleration-cell index (at level 1: the merged cell's origin)
+    // §3.5b: the sign bit of the stored majorant says whether the cell belongs to a merged cell
+    auto load = [&](R& kh_out) {
+      float s = khat[((size_t)c[2] * ncy + c[1]) * ncx + c[0]];
+      kh_out = (R)std::fabs(s);
+      return std::signbit(s) ? 1 : 0;
+    };
+    R kh;
+    int lev = load(kh);
+    if (lev) { c[0] -= c[0] % P.mx; c[1] -= c[1] % P.my; c[2] -= c[2] % P.mz; }
+    // Position inside the current cell is carried as the REMAINING DISTANCES r[0..2] along the flight
+    // direction to the cell's next face on each axis: a cell crossing subtracts the
+    // smallest one from the other two and resets its own to the face spacing del = L |1/v| exactly, so
+    // magnitudes never grow and rounding does not accumulate along a path.  Local coordinates are
+    // recovered when needed as q = face - v r.
+    R d[3] = {sun_x, sun_y, sun_z};            // unit direction
+    R v[3], iv[3];                             // nudged components and reciprocals
+    R del[2][3];                               // distance between successive faces, per level and axis
+    R r[3];                                    // remaining distance to the next face on each axis
     auto set_dir = [&]() {
-      va = (std::fabs(da) < TINY) ? TINY : da;
-      vb = (std::fabs(db) < TINY) ? TINY : db;
-      vc = (std::fabs(dc) < TINY) ? TINY : dc;
-      ia = (R)1 / va; ib = (R)1 / vb; ic = (R)1 / vc;
-      delx = Lx * std::fabs(ia); dely = Ly * std::fabs(ib); delz = Lz * std::fabs(ic);
+      for (int a = 0; a < 3; ++a) {
+        v[a] = (std::fabs(d[a]) < TINY) ? TINY : d[a];
+        iv[a] = (R)1 / v[a];
+        del[0][a] = Lv[0][a] * std::fabs(iv[a]);
+        del[1][a] = Lv[1][a] * std::fabs(iv[a]);
+      }
     };
-    auto face = [&](R v, R L) { return (v > 0) ? L : (R)0; };
-    auto place = [&](R qx, R qy, R qz) {        // remaining distances from local coordinates
-      rx = (face(va, Lx) - qx) * ia; ry = (face(vb, Ly) - qy) * ib; rz = (face(vc, Lz) - qz) * ic;
+    auto face = [&](int a) { return (v[a] > 0) ? Lv[lev][a] : (R)0; };
+    auto place = [&](const R q[3]) {           // remaining distances from local coordinates
+      for (int a = 0; a < 3; ++a) r[a] = (face(a) - q[a]) * iv[a];
     };
-    auto local = [&](R v, R r, R L) {           // local coordinate from a remaining distance
-      return std::min(L, std::max((R)0, E::fma(-v, r, face(v, L))));
+    auto local = [&](int a) {                  // local coordinate from a remaining distance
+      return std::min(Lv[lev][a], std::max((R)0, E::fma(-v[a], r[a], face(a))));
     };
     set_dir();
-    place(((R)(ix % bx) + u0) * dx, ((R)(iy % by) + u1) * dy, Lz);
+    {
+      const R q[3] = {((R)(ix % ((lev ? P.mx : 1) * bx)) + u0) * dx,
+                      ((R)(iy % ((lev ? P.my : 1) * by)) + u1) * dy, Lv[lev][2]};
+      place(q);
+    }
     bool direct = true;
     uint32_t e = 1, n_ev = 0, n_sc = 0, n_sfc = 0;
     int fate = 0; uint32_t term = 0;
@@ -322,42 +342,43 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
       tau = E::neg_log_1m(u0);
     };
     draw();
-    size_t cell = ((size_t)cz * ncy + cy) * ncx + cx;
-    R kh = (R)khat[cell];
     R rk = (kh > 0) ? (R)1 / kh : (R)0;
+    const int bs[3] = {bx, by, bz};
+    const R rds[3] = {rdx, rdy, rdz};
 
     while (fate == 0) {
       // ---- step 5: nearest face of the current cell; ties x < y < z -----------
       int axis; R t;
-      if (rx <= ry && rx <= rz) { axis = 0; t = rx; }
-      else if (ry <= rz)        { axis = 1; t = ry; }
-      else                      { axis = 2; t = rz; }
+      if (r[0] <= r[1] && r[0] <= r[2]) { axis = 0; t = r[0]; }
+      else if (r[1] <= r[2])            { axis = 1; t = r[1]; }
+      else                              { axis = 2; t = r[2]; }
       R dtau = kh * t;
       if (kh > 0 && tau <= dtau) {
         // ---- step 7: tentative collision inside this cell -------------------
         R s = tau * rk;
-        rx = std::max((R)0, rx - s); ry = std::max((R)0, ry - s); rz = std::max((R)0, rz - s);
-        R qx = local(va, rx, Lx), qy = local(vb, ry, Ly), qz = local(vc, rz, Lz);
-        int lx = std::min((int)(qx * rdx), bx - 1);
-        int ly = std::min((int)(qy * rdy), by - 1);
-        int lz = std::min((int)(qz * rdz), bz - 1);
-        size_t vox = ((size_t)(cz * bz + lz) * ny + (cy * by + ly)) * nx + (cx * bx + lx);
-        Vox<R> v = pack_voxel<R>(P.k_ext[vox], P.k_cloud[vox], P.ssa[vox], P.g[vox]);
+        for (int a = 0; a < 3; ++a) r[a] = std::max((R)0, r[a] - s);
+        R q[3]; int gv[3];
+        for (int a = 0; a < 3; ++a) {
+          q[a] = local(a);
+          gv[a] = c[a] * bs[a] + std::min((int)(q[a] * rds[a]), (lev ? mxyz[a] : 1) * bs[a] - 1);
+        }
+        size_t vox = ((size_t)gv[2] * ny + gv[1]) * nx + gv[0];
+        Vox<R> vx = pack_voxel<R>(P.k_ext[vox], P.k_cloud[vox], P.ssa[vox], P.g[vox]);
         ++n_ev; ++C.n_events;                  // step 6
         // ---- step 8: classify ----------------------------------------------
         R xi = u1 * kh;
-        if (xi < v.c1) {
+        if (xi < vx.c1) {
           add64(&P.atm_abs[vox], W0); ++C.n_atm_abs;
           fate = ORC_ATM_ABS; term = (uint32_t)vox; break;
-        } else if (xi < v.c2) {                // cloud droplet: Henyey-Greenstein
-          R mu = sample_hg<R>(v.g, u2);
+        } else if (xi < vx.c2) {               // cloud droplet: Henyey-Greenstein
+          R mu = sample_hg<R>(vx.g, u2);
           R sp, cp; E::sincos_2pi(u3, sp, cp);
-          rotate_dir<R>(da, db, dc, mu, cp, sp); set_dir(); place(qx, qy, qz);
+          rotate_dir<R>(d[0], d[1], d[2], mu, cp, sp); set_dir(); place(q);
           direct = false; ++n_sc; ++C.n_hg;
-        } else if (xi < v.c3) {                // gas: Rayleigh
+        } else if (xi < vx.c3) {               // gas: Rayleigh
           R mu = sample_rayleigh<R>(u2);
           R sp, cp; E::sincos_2pi(u3, sp, cp);
-          rotate_dir<R>(da, db, dc, mu, cp, sp); set_dir(); place(qx, qy, qz);
+          rotate_dir<R>(d[0], d[1], d[2], mu, cp, sp); set_dir(); place(q);
           direct = false; ++n_sc; ++C.n_rayleigh;
         } else {
           ++C.n_null;                          // null collision: direction unchanged
@@ -371,24 +392,20 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
         // ---- step 5 (cont.): leave the cell through `axis` -------------------
         tau = tau - dtau;
         ++C.n_cell_steps;
+        const int step = lev ? mxyz[axis] : 1;
+        for (int a = 0; a < 3; ++a) r[a] = (a == axis) ? del[lev][a] : r[a] - t;
         bool at_sfc = false, at_top = false;
-        if (axis == 0) {
-          ry = ry - t; rz = rz - t; rx = delx;
-          if (va > 0) { ++cx; if (cx == ncx) cx = 0; }
-          else        { --cx; if (cx < 0) cx = ncx - 1; }
-        } else if (axis == 1) {
-          rx = rx - t; rz = rz - t; ry = dely;
-          if (vb > 0) { ++cy; if (cy == ncy) cy = 0; }
-          else        { --cy; if (cy < 0) cy = ncy - 1; }
+        if (v[axis] > 0) {
+          c[axis] += step;
+          if (c[axis] >= ncs[axis]) { if (axis == 2) at_top = true; else c[axis] -= ncs[axis]; }
         } else {
-          rx = rx - t; ry = ry - t; rz = delz;
-          if (vc > 0) { ++cz; if (cz == ncz) at_top = true; }
-          else        { --cz; if (cz < 0) at_sfc = true; }
+          c[axis] -= step;
+          if (c[axis] < 0) { if (axis == 2) at_sfc = true; else c[axis] += ncs[axis]; }
         }
         if (at_sfc || at_top) {
-          R qx = local(va, rx, Lx), qy = local(vb, ry, Ly);
-          int hx = cx * bx + std::min((int)(qx * rdx), bx - 1);
-          int hy = cy * by + std::min((int)(qy * rdy), by - 1);
+          R qx = local(0), qy = local(1);
+          int hx = c[0] * bx + std::min((int)(qx * rdx), (lev ? P.mx : 1) * bx - 1);
+          int hy = c[1] * by + std::min((int)(qy * rdy), (lev ? P.my : 1) * by - 1);
           size_t col = (size_t)hy * nx + hx;
           if (at_top) {                        // step 11
             add64(&P.toa_up[col], W0); ++C.n_toa;
@@ -400,8 +417,10 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
           if (u1 < (R)P.albedo[col]) {
             R mu = std::sqrt((R)1 - u2), s = std::sqrt(u2);
             R sp, cp; E::sincos_2pi(u3, sp, cp);
-            da = s * cp; db = s * sp; dc = mu; set_dir();
-            direct = false; cz = 0; place(qx, qy, (R)0);
+            d[0] = s * cp; d[1] = s * sp; d[2] = mu; set_dir();
+            direct = false; c[2] = 0;          // back in the cell it left (level unchanged)
+            const R q[3] = {qx, qy, (R)0};
+            place(q);
             ++e;
             if (e > EVENT_CAP) {
               ++C.n_capped; C.capped_energy += W0; fate = ORC_CAPPED; term = 0; break;
@@ -411,9 +430,42 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
             add64(&P.sfc_abs[col], W0); ++C.n_sfc_abs;
             fate = ORC_SFC_ABS; term = (uint32_t)col; break;
           }
+        } else {
+          // ---- §3.7b: the entered cell's level; change of level at a merged cell's face ------
+          const int lev_new = load(kh);
+          if (lev_new != lev) {
+            ++C.n_relevel;
+            if (lev_new == 1) {
+              // into a merged cell: distances to ITS faces; the index becomes its origin
+              for (int a = 0; a < 3; ++a) {
+                const int m = mxyz[a], o = c[a] % m;
+                if (a != axis) {
+                  const int n = (v[a] > 0) ? (m - 1 - o) : o;   // whole cells between here and that face
+                  r[a] = E::fma((R)n, del[0][a], r[a]);
+                } else {
+                  r[a] = del[1][a];
+                }
+                c[a] -= o;
+              }
+            } else {
+              // out of a merged cell into single cells: which cell of the entered block, and the
+              // distance to that cell's faces
+              for (int a = 0; a < 3; ++a) {
+                const int m = mxyz[a];
+                if (a != axis) {
+                  const int k = std::min(m - 1, (int)(r[a] / del[0][a]));
+                  r[a] = std::max((R)0, E::fma(-(R)k, del[0][a], r[a]));
+                  c[a] += (v[a] > 0) ? (m - 1 - k) : k;
+                } else {
+                  r[a] = del[0][a];
+                  if (!(v[a] > 0)) c[a] += m - 1;               // entered through the block's far side
+                }
+              }
+              load(kh);                                          // the single cell's own majorant
+            }
+            lev = lev_new;
+          }
         }
-        cell = ((size_t)cz * ncy + cy) * ncx + cx;
-        kh = (R)khat[cell];
         rk = (kh > 0) ? (R)1 / kh : (R)0;
       }
     }
@@ -426,7 +478,10 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
   }
 }
 
-// §3.2 majorant: highest extinction coefficient within each acceleration cell.
+// §3.5 majorant: highest extinction coefficient within each acceleration cell.
+// §3.5b merged cells: blocks of mx x my x mz acceleration cells whose voxels all have nearly the same
+// extinction (max <= merge_ratio * min, one fp32 multiply) are traversed as ONE cell with the block's
+// maximum; every cell of such a block stores -(block maximum) (sign bit set, also for 0).
 std::vector<float> build_majorant(const Problem& P) {
   const int ncx = P.nx / P.bx, ncy = P.ny / P.by, ncz = P.nz / P.bz;
   std::vector<float> kh((size_t)ncx * ncy * ncz, 0.0f);
@@ -436,6 +491,24 @@ std::vector<float> build_majorant(const Problem& P) {
         float k = P.k_ext[((size_t)z * P.ny + y) * P.nx + x];
         float& m = kh[((size_t)(z / P.bz) * ncy + (y / P.by)) * ncx + (x / P.bx)];
         if (k > m) m = k;
+      }
+  if (P.mx * P.my * P.mz == 1) return kh;
+  const int sx = P.mx * P.bx, sy = P.my * P.by, sz = P.mz * P.bz;   // merged-cell extent in voxels
+  for (int Z = 0; Z < P.nz / sz; ++Z)
+    for (int Y = 0; Y < P.ny / sy; ++Y)
+      for (int X = 0; X < P.nx / sx; ++X) {
+        float kmax = 0.0f, kmin = INFINITY;
+        for (int z = Z * sz; z < (Z + 1) * sz; ++z)
+          for (int y = Y * sy; y < (Y + 1) * sy; ++y)
+            for (int x = X * sx; x < (X + 1) * sx; ++x) {
+              float k = P.k_ext[((size_t)z * P.ny + y) * P.nx + x];
+              kmax = std::max(kmax, k); kmin = std::min(kmin, k);
+            }
+        if (!(kmax <= P.merge_ratio * kmin)) continue;
+        for (int cz = Z * P.mz; cz < (Z + 1) * P.mz; ++cz)
+          for (int cy = Y * P.my; cy < (Y + 1) * P.my; ++cy)
+            for (int cx = X * P.mx; cx < (X + 1) * P.mx; ++cx)
+              kh[((size_t)cz * ncy + cy) * ncx + cx] = -kmax;
       }
   return kh;
 }
@@ -447,16 +520,17 @@ extern "C" {
 // Returns 0 on success, -1 on bad arguments.  Tallies and counters are ADDED to.
 // elapsed_s (may be NULL) receives the wall time of the photon loop only.
 int orc_trace(int precision, int nx, int ny, int nz, float dx, float dy, float dz, int bx, int by,
-              int bz, const float* k_ext, const float* k_ext_cloud, const float* ssa, const float* g,
+              int bz, int mx, int my, int mz, float merge_ratio, const float* k_ext, const float* k_ext_cloud, const float* ssa, const float* g,
               const float* sfc_albedo, double zenith_deg, double azimuth_deg, uint64_t n_photons,
               uint64_t first_photon_id, uint64_t seed, uint32_t stream_id, int64_t* atm_abs,
               int64_t* sfc_dir, int64_t* sfc_dif, int64_t* sfc_abs, int64_t* toa_up,
               orc_counters* counters, uint32_t* records, int n_threads, double* elapsed_s) {
   if (nx <= 0 || ny <= 0 || nz <= 0 || bx <= 0 || by <= 0 || bz <= 0) return -1;
   if (nx % bx || ny % by || nz % bz) return -1;
+  if (mx <= 0 || my <= 0 || mz <= 0 || (nx / bx) % mx || (ny / by) % my || (nz / bz) % mz) return -1;
   if (!(zenith_deg >= 0.0 && zenith_deg < 90.0)) return -1;
   if (precision != 32 && precision != 64) return -1;
-  Problem P{nx, ny, nz, bx, by, bz, dx, dy, dz, k_ext, k_ext_cloud, ssa, g, sfc_albedo,
+  Problem P{nx, ny, nz, bx, by, bz, mx, my, mz, merge_ratio, dx, dy, dz, k_ext, k_ext_cloud, ssa, g, sfc_albedo,
             zenith_deg, azimuth_deg, n_photons, first_photon_id, seed, stream_id,
             atm_abs, sfc_dir, sfc_dif, sfc_abs, toa_up, records};
   std::vector<float> khat = build_majorant(P);
@@ -526,8 +600,10 @@ void orc_pack_optics_f32(const float* k, const float* kc, const float* w, const 
     c[4 * i] = v.c1; c[4 * i + 1] = v.c2; c[4 * i + 2] = v.c3; c[4 * i + 3] = v.g;
   }
 }
-void orc_majorant(int nx, int ny, int nz, int bx, int by, int bz, const float* k_ext, float* out) {
+void orc_majorant(int nx, int ny, int nz, int bx, int by, int bz, int mx, int my, int mz,
+                  float merge_ratio, const float* k_ext, float* out) {
   Problem P{}; P.nx = nx; P.ny = ny; P.nz = nz; P.bx = bx; P.by = by; P.bz = bz; P.k_ext = k_ext;
+  P.mx = mx; P.my = my; P.mz = mz; P.merge_ratio = merge_ratio;
   std::vector<float> kh = build_majorant(P);
   std::memcpy(out, kh.data(), kh.size() * sizeof(float));
 }

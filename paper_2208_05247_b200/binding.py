@@ -11,12 +11,12 @@ LIB_PATH = os.path.join(HERE, "librt_b200.so")
 W0 = 1 << 32
 FATE_ATM_ABS, FATE_SFC_ABS, FATE_TOD_EXIT, FATE_CAPPED = 1, 2, 3, 4
 
-EXPORTS = ("rt_create_grid", "rt_set_optics", "rt_trace", "rt_trace_records", "rt_read_tallies",
+EXPORTS = ("rt_create_grid", "rt_set_merge", "rt_set_optics", "rt_trace", "rt_trace_records", "rt_read_tallies",
            "rt_reset_tallies", "rt_read_majorant", "rt_read_packed_optics", "rt_gather_bench",
            "rt_last_trace_ms", "rt_launch_count", "rt_philox_words", "rt_last_error", "rt_destroy")
 
 COUNTER_FIELDS = ("n_photons", "n_events", "n_null", "n_rayleigh", "n_hg", "n_atm_abs", "n_sfc_hits",
-                  "n_sfc_abs", "n_toa", "n_capped", "n_cell_steps", "capped_energy")
+                  "n_sfc_abs", "n_toa", "n_capped", "n_cell_steps", "n_relevel", "capped_energy")
 
 
 class RtError(RuntimeError):
@@ -44,6 +44,7 @@ def lib():
     L = C.CDLL(LIB_PATH)
     vp, i32, u32, u64, f32, f64 = C.c_void_p, C.c_int, C.c_uint32, C.c_uint64, C.c_float, C.c_double
     L.rt_create_grid.argtypes = [C.POINTER(vp), i32, i32, i32, f32, f32, f32, i32, i32, i32, i32]
+    L.rt_set_merge.argtypes = [vp, i32, i32, i32, f32]
     L.rt_set_optics.argtypes = [vp, vp, vp, vp, vp, vp, vp]
     L.rt_trace.argtypes = [vp, f64, f64, u64, u64, u64, u32, vp]
     L.rt_trace_records.argtypes = [vp, f64, f64, u64, u64, u64, u32, vp, vp]
@@ -90,7 +91,7 @@ class Tallies:
 class Grid:
     """One rt_ctx: rt_create_grid / rt_set_optics / rt_trace / rt_read_tallies (include/rt.h)."""
 
-    def __init__(self, nx, ny, nz, dx, dy, dz, bx=8, by=8, bz=8, device=0):
+    def __init__(self, nx, ny, nz, dx, dy, dz, bx=8, by=8, bz=8, device=0, merge=(1, 1, 1), merge_ratio=1.25):
         if not torch.cuda.is_available():
             raise RtError("no CUDA device: this library has no CPU path")
         self.L = lib()
@@ -105,6 +106,12 @@ class Grid:
                 self.L.rt_destroy(self.ctx)
                 self.ctx = C.c_void_p(None)
             raise RtError("rt_create_grid failed (%d): %s" % (rc, msg))
+        if tuple(merge) != (1, 1, 1):
+            self.set_merge(*merge, merge_ratio=merge_ratio)
+
+    def set_merge(self, mx, my, mz, merge_ratio=1.25):
+        """Merged acceleration cells (include/rt.h rt_set_merge); call before set_optics."""
+        self._check(self.L.rt_set_merge(self.ctx, int(mx), int(my), int(mz), float(merge_ratio)), "rt_set_merge")
 
     def _check(self, rc, name):
         if rc != 0:

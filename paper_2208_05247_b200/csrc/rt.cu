@@ -14,6 +14,9 @@ struct rt_ctx {
   int device = 0;
   int nx = 0, ny = 0, nz = 0, bx = 0, by = 0, bz = 0, ncx = 0, ncy = 0, ncz = 0;
   float dx = 0, dy = 0, dz = 0;
+  int mx = 1, my = 1, mz = 1;             // merged-cell factors (rt_set_merge)
+  float merge_ratio = 1.25f;
+  float* kmin = nullptr;                  // per-cell minimum extinction; allocated when merging is on
   size_t nvox = 0, ncol = 0, ncell = 0;
   float4* optics = nullptr;
   float* khat = nullptr;
@@ -87,6 +90,9 @@ int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photon
   A.dx = c->dx; A.dy = c->dy; A.dz = c->dz;
   A.rdx = 1.0f / c->dx; A.rdy = 1.0f / c->dy; A.rdz = 1.0f / c->dz;
   A.Lx = (float)c->bx * c->dx; A.Ly = (float)c->by * c->dy; A.Lz = (float)c->bz * c->dz;
+  A.mx = c->mx; A.my = c->my; A.mz = c->mz;
+  A.rmx = 1.0f / (float)c->mx; A.rmy = 1.0f / (float)c->my; A.rmz = 1.0f / (float)c->mz;
+  A.Lx1 = (float)(c->mx * c->bx) * c->dx; A.Ly1 = (float)(c->my * c->by) * c->dy; A.Lz1 = (float)(c->mz * c->bz) * c->dz;
   // sun direction evaluated in double on the host, rounded once to fp32
   const double deg = 3.14159265358979323846 / 180.0;
   const double th = zenith_deg * deg, ph = azimuth_deg * deg;
@@ -188,10 +194,22 @@ int rt_set_optics(rt_ctx* c, const float* k_ext, const float* k_ext_cloud, const
   RT_CUDA(c, cudaMemsetAsync(c->khat, 0, c->ncell * sizeof(float), st));
   RT_CUDA(c, cudaMemcpyAsync(c->albedo, sfc_albedo, c->ncol * sizeof(float), cudaMemcpyDeviceToDevice, st));
   const int blocks = c->sm_count * 8;
-  rt::pack_optics_kernel<<<blocks, 256, 0, st>>>(k_ext, k_ext_cloud, ssa, g, c->optics, (int*)c->khat, c->nx,
+  const bool merging = c->mx * c->my * c->mz > 1;
+  if (merging) {
+    if (!c->kmin) RT_CUDA(c, cudaMalloc(&c->kmin, c->ncell * sizeof(float)));
+    RT_CUDA(c, cudaMemsetAsync(c->kmin, 0x7f, c->ncell * sizeof(float), st));   // 0x7f7f7f7f: above any finite input's bits that matter (3.4e38)
+  }
+  rt::pack_optics_kernel<<<blocks, 256, 0, st>>>(k_ext, k_ext_cloud, ssa, g, c->optics, (int*)c->khat,
+                                                merging ? (int*)c->kmin : nullptr, c->nx,
                                                 c->ny, c->nz, c->bx, c->by, c->bz, c->bad);
   rt::check_albedo_kernel<<<c->sm_count, 256, 0, st>>>(c->albedo, c->ncol, c->bad);
   c->launches += 2;
+  if (merging) {
+    const size_t nblk = c->ncell / ((size_t)c->mx * c->my * c->mz);
+    rt::merge_cells_kernel<<<(unsigned)((nblk + 127) / 128), 128, 0, st>>>(c->khat, c->kmin, c->ncx, c->ncy, c->ncz,
+                                                                            c->mx, c->my, c->mz, c->merge_ratio);
+    ++c->launches;
+  }
   RT_CUDA(c, cudaGetLastError());
   int bad = 0;
   RT_CUDA(c, cudaMemcpyAsync(&bad, c->bad, sizeof(int), cudaMemcpyDeviceToHost, st));
@@ -232,10 +250,21 @@ int rt_read_tallies(rt_ctx* c, int64_t* atm_abs, int64_t* sfc_dir, int64_t* sfc_
     counters->n_null = h[rt::C_NULL]; counters->n_rayleigh = h[rt::C_RAY]; counters->n_hg = h[rt::C_HG];
     counters->n_atm_abs = h[rt::C_ATM_ABS]; counters->n_sfc_hits = h[rt::C_SFC_HITS];
     counters->n_sfc_abs = h[rt::C_SFC_ABS]; counters->n_toa = h[rt::C_TOA]; counters->n_capped = h[rt::C_CAPPED];
-    counters->n_cell_steps = h[rt::C_CELLS]; counters->capped_energy = (int64_t)h[rt::C_CAPPED_E];
+    counters->n_cell_steps = h[rt::C_CELLS]; counters->n_relevel = h[rt::C_RELEVEL]; counters->capped_energy = (int64_t)h[rt::C_CAPPED_E];
     counters->n_events = h[rt::C_NULL] + h[rt::C_RAY] + h[rt::C_HG] + h[rt::C_ATM_ABS];
     counters->n_photons = h[rt::C_ATM_ABS] + h[rt::C_SFC_ABS] + h[rt::C_TOA] + h[rt::C_CAPPED];
   }
+  return RT_OK;
+}
+
+int rt_set_merge(rt_ctx* c, int mx, int my, int mz, float merge_ratio) {
+  if (!c) return RT_EINVAL;
+  auto pow2 = [](int v) { return v > 0 && !(v & (v - 1)); };
+  if (!pow2(mx) || !pow2(my) || !pow2(mz) || c->ncx % mx || c->ncy % my || c->ncz % mz)
+    return fail(c, RT_EINVAL, "rt_set_merge: factors must be powers of two dividing the acceleration grid");
+  if (!(merge_ratio >= 1.0f) || !std::isfinite(merge_ratio)) return fail(c, RT_EINVAL, "rt_set_merge: merge_ratio must be >= 1");
+  c->mx = mx; c->my = my; c->mz = mz; c->merge_ratio = merge_ratio;
+  c->have_optics = false;                 // the majorant table is rebuilt by the next rt_set_optics
   return RT_OK;
 }
 
@@ -316,7 +345,7 @@ void rt_destroy(rt_ctx* c) {
   {
     DeviceGuard guard(c->device);
     cudaDeviceSynchronize();
-    cudaFree(c->optics); cudaFree(c->khat); cudaFree(c->albedo); cudaFree(c->tallies);
+    cudaFree(c->optics); cudaFree(c->khat); cudaFree(c->kmin); cudaFree(c->albedo); cudaFree(c->tallies);
     cudaFree(c->counters); cudaFree(c->bad); cudaFree(c->sink); cudaFree(c->stage);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);

@@ -11,7 +11,8 @@ namespace rt {
 // integer atomicMax (exact).  `bad` receives a bit mask of violated input ranges.
 __global__ void pack_optics_kernel(const float* __restrict__ k_ext, const float* __restrict__ k_cloud,
                                    const float* __restrict__ ssa, const float* __restrict__ g,
-                                   float4* __restrict__ optics, int* __restrict__ khat_bits, int nx, int ny,
+                                   float4* __restrict__ optics, int* __restrict__ khat_bits,
+                                   int* __restrict__ kmin_bits, int nx, int ny,
                                    int nz, int bx, int by, int bz, int* __restrict__ bad) {
   const size_t nvox = (size_t)nx * ny * nz;
   const size_t stride = (size_t)gridDim.x * blockDim.x;
@@ -37,22 +38,53 @@ __global__ void pack_optics_kernel(const float* __restrict__ k_ext, const float*
     const unsigned act = __activemask();
     const unsigned peers = __match_any_sync(act, cell);
     int m = flags ? 0 : __float_as_int(k);
+    int mn = m;                              // §3.5b: the cell minimum, for the merge criterion
     const int leader = __ffs(peers) - 1;
     for (int off = 16; off > 0; off >>= 1) {
       const int o = __shfl_down_sync(act, m, off);
+      const int on = __shfl_down_sync(act, mn, off);
       const unsigned src = (threadIdx.x & 31u) + off;
-      if (src < 32u && ((peers >> src) & 1u)) m = max(m, o);
+      if (src < 32u && ((peers >> src) & 1u)) { m = max(m, o); mn = min(mn, on); }
     }
     // shfl_down reduction is only complete when peers are contiguous; contiguous x runs are,
     // but guard the general case with a per-lane atomic when they are not.
     const unsigned run = peers >> leader;
     const bool contiguous = (run & (run + 1u)) == 0u;
     if (contiguous) {
-      if ((int)(threadIdx.x & 31u) == leader) atomicMax(&khat_bits[cell], m);
+      if ((int)(threadIdx.x & 31u) == leader) {
+        atomicMax(&khat_bits[cell], m);
+        if (kmin_bits) atomicMin(&kmin_bits[cell], mn);
+      }
     } else {
       atomicMax(&khat_bits[cell], flags ? 0 : __float_as_int(k));
+      if (kmin_bits) atomicMin(&kmin_bits[cell], flags ? 0 : __float_as_int(k));
     }
   }
+}
+
+// §3.5b merged cells.  One thread per block of mx x my x mz acceleration cells: if the block's highest
+// extinction is at most merge_ratio times its lowest (one fp32 multiply), every cell of the block stores
+// -(block maximum); the sign bit is what the trace kernel tests (set also for a maximum of 0).
+__global__ void merge_cells_kernel(float* __restrict__ khat, const float* __restrict__ kmin, int ncx, int ncy,
+                                   int ncz, int mx, int my, int mz, float merge_ratio) {
+  const int nbx = ncx / mx, nby = ncy / my, nbz = ncz / mz;
+  const size_t nblk = (size_t)nbx * nby * nbz;
+  const size_t b = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= nblk) return;
+  const int X = (int)(b % nbx), Y = (int)((b / nbx) % nby), Z = (int)(b / ((size_t)nbx * nby));
+  float hi = 0.0f, lo = INFINITY;
+  for (int z = Z * mz; z < (Z + 1) * mz; ++z)
+    for (int y = Y * my; y < (Y + 1) * my; ++y)
+      for (int x = X * mx; x < (X + 1) * mx; ++x) {
+        const size_t c = ((size_t)z * ncy + y) * ncx + x;
+        hi = fmaxf(hi, khat[c]);
+        lo = fminf(lo, kmin[c]);
+      }
+  if (!(hi <= merge_ratio * lo)) return;
+  const float v = -hi;
+  for (int z = Z * mz; z < (Z + 1) * mz; ++z)
+    for (int y = Y * my; y < (Y + 1) * my; ++y)
+      for (int x = X * mx; x < (X + 1) * mx; ++x) khat[((size_t)z * ncy + y) * ncx + x] = v;
 }
 
 __global__ void check_albedo_kernel(const float* __restrict__ albedo, size_t ncol, int* __restrict__ bad) {

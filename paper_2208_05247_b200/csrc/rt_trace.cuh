@@ -44,6 +44,9 @@ constexpr int kChunk = 128;                     // photon ids a warp takes per g
 #ifndef RT_MOVE_STEPS
 #define RT_MOVE_STEPS 3
 #endif
+#ifndef RT_MOVE_MIN
+#define RT_MOVE_MIN 0
+#endif
 #ifndef RT_BOUNDARY_BATCH
 #define RT_BOUNDARY_BATCH 4
 #endif
@@ -51,16 +54,20 @@ constexpr int kRegenBatch = RT_REGEN_BATCH;       // refill when this many lanes
 constexpr int kScatterBatch = RT_SCATTER_BATCH;   // run SCATTER when this many lanes wait for it (or nothing moves)
 constexpr int kCollideBatch = RT_COLLIDE_BATCH;   // ... COLLIDE
 constexpr int kBoundaryBatch = RT_BOUNDARY_BATCH; // ... BOUNDARY
-constexpr int kMoveSteps = RT_MOVE_STEPS;         // MOVE steps between two votes
+constexpr int kMoveSteps = RT_MOVE_STEPS;         // MOVE steps between two votes (at most)
+constexpr int kMoveMin = RT_MOVE_MIN;             // ... cut short when fewer lanes than this still move (0: never)
 
 enum Counter { C_NULL = 0, C_RAY, C_HG, C_ATM_ABS, C_SFC_HITS, C_SFC_ABS, C_TOA, C_CAPPED, C_CELLS,
-               C_CAPPED_E, C_COUNT };
+               C_CAPPED_E, C_RELEVEL, C_COUNT };
 
 enum : uint32_t { ST_DEAD = 0, ST_MOVE = 1, ST_COLLIDE = 2, ST_SCATTER = 3, ST_BOUNDARY = 4 };
 
 struct TraceArgs {
   int nx, ny, nz, bx, by, bz, ncx, ncy, ncz;
   float dx, dy, dz, rdx, rdy, rdz, Lx, Ly, Lz;
+  // §3.5b merged cells: factors (powers of two), their reciprocals, merged-cell extents (m b) d
+  int mx, my, mz;
+  float rmx, rmy, rmz, Lx1, Ly1, Lz1;
   float sun_x, sun_y, sun_z, sun_ix, sun_iy, sun_iz;  // beam direction and 1/nudge(component), host-computed
   const float4* __restrict__ optics;   // [z][y][x] (c1, c2, c3, g)
   const float* __restrict__ khat;      // [cz][cy][cx]
@@ -117,8 +124,12 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
   uint32_t sw2 = 0, sw3 = 0;              // ... of the event that chose SCATTER (its draw is already replaced)
   float sg = 0;                           // asymmetry parameter for the pending scatter; 2 = Rayleigh
   bool direct = true;
+  // §3.7b: kh holds the majorant table's word as stored, i.e. its sign bit says whether the photon travels
+  // through a merged cell (then cx, cy, cz = that cell's origin); the majorant itself is |kh|
+  uint32_t stp = 0;                       // index step per axis as three signed bytes (+-1, or +-m in a merged
+                                          // cell), top byte: axis of the crossing that asked for a change of level
   // event counts: running totals of this thread; a photon's own counts are differences (records)
-  uint32_t t_ev = 0, t_sc = 0, t_hg = 0, t_sfc = 0, t_cells = 0;
+  uint32_t t_ev = 0, t_sc = 0, t_hg = 0, t_sfc = 0, t_cells = 0, t_relevel = 0;
   uint32_t b_ev = 0, b_sc = 0, b_sfc = 0;  // totals when the current photon was launched (records only)
 
   auto draw = [&]() {
@@ -132,20 +143,30 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
     return fminf(L, fmaxf(0.0f, fmaf(-v, r, v > 0.0f ? L : 0.0f)));
   };
   // after a change of direction at local position (qx, qy, qz): reciprocals, face spacings, distances
+  auto set_steps = [&](bool lev) {
+    const int ax_ = (da > -kTiny) ? 1 : -1, ay_ = (db > -kTiny) ? 1 : -1, az_ = (dc > -kTiny) ? 1 : -1;
+    const int sx = lev ? ax_ * A.mx : ax_, sy = lev ? ay_ * A.my : ay_, sz = lev ? az_ * A.mz : az_;
+    stp = ((uint32_t)sx & 0xffu) | (((uint32_t)sy & 0xffu) << 8) | (((uint32_t)sz & 0xffu) << 16);
+  };
   auto place = [&](float qx, float qy, float qz) {
+    const bool lev = __float_as_int(kh) < 0;
+    set_steps(lev);
     const float va = nudge(da), vb = nudge(db), vc = nudge(dc);
     const float ia = 1.0f / va, ib = 1.0f / vb, ic = 1.0f / vc;
-    delx = A.Lx * fabsf(ia); dely = A.Ly * fabsf(ib); delz = A.Lz * fabsf(ic);
-    rx = ((va > 0.0f ? A.Lx : 0.0f) - qx) * ia;
-    ry = ((vb > 0.0f ? A.Ly : 0.0f) - qy) * ib;
-    rz = ((vc > 0.0f ? A.Lz : 0.0f) - qz) * ic;
+    const float Lx = lev ? A.Lx1 : A.Lx, Ly = lev ? A.Ly1 : A.Ly, Lz = lev ? A.Lz1 : A.Lz;
+    delx = Lx * fabsf(ia); dely = Ly * fabsf(ib); delz = Lz * fabsf(ic);
+    rx = ((va > 0.0f ? Lx : 0.0f) - qx) * ia;
+    ry = ((vb > 0.0f ? Ly : 0.0f) - qy) * ib;
+    rz = ((vc > 0.0f ? Lz : 0.0f) - qz) * ic;
   };
+  auto cell_of = [&]() { return ((unsigned)cz * (unsigned)A.ncy + (unsigned)cy) * (unsigned)A.ncx + (unsigned)cx; };
   auto flush_thread_counters = [&]() {
     unsigned long long v;
     v = warp_sum(t_sc - t_hg);  if (lane == 0 && v) atomicAdd(&s_cnt[C_RAY], v);
     v = warp_sum(t_hg);         if (lane == 0 && v) atomicAdd(&s_cnt[C_HG], v);
     v = warp_sum(t_sfc);        if (lane == 0 && v) atomicAdd(&s_cnt[C_SFC_HITS], v);
     v = warp_sum(t_cells);      if (lane == 0 && v) atomicAdd(&s_cnt[C_CELLS], v);
+    v = warp_sum(t_relevel);    if (lane == 0 && v) atomicAdd(&s_cnt[C_RELEVEL], v);
     // null = events - scatters - absorptions; absorptions are counted at the photon's end, so park the
     // (events - scatters) part here and subtract C_ATM_ABS when the block folds its counters
     v = warp_sum(t_ev - t_sc);  if (lane == 0 && v) atomicAdd(&s_cnt[C_NULL], v);
@@ -184,7 +205,7 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
       if (__any_sync(0xffffffffu, t_ev > (1u << 30) || t_cells > (1u << 30))) {
         flush_thread_counters();                   // keep the 32-bit running totals far from overflow
         if (kRecords) { b_ev -= t_ev; b_sc -= t_sc; b_sfc -= t_sfc; }
-        t_ev = t_sc = t_hg = t_sfc = t_cells = 0;
+        t_ev = t_sc = t_hg = t_sfc = t_cells = t_relevel = 0;
       }
       if (got) {
         // ---- §3.6 launch, event index 0 ------------------------------------------------------
@@ -202,16 +223,25 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
         }
         cx = ix / A.bx; cy = iy / A.by; cz = A.ncz - 1;
         da = A.sun_x; db = A.sun_y; dc = A.sun_z;
+        // §3.5b: the sign bit of the stored majorant marks the cells of a merged cell
+        kh = __ldg(A.khat + cell_of());
+        const bool lev = __float_as_int(kh) < 0;
+        set_steps(lev);
+        int wx = A.bx, wy = A.by;             // cell extent in voxels at this level
+        float Lx = A.Lx, Ly = A.Ly, Lz = A.Lz;
+        if (lev) {
+          cx &= -A.mx; cy &= -A.my; cz &= -A.mz;      // merged-cell origin (factors are powers of two)
+          wx *= A.mx; wy *= A.my; Lx = A.Lx1; Ly = A.Ly1; Lz = A.Lz1;
+        }
         // place() with the beam's host-computed reciprocals (same IEEE operations)
-        delx = A.Lx * fabsf(A.sun_ix); dely = A.Ly * fabsf(A.sun_iy); delz = A.Lz * fabsf(A.sun_iz);
-        rx = ((A.sun_ix > 0.0f ? A.Lx : 0.0f) - ((float)(ix % A.bx) + u24(X.x)) * A.dx) * A.sun_ix;
-        ry = ((A.sun_iy > 0.0f ? A.Ly : 0.0f) - ((float)(iy % A.by) + u24(X.y)) * A.dy) * A.sun_iy;
-        rz = ((A.sun_iz > 0.0f ? A.Lz : 0.0f) - A.Lz) * A.sun_iz;
+        delx = Lx * fabsf(A.sun_ix); dely = Ly * fabsf(A.sun_iy); delz = Lz * fabsf(A.sun_iz);
+        rx = ((A.sun_ix > 0.0f ? Lx : 0.0f) - ((float)(ix % wx) + u24(X.x)) * A.dx) * A.sun_ix;
+        ry = ((A.sun_iy > 0.0f ? Ly : 0.0f) - ((float)(iy % wy) + u24(X.y)) * A.dy) * A.sun_iy;
+        rz = ((A.sun_iz > 0.0f ? Lz : 0.0f) - Lz) * A.sun_iz;
         direct = true;
         e = 1;
         if (kRecords) { b_ev = t_ev; b_sc = t_sc; b_sfc = t_sfc; }
         draw();
-        kh = __ldg(A.khat + (((unsigned)cz * (unsigned)A.ncy + (unsigned)cy) * (unsigned)A.ncx + (unsigned)cx));
         st = ST_MOVE;
       }
       continue;
@@ -221,15 +251,18 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
     const bool stuck = (nM == 0);                  // nothing can move: run the fullest parked phase
     if (!stuck && nC < kCollideBatch && nS < kScatterBatch && nB < kBoundaryBatch) {
       // ---- MOVE: nearest face of the current cell (ties x < y < z), then cross or park (§3.7) -------
+      // index step per axis: +-1 cell, or +-m cells inside a merged cell
+      const int sx = (int)(stp << 24) >> 24, sy = (int)(stp << 16) >> 24, sz = (int)(stp << 8) >> 24;
 #pragma unroll
-      for (int rep = 0; rep < kMoveSteps; ++rep)
+      for (int rep = 0; rep < kMoveSteps; ++rep) {
+      if (kMoveMin > 0 && rep > 0 && __popc(__ballot_sync(0xffffffffu, st == ST_MOVE)) < kMoveMin) break;
       if (st == ST_MOVE) {
         const bool ax0 = (rx <= ry) && (rx <= rz);
         const bool ax1 = !ax0 && (ry <= rz);
         const bool ax2 = !ax0 && !ax1;
         const float t = ax0 ? rx : (ax1 ? ry : rz);
-        const float dtau = kh * t;
-        if (kh > 0.0f && tau <= dtau) {
+        const float dtau = fabsf(kh) * t;
+        if (fabsf(kh) > 0.0f && tau <= dtau) {
           st = ST_COLLIDE;                           // the tentative collision comes first
         } else {
           // leave the cell through that face, carrying the residual optical depth
@@ -238,18 +271,26 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
           rx = ax0 ? delx : rx - t;
           ry = ax1 ? dely : ry - t;
           rz = ax2 ? delz : rz - t;
-          // step the cell index; x and y wrap (periodic).  d > -tiny is "the nudged component is positive"
+          // step the cell index; x and y wrap (periodic)
           if (kPow2) {
-            if (ax0) cx = (cx + ((da > -kTiny) ? 1 : -1)) & (A.ncx - 1);
-            if (ax1) cy = (cy + ((db > -kTiny) ? 1 : -1)) & (A.ncy - 1);
+            if (ax0) cx = (cx + sx) & (A.ncx - 1);
+            if (ax1) cy = (cy + sy) & (A.ncy - 1);
           } else {
-            if (ax0) { cx += (da > -kTiny) ? 1 : -1; cx = (cx == A.ncx) ? 0 : cx; cx = (cx < 0) ? A.ncx - 1 : cx; }
-            if (ax1) { cy += (db > -kTiny) ? 1 : -1; cy = (cy == A.ncy) ? 0 : cy; cy = (cy < 0) ? A.ncy - 1 : cy; }
+            if (ax0) { cx += sx; cx = (cx >= A.ncx) ? cx - A.ncx : cx; cx = (cx < 0) ? cx + A.ncx : cx; }
+            if (ax1) { cy += sy; cy = (cy >= A.ncy) ? cy - A.ncy : cy; cy = (cy < 0) ? cy + A.ncy : cy; }
           }
-          if (ax2) cz += (dc > -kTiny) ? 1 : -1;
-          if ((unsigned)cz >= (unsigned)A.ncz) st = ST_BOUNDARY;   // surface (cz = -1) or domain top
-          else kh = __ldg(A.khat + (((unsigned)cz * (unsigned)A.ncy + (unsigned)cy) * (unsigned)A.ncx + (unsigned)cx));
+          if (ax2) cz += sz;
+          if ((unsigned)cz >= (unsigned)A.ncz) st = ST_BOUNDARY;   // surface (cz < 0) or domain top
+          else {
+            const float raw = __ldg(A.khat + cell_of());
+            if ((__float_as_int(raw) ^ __float_as_int(kh)) < 0) {   // §3.7b: the entered cell is at the other level
+              st = ST_BOUNDARY;
+              stp = (stp & 0x00ffffffu) | (ax0 ? 0u : (ax1 ? 0x01000000u : 0x02000000u));
+            }
+            kh = raw;
+          }
         }
+      }
       }
       continue;
     }
@@ -262,7 +303,9 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
     if (phase == ST_SCATTER) {
       // ---- SCATTER: phase-function angle, rotation, new distances to the faces (§3.9) --------------
       if (st == ST_SCATTER) {
-        const float qx = local(da, rx, A.Lx), qy = local(db, ry, A.Ly), qz = local(dc, rz, A.Lz);
+        const bool lev = __float_as_int(kh) < 0;
+        const float qx = local(da, rx, lev ? A.Lx1 : A.Lx), qy = local(db, ry, lev ? A.Ly1 : A.Ly),
+                    qz = local(dc, rz, lev ? A.Lz1 : A.Lz);
         float mu;
         if (sg < 1.5f) { mu = sample_hg(sg, u24(sw2)); ++t_hg; }
         else           { mu = sample_rayleigh(u24(sw2)); }
@@ -283,18 +326,20 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
     if (phase == ST_COLLIDE) {
       // ---- COLLIDE: fetch the voxel, classify, draw the next event (§3.8) --------------------------
       if (st == ST_COLLIDE) {
-        const float s = tau * (1.0f / kh);
+        const bool lev = __float_as_int(kh) < 0;
+        const float s = tau * (1.0f / fabsf(kh));
         rx = fmaxf(0.0f, rx - s); ry = fmaxf(0.0f, ry - s); rz = fmaxf(0.0f, rz - s);
-        const float qx = local(da, rx, A.Lx), qy = local(db, ry, A.Ly), qz = local(dc, rz, A.Lz);
-        const int lx = min((int)(qx * A.rdx), A.bx - 1);
-        const int ly = min((int)(qy * A.rdy), A.by - 1);
-        const int lz = min((int)(qz * A.rdz), A.bz - 1);
+        const float qx = local(da, rx, lev ? A.Lx1 : A.Lx), qy = local(db, ry, lev ? A.Ly1 : A.Ly),
+                    qz = local(dc, rz, lev ? A.Lz1 : A.Lz);
+        const int lx = min((int)(qx * A.rdx), (lev ? A.mx * A.bx : A.bx) - 1);
+        const int ly = min((int)(qy * A.rdy), (lev ? A.my * A.by : A.by) - 1);
+        const int lz = min((int)(qz * A.rdz), (lev ? A.mz * A.bz : A.bz) - 1);
         // 32-bit indices: rt_create_grid refuses grids of 2^32 voxels or more
         const unsigned vox = ((unsigned)(cz * A.bz + lz) * (unsigned)A.ny + (unsigned)(cy * A.by + ly)) * (unsigned)A.nx
                              + (unsigned)(cx * A.bx + lx);
         const float4 v = __ldg(&A.optics[vox]);
         ++t_ev;
-        const float xi = u1 * kh;
+        const float xi = u1 * fabsf(kh);
         st = ST_MOVE;
         if (xi < v.x) {                             // absorbed by the gas / droplet
           tally_a = A.atm_abs + vox;
@@ -315,11 +360,43 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
         }
       }
     } else {
-      // ---- BOUNDARY: arrival at the surface (§3.10) or exit through the domain top (§3.11) ----------
-      if (st == ST_BOUNDARY) {
-        const float qx = local(da, rx, A.Lx), qy = local(db, ry, A.Ly);
-        const int hx = cx * A.bx + min((int)(qx * A.rdx), A.bx - 1);
-        const int hy = cy * A.by + min((int)(qy * A.rdy), A.by - 1);
+      // ---- BOUNDARY: arrival at the surface (§3.10), exit through the domain top (§3.11), or a change
+      //      of level at the face of a merged cell (§3.7b) -------------------------------------------
+      if (st == ST_BOUNDARY && (unsigned)cz < (unsigned)A.ncz) {
+        const bool px = da > -kTiny, py = db > -kTiny, pz = dc > -kTiny;   // nudged component positive
+        const int ax = (int)(stp >> 24);
+        const bool lev = !(__float_as_int(kh) < 0);   // kh already holds the ENTERED cell's word
+        if (!lev) {
+          // into a merged cell: distances to ITS faces (n whole cells further on the other two axes),
+          // the index becomes its origin
+          const int ox = cx & (A.mx - 1), oy = cy & (A.my - 1), oz = cz & (A.mz - 1);   // powers of two
+          const float fx = (float)A.mx, fy = (float)A.my, fz = (float)A.mz;
+          rx = (ax == 0) ? delx * fx : fmaf((float)(px ? A.mx - 1 - ox : ox), delx, rx);
+          ry = (ax == 1) ? dely * fy : fmaf((float)(py ? A.my - 1 - oy : oy), dely, ry);
+          rz = (ax == 2) ? delz * fz : fmaf((float)(pz ? A.mz - 1 - oz : oz), delz, rz);
+          delx *= fx; dely *= fy; delz *= fz;       // exact: the factors are powers of two
+          cx -= ox; cy -= oy; cz -= oz;
+          set_steps(true);
+        } else {
+          // out of a merged cell into single cells: which cell of the entered block on the other two
+          // axes (k whole cells before the block's face), and the distances to that cell's faces
+          delx *= A.rmx; dely *= A.rmy; delz *= A.rmz;
+          if (ax == 0) { rx = delx; if (!px) cx += A.mx - 1; }
+          else { const int k = min(A.mx - 1, (int)(rx / delx)); rx = fmaxf(0.0f, fmaf(-(float)k, delx, rx)); cx += px ? A.mx - 1 - k : k; }
+          if (ax == 1) { ry = dely; if (!py) cy += A.my - 1; }
+          else { const int k = min(A.my - 1, (int)(ry / dely)); ry = fmaxf(0.0f, fmaf(-(float)k, dely, ry)); cy += py ? A.my - 1 - k : k; }
+          if (ax == 2) { rz = delz; if (!pz) cz += A.mz - 1; }
+          else { const int k = min(A.mz - 1, (int)(rz / delz)); rz = fmaxf(0.0f, fmaf(-(float)k, delz, rz)); cz += pz ? A.mz - 1 - k : k; }
+          kh = __ldg(A.khat + cell_of());             // the single cell's own majorant (sign bit clear)
+          set_steps(false);
+        }
+        ++t_relevel;
+        st = ST_MOVE;
+      } else if (st == ST_BOUNDARY) {
+        const bool lev = __float_as_int(kh) < 0;
+        const float qx = local(da, rx, lev ? A.Lx1 : A.Lx), qy = local(db, ry, lev ? A.Ly1 : A.Ly);
+        const int hx = cx * A.bx + min((int)(qx * A.rdx), (lev ? A.mx * A.bx : A.bx) - 1);
+        const int hy = cy * A.by + min((int)(qy * A.rdy), (lev ? A.my * A.by : A.by) - 1);
         const unsigned col = (unsigned)hy * (unsigned)A.nx + (unsigned)hx;
         if (cz >= 0) {                              // left through the domain top
           tally_a = A.toa_up + col;
@@ -333,13 +410,12 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
             float sp, cp;
             sincos_2pi(u24(w3), sp, cp);
             da = sn * cp; db = sn * sp; dc = mu;
-            direct = false; cz = 0;
+            direct = false; cz = 0;                 // back in the cell it left: same level, same majorant
             place(qx, qy, 0.0f);
             ++e;
             if (e > kEventCap) { fate = 4; term = 0; }   // §3.12
             else {
               draw();
-              kh = __ldg(A.khat + (((unsigned)cz * (unsigned)A.ncy + (unsigned)cy) * (unsigned)A.ncx + (unsigned)cx));
               st = ST_MOVE;
             }
           } else {

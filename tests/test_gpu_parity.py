@@ -19,9 +19,9 @@ def _rt():
     return rt
 
 
-def _run_gpu(cfg_grid, opt, zen, azi, n, seed=1, stream_id=0, first=0, records=True):
+def _run_gpu(cfg_grid, opt, zen, azi, n, seed=1, stream_id=0, first=0, records=True, accel=None):
     rt = _rt()
-    g = rt.Grid(*cfg_grid, device=0)
+    g = rt.Grid(*cfg_grid, device=0, **(accel or {}))
     g.set_optics(opt["k_ext"], opt["k_ext_cloud"], opt["ssa"], opt["g"], opt["sfc_albedo"])
     rec = g.trace(zen, azi, n, first_photon_id=first, seed=seed, stream_id=stream_id, records=records)
     t = g.read_tallies()
@@ -36,13 +36,13 @@ def _same_fraction(a, b):
 
 def _compare(cfg, opt, n, min_same64=0.999):
     rt = _rt()
-    t, rec = _run_gpu(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed)
+    t, rec = _run_gpu(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed, accel=cfg.accel)
     assert t.closure() == n * rt.W0                      # bit-exact closure
     assert t.counters.n_capped == 0 and t.counters.n_photons == n
     o32, rec32, _ = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed, precision=32,
-                            records=True, n_threads=8)
+                            records=True, n_threads=8, **cfg.accel)
     o64, rec64, _ = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed, precision=64,
-                            records=True, n_threads=8)
+                            records=True, n_threads=8, **cfg.accel)
     assert o64.closure() == n * rt.W0
     # same precision, same fixed operations: identical paths and identical integer tallies
     assert _same_fraction(rec, rec32) == 1.0
@@ -104,6 +104,15 @@ def test_pack_and_majorant_bit_exact():
     want = O.pack_optics_f32(opt["k_ext"], opt["k_ext_cloud"], opt["ssa"], opt["g"])
     assert np.array_equal(packed.view(np.uint32), want.view(np.uint32))
     assert np.array_equal(kh, O.majorant(cfg.nx, cfg.ny, cfg.nz, *cfg.block, opt["k_ext"]))
+    # merged cells: same table, sign bits included
+    for block, merge, ratio in (((2, 2, 2), (8, 8, 4), 1.25), ((4, 4, 4), (2, 4, 2), 1.05)):
+        g = rt.Grid(*cfg.grid[:6], *block, device=0, merge=merge, merge_ratio=ratio)
+        g.set_optics(opt["k_ext"], opt["k_ext_cloud"], opt["ssa"], opt["g"], opt["sfc_albedo"])
+        kh = g.read_majorant().numpy()
+        g.close()
+        want = O.majorant(cfg.nx, cfg.ny, cfg.nz, *block, opt["k_ext"], merge=merge, merge_ratio=ratio)
+        assert np.array_equal(kh.view(np.uint32), want.view(np.uint32)), (block, merge)
+        assert np.signbit(kh).any() and not np.signbit(kh).all()
 
 
 def test_config1_full():
@@ -126,9 +135,46 @@ def test_config2_sample():
     assert nb > 0 and rms < 0.02, (rms, nb)
 
 
+def test_config2_merged_cells():
+    """BASELINE.json configs[1] field with 2^3-voxel cells merged 8 x 8 x 4 where the air is clear (DESIGN.md
+    §3.5b, §3.7b): every level change, in both directions and on all axes, against the oracle."""
+    from dataclasses import replace
+    cfg = replace(CONFIGS[2], block=(2, 2, 2), merge=(8, 8, 4))
+    opt = make_optics(cfg)
+    t, o64, same = _compare(cfg, opt, 1 << 20, min_same64=0.98)
+    assert t.counters.n_relevel > (1 << 20)
+
+
+def test_merged_cells_non_power_of_two_grid():
+    """Acceleration grid of 24 x 12 x 16 cells (wrap by compare, not by mask), merged 4 x 2 x 4, sun from the
+    north-east so photons wrap in both x and y."""
+    rt = _rt()
+    from rt_inputs.fields import Config
+    nx, ny, nz = 48, 24, 32
+    rng = np.random.default_rng(17)
+    k = np.full((nz, ny, nx), 1.5e-4)
+    for _ in range(6):
+        x, y, z = rng.integers(0, nx - 6), rng.integers(0, ny - 6), rng.integers(6, nz - 10)
+        k[z:z + 6, y:y + 5, x:x + 6] = rng.uniform(5e-3, 3e-2, size=(6, 5, 6))
+    cfg, opt = plane_parallel(nx, ny, nz, 60.0, 40.0, 30.0, 0.0, 0.0, albedo=0.4, block=(2, 2, 2))
+    opt["k_ext"] = k.astype(np.float32)
+    opt["ssa"] = np.where(k > 1e-3, 0.999, 0.6).astype(np.float32)
+    opt["k_ext_cloud"] = np.where(k > 1e-3, k, 0.0).astype(np.float32)
+    opt["g"][:] = 0.85
+    accel = {"merge": (4, 2, 4), "merge_ratio": 1.25}
+    n = (1 << 17) + 77
+    t, rec = _run_gpu(cfg.grid, opt, 55.0, 40.0, n, seed=4, accel=accel)
+    o32, rec32, _ = O.trace(cfg.grid, opt, 55.0, 40.0, n, seed=4, precision=32, records=True, n_threads=8, **accel)
+    assert np.array_equal(rec, rec32)
+    for name in ("atm_abs", "sfc_dir", "sfc_dif", "sfc_abs", "toa_up"):
+        assert np.array_equal(getattr(t, name).numpy(), getattr(o32, name)), name
+    assert t.counters.asdict() == o32.counters.asdict() and t.counters.n_relevel > n
+    assert t.closure() == n * rt.W0
+
+
 def test_config3_bench_configuration_sample():
-    """BASELINE.json configs[2] (512x512x128, the field bench.py times), same 2^3-voxel acceleration cells and
-    launch configuration: photon ids [0, 2^19) (two full passes over the columns) against the oracle in
+    """BASELINE.json configs[2] (512x512x128, the field bench.py times), same 2^3-voxel acceleration cells
+    merged 8 x 8 x 4 in clear air and launch configuration: photon ids [0, 2^19) (two full passes over the columns) against the oracle in
     kernel precision, record by record and tally by tally; then the full 2^26-photon launch checked through
     properties that hold at any size (exact closure, counters consistent, no capped photon) and through
     the sampled ids, whose records must not depend on how many other photons share the launch."""
@@ -136,12 +182,12 @@ def test_config3_bench_configuration_sample():
     cfg = CONFIGS[3]
     opt = make_optics(cfg)
     n = 1 << 19
-    g = rt.Grid(*cfg.grid, device=0)
+    g = rt.Grid(*cfg.grid, device=0, **cfg.accel)
     g.set_optics(opt["k_ext"], opt["k_ext_cloud"], opt["ssa"], opt["g"], opt["sfc_albedo"])
     rec = g.trace(cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed, records=True).cpu().numpy().view(np.uint32)
     t = g.read_tallies()
     o32, rec32, _ = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed, precision=32,
-                            records=True, n_threads=8)
+                            records=True, n_threads=8, **cfg.accel)
     assert np.array_equal(rec, rec32)
     for name in ("atm_abs", "sfc_dir", "sfc_dif", "sfc_abs", "toa_up"):
         assert np.array_equal(getattr(t, name).numpy(), getattr(o32, name)), name
@@ -203,8 +249,9 @@ def test_limits_on_gpu():
     t, _ = _run_gpu(cfg.grid, opt, 40.0, 10.0, n, records=False)
     assert int(t.atm_abs.sum()) == 0 and int(t.sfc_abs.sum()) == 0 and int(t.toa_up.sum()) == n * rt.W0
     cfg, opt = plane_parallel(16, 16, 16, 100.0, 100.0, 100.0, 0.0, 0.0, albedo=0.0)
-    t, _ = _run_gpu(cfg.grid, opt, 40.0, 10.0, n, records=False)
-    assert int(t.sfc_dir.sum()) == n * rt.W0 and int(t.sfc_abs.sum()) == n * rt.W0 and t.counters.n_events == 0
+    for accel in (None, {"merge": (2, 2, 2)}):            # merged vacuum: the table holds -0.0
+        t, _ = _run_gpu(cfg.grid, opt, 40.0, 10.0, n, records=False, accel=accel)
+        assert int(t.sfc_dir.sum()) == n * rt.W0 and int(t.sfc_abs.sum()) == n * rt.W0 and t.counters.n_events == 0
 
 
 def test_bad_inputs_fail_loudly():

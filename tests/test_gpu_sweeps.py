@@ -29,7 +29,7 @@ def test_config4_spectral_sweep():
     pts = spectral_points(112)
     counts = split_photons(cfg.n_photons, [p["weight"] for p in pts])
     assert sum(counts) == cfg.n_photons and len(counts) == 112 and min(counts) > 0
-    g = rt.Grid(*cfg.grid, device=0)
+    g = rt.Grid(*cfg.grid, device=0, **cfg.accel)
 
     # the device-side field assembly hands the library the same fp32 arrays as the host recipe
     sample = (0, 37, 111)
@@ -50,7 +50,7 @@ def test_config4_spectral_sweep():
         rec = g.trace(cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed, stream_id=j, records=True)
         t = g.read_tallies()
         o32, rec32, _ = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed, stream_id=j,
-                                precision=32, records=True, n_threads=8)
+                                precision=32, records=True, n_threads=8, **cfg.accel)
         assert np.array_equal(rec.cpu().numpy().view(np.uint32), rec32), j
         for name in TALLIES:
             assert np.array_equal(getattr(t, name).numpy(), getattr(o32, name)), (j, name)
@@ -78,7 +78,7 @@ def test_config5_convergence_sweep():
     from paper_2208_05247_b200.sweeps import convergence_sweep
     cfg = CONFIGS[5]
     opt = make_optics(cfg)
-    g = rt.Grid(*cfg.grid, device=0)
+    g = rt.Grid(*cfg.grid, device=0, **cfg.accel)
     g.set_optics(*[opt[k] for k in NAMES])
 
     # 1 photon per column (2^20 photons, one full pass) against the oracle in kernel precision
@@ -86,7 +86,7 @@ def test_config5_convergence_sweep():
     rec = g.trace(cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed, records=True).cpu().numpy().view(np.uint32)
     t = g.read_tallies()
     o32, rec32, _ = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed, precision=32,
-                            records=True, n_threads=8)
+                            records=True, n_threads=8, **cfg.accel)
     assert np.array_equal(rec, rec32)
     for name in TALLIES:
         assert np.array_equal(getattr(t, name).numpy(), getattr(o32, name)), name
