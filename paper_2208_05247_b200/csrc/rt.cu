@@ -108,6 +108,14 @@ int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photon
   A.records = records;
   A.n_photons = n_photons; A.first_id = first_id; A.ncol = c->ncol;
   A.n_full = (n_photons / c->ncol) * c->ncol;
+  {
+    // ids per work-counter atomic: 128, or fewer (a multiple of 32) when the launch has under ~8 chunks per warp,
+    // so that short launches (one spectral point of config 4) balance over all resident warps
+    const unsigned long long warps = (unsigned long long)(records ? c->trace_blocks_rec : c->trace_blocks) * (rt::kTraceThreads / 32);
+    unsigned long long ch = n_photons / (warps * 8ull);
+    ch = (ch / 32ull) * 32ull;
+    A.chunk = (unsigned)(ch < 32ull ? 32ull : (ch > (unsigned long long)rt::kChunk ? (unsigned long long)rt::kChunk : ch));
+  }
   A.keys = rt::philox_round_keys((uint32_t)seed, (uint32_t)(seed >> 32)); A.stream_id = stream_id;
   RT_CUDA(c, cudaMemsetAsync(A.next_photon, 0, sizeof(unsigned long long), st));
   RT_CUDA(c, cudaEventRecord(c->ev0, st));

@@ -28,7 +28,7 @@ constexpr unsigned long long kW0 = 1ull << 32;  // tally quanta per photon
 constexpr uint32_t kEventCap = 1u << 20;        // §3.12
 constexpr float kTiny = 1e-30f;                 // direction components are nudged away from 0
 constexpr int kTraceThreads = 256;
-constexpr int kChunk = 128;                     // photon ids a warp takes per global atomic
+constexpr int kChunk = 128;                     // photon ids a warp takes per global atomic (fewer in small launches)
 #ifndef RT_MIN_BLOCKS
 #define RT_MIN_BLOCKS 3
 #endif
@@ -78,6 +78,7 @@ struct TraceArgs {
   unsigned long long* next_photon;     // work counter, zeroed before launch
   uint32_t* records;                   // 4 words per photon or nullptr
   unsigned long long n_photons, first_id, n_full, ncol;
+  unsigned chunk;                      // photon ids per global atomic: kChunk, or less so that a small launch still spreads over all warps
   PhiloxKeys keys;                     // round keys of the Philox key (seed)
   uint32_t stream_id;
 };
@@ -176,10 +177,14 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
   for (;;) {
     // the vote: one warp-wide integer add counts the lanes in each of the five states (6 bits each)
     const unsigned votes = __reduce_add_sync(0xffffffffu, 1u << (6u * st));
-    const int nD = votes & 63u, nM = (votes >> 6) & 63u, nC = (votes >> 12) & 63u, nS = (votes >> 18) & 63u,
-              nB = (votes >> 24) & 63u;
+    // count >= threshold for all five states at once: adding 32 - threshold to a 6-bit field sets its top bit
+    // exactly when the count (<= 32) has reached the threshold, and never carries into the next field
+    constexpr unsigned kBias = (32u - kRegenBatch) | ((32u - 1u) << 6) | ((32u - kCollideBatch) << 12) |
+                               ((32u - kScatterBatch) << 18) | ((32u - kBoundaryBatch) << 24);
+    constexpr unsigned bD = 32u, bM = 32u << 6, bC = 32u << 12, bS = 32u << 18, bB = 32u << 24;
+    const unsigned full = (votes + kBias) & (bD | bM | bC | bS | bB);
 
-    if (!exhausted && (nD >= kRegenBatch || nD == 32)) {
+    if (!exhausted && (full & bD)) {
       // ---- regeneration: hand photon ids to the idle lanes -------------------------------------
       unsigned waiting = __ballot_sync(0xffffffffu, st == ST_DEAD);
       bool got = false;
@@ -194,10 +199,10 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
         waiting &= ~took;
         if (waiting && pass == 0) {
           unsigned long long base = 0;
-          if (lane == 0) base = atomicAdd(A.next_photon, (unsigned long long)kChunk);
+          if (lane == 0) base = atomicAdd(A.next_photon, (unsigned long long)A.chunk);
           base = __shfl_sync(0xffffffffu, base, 0);
           pool_next = base < A.n_photons ? base : A.n_photons;
-          pool_end = (base + kChunk < A.n_photons) ? base + kChunk : A.n_photons;
+          pool_end = (base + A.chunk < A.n_photons) ? base + A.chunk : A.n_photons;
           if (pool_next > pool_end) pool_next = pool_end;
         }
       }
@@ -246,10 +251,10 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
       }
       continue;
     }
-    if (nD == 32) break;
+    if ((votes & 63u) == 32u) break;
 
-    const bool stuck = (nM == 0);                  // nothing can move: run the fullest parked phase
-    if (!stuck && nC < kCollideBatch && nS < kScatterBatch && nB < kBoundaryBatch) {
+    // a lane moves and no parked phase has reached its batch size
+    if ((full & (bM | bC | bS | bB)) == bM) {
       // ---- MOVE: nearest face of the current cell (ties x < y < z), then cross or park (§3.7) -------
       // index step per axis: +-1 cell, or +-m cells inside a merged cell
       const int sx = (int)(stp << 24) >> 24, sy = (int)(stp << 16) >> 24, sz = (int)(stp << 8) >> 24;
@@ -297,8 +302,12 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
 
     // which parked phase: one that reached its batch size, or (nothing moves) the fullest one
     int phase;
-    if (stuck) phase = (nC >= nS && nC >= nB) ? ST_COLLIDE : (nS >= nB ? ST_SCATTER : ST_BOUNDARY);
-    else       phase = (nC >= kCollideBatch) ? ST_COLLIDE : (nS >= kScatterBatch ? ST_SCATTER : ST_BOUNDARY);
+    if (!(full & bM)) {                            // nothing can move
+      const unsigned nC = (votes >> 12) & 63u, nS = (votes >> 18) & 63u, nB = (votes >> 24) & 63u;
+      phase = (nC >= nS && nC >= nB) ? ST_COLLIDE : (nS >= nB ? ST_SCATTER : ST_BOUNDARY);
+    } else {
+      phase = (full & bC) ? ST_COLLIDE : ((full & bS) ? ST_SCATTER : ST_BOUNDARY);
+    }
 
     if (phase == ST_SCATTER) {
       // ---- SCATTER: phase-function angle, rotation, new distances to the faces (§3.9) --------------
