@@ -30,10 +30,10 @@ REF_SAMPLE_PHOTONS = 1 << 23      # per --impl reference step: 32 photons per co
 CPU_BASELINE_PHOTONS = 1 << 25    # cpu_baseline leg: 128 photons per column (~10 s on 16 cores)
 SECTOR = 32                       # bytes moved per random 16-byte gather (one DRAM/L2 sector)
 # thread instructions per unit of the method's work, counted in the shipped kernel's SASS
-# (profiles/r1_trace_kernel.md): one MOVE step (find the nearest face; cross or park),
+# (profiles/r1b_trace_kernel.md E): one MOVE step (find the nearest face; cross or park),
 # one tentative collision (gather, classify, Philox draw, logarithm), one real scatter, one surface
-# or top arrival, one photon launch.
-INST_PER_UNIT = {"move": 50, "collide": 200, "scatter": 240, "boundary": 150, "launch": 190}
+# or top arrival, one photon launch, one change of level at a merged cell's face.
+INST_PER_UNIT = {"move": 52, "collide": 190, "scatter": 250, "boundary": 150, "launch": 265, "relevel": 45}
 
 
 def _peaks():
@@ -272,14 +272,14 @@ def run_ours(args):
     # ---- roofline of the dominant kernel (trace_kernel), this rank ---------------------------------------
     # The kernel is bound by instruction issue, not by memory (0.5 % of the HBM copy rate, 80 %
     # of issue slots busy), so the bound is "alu".  Algorithmic work = thread instructions the method's steps
-    # need, per unit, as counted in the shipped kernel's SASS (profiles/r1_trace_kernel.md) x the units the
+    # need, per unit, as counted in the shipped kernel's SASS (profiles/r1b_trace_kernel.md) x the units the
     # launch processed; peak = every lane of every SM sub-partition issuing each cycle at the SM clock.
     hbm_peak, peak_src = _peaks()
     ms_avg = sum(trace_ms) / len(trace_ms)
     per = {k: v / args.steps for k, v in csum.items()}
     units = {"move": per["n_cell_steps"] + per["n_events"], "collide": per["n_events"],
              "scatter": per["n_hg"] + per["n_rayleigh"], "boundary": per["n_sfc_hits"] + per["n_toa"],
-             "launch": per["n_photons"]}
+             "launch": per["n_photons"], "relevel": per["n_relevel"]}
     alg_inst = sum(INST_PER_UNIT[k] * units[k] for k in units)
     sm_mhz = _sm_max_mhz()
     alu_peak = 148 * 4 * 32 * sm_mhz * 1e6 / 1e12            # T thread-instructions / s
@@ -292,7 +292,8 @@ def run_ours(args):
     if os.path.exists(tpath):
         with open(tpath) as f:
             tj = json.load(f)
-        if tj.get("n_photons") == n and tj.get("workload") == cfg.name and tj.get("block") == list(cfg.block):
+        if (tj.get("n_photons") == n and tj.get("workload") == cfg.name and tj.get("block") == list(cfg.block)
+                and tj.get("merge", [1, 1, 1]) == list(cfg.merge)):
             traffic = tj.get("dram_bytes_per_launch")
     trace_events_per_s = ev_per_launch / (ms_avg * 1e-3)
     trace_gathers_per_s = (units["move"] + units["collide"]) / (ms_avg * 1e-3)   # majorant + voxel loads
