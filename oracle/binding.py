@@ -10,14 +10,16 @@ import numpy as np
 from . import build as _build
 
 W0 = 1 << 32  # tally quanta per photon
-FATE_ATM_ABS, FATE_SFC_ABS, FATE_TOD_EXIT, FATE_CAPPED = 1, 2, 3, 4
+FATE_ATM_ABS, FATE_SFC_ABS, FATE_TOD_EXIT, FATE_CAPPED, FATE_ROULETTE = 1, 2, 3, 4, 5
 
 COUNTER_FIELDS = ("n_photons", "n_events", "n_null", "n_rayleigh", "n_hg", "n_atm_abs",
-                  "n_sfc_hits", "n_sfc_abs", "n_toa", "n_capped", "n_cell_steps", "n_relevel", "capped_energy")
+                  "n_sfc_hits", "n_sfc_abs", "n_toa", "n_capped", "n_cell_steps", "n_relevel",
+                  "n_roulette_killed", "n_roulette_kept", "capped_energy", "roulette_lost", "roulette_gained")
+N_SIGNED = 3  # the last three are int64 energies
 
 
 class Counters(C.Structure):
-    _fields_ = [(n, C.c_uint64) for n in COUNTER_FIELDS[:-1]] + [("capped_energy", C.c_int64)]
+    _fields_ = [(n, C.c_uint64) for n in COUNTER_FIELDS[:-N_SIGNED]] + [(n, C.c_int64) for n in COUNTER_FIELDS[-N_SIGNED:]]
 
     def asdict(self):
         return {n: int(getattr(self, n)) for n in COUNTER_FIELDS}
@@ -34,7 +36,7 @@ def lib():
         ip = C.POINTER(C.c_int64)
         _lib.orc_trace.restype = C.c_int
         _lib.orc_trace.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float,
-                                   C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_float,
+                                   C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_float, C.c_int,
                                    fp, fp, fp, fp, fp, C.c_double, C.c_double,
                                    C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint32, ip, ip, ip, ip, ip,
                                    C.POINTER(Counters), C.POINTER(C.c_uint32), C.c_int,
@@ -60,16 +62,20 @@ class Tallies:
         self.counters = Counters()
 
     def closure(self):
-        """Sum of the terminal bins (must equal n_photons * W0 exactly)."""
+        """Sum of the terminal bins (must equal n_photons * W0 exactly); in weighted mode the roulette
+        ledger (energy of ended photons minus energy given to survivors) is part of the balance."""
         return (int(self.atm_abs.sum()) + int(self.sfc_abs.sum()) + int(self.toa_up.sum())
-                + int(self.counters.capped_energy))
+                + int(self.counters.capped_energy) + int(self.counters.roulette_lost)
+                - int(self.counters.roulette_gained))
 
 
 def trace(grid, optics, zenith_deg, azimuth_deg, n_photons, first_photon_id=0, seed=1, stream_id=0,
-          precision=64, tallies=None, records=False, n_threads=1, merge=(1, 1, 1), merge_ratio=1.25):
+          precision=64, tallies=None, records=False, n_threads=1, merge=(1, 1, 1), merge_ratio=1.25,
+          weighted=False):
     """Run the oracle.  grid = (nx, ny, nz, dx, dy, dz, bx, by, bz); optics = dict with
     k_ext, k_ext_cloud, ssa, g ([nz][ny][nx] fp32) and sfc_albedo ([ny][nx] fp32); merge = merged-cell
-    factors ((1, 1, 1) = single-level acceleration grid).
+    factors ((1, 1, 1) = single-level acceleration grid); weighted = the paper's absorption
+    weights + Russian roulette instead of analog absorption.
     Returns (tallies, records or None, elapsed seconds of the photon loop)."""
     nx, ny, nz, dx, dy, dz, bx, by, bz = grid
     k, kp = _f32(optics["k_ext"])
@@ -83,7 +89,7 @@ def trace(grid, optics, zenith_deg, azimuth_deg, n_photons, first_photon_id=0, s
     ip = C.POINTER(C.c_int64)
     el = C.c_double(0.0)
     rc = lib().orc_trace(int(precision), nx, ny, nz, dx, dy, dz, bx, by, bz, int(merge[0]), int(merge[1]),
-                         int(merge[2]), float(merge_ratio), kp, kcp, wp, gp, alp,
+                         int(merge[2]), float(merge_ratio), int(bool(weighted)), kp, kcp, wp, gp, alp,
                          float(zenith_deg), float(azimuth_deg), int(n_photons), int(first_photon_id),
                          int(seed), int(stream_id), t.atm_abs.ctypes.data_as(ip),
                          t.sfc_dir.ctypes.data_as(ip), t.sfc_dif.ctypes.data_as(ip),

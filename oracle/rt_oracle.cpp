@@ -206,11 +206,11 @@ extern "C" {
 
 struct orc_counters {
   uint64_t n_photons, n_events, n_null, n_rayleigh, n_hg, n_atm_abs, n_sfc_hits, n_sfc_abs,
-      n_toa, n_capped, n_cell_steps, n_relevel;
-  int64_t capped_energy;
+      n_toa, n_capped, n_cell_steps, n_relevel, n_roulette_killed, n_roulette_kept;
+  int64_t capped_energy, roulette_lost, roulette_gained;
 };
 
-enum { ORC_ATM_ABS = 1, ORC_SFC_ABS = 2, ORC_TOD_EXIT = 3, ORC_CAPPED = 4 };
+enum { ORC_ATM_ABS = 1, ORC_SFC_ABS = 2, ORC_TOD_EXIT = 3, ORC_CAPPED = 4, ORC_ROULETTE = 5 };
 
 }  // extern "C"
 
@@ -223,6 +223,7 @@ struct Problem {
   int nx, ny, nz, bx, by, bz;
   int mx, my, mz;            // §3.5b: merged cells of mx x my x mz acceleration cells (1,1,1 = none)
   float merge_ratio;         // §3.5b: merged iff max c3 <= merge_ratio * min c3 over the merged cell's voxels
+  int weighted;              // §3.14: 0 = analog absorption, 1 = the paper's weights + Russian roulette
   float dx, dy, dz;
   const float *k_ext, *k_cloud, *ssa, *g, *albedo;
   double zenith_deg, azimuth_deg;
@@ -333,6 +334,18 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
     bool direct = true;
     uint32_t e = 1, n_ev = 0, n_sc = 0, n_sfc = 0;
     int fate = 0; uint32_t term = 0;
+    // §3.14 weighted mode: integer weight in tally quanta, W0 at launch.  Roulette (Iwabuchi 2006
+    // as quoted in P:56): below W0/2 the photon survives with probability w/W0 exactly (a 32-bit word of
+    // the Philox block at counter e | 2^31 is compared with w) and continues with W0, else it ends; both
+    // branches go to a ledger so that energy closes exactly.  Returns true if the photon ended.
+    uint64_t w = (uint64_t)W0;
+    auto roulette = [&](uint32_t where) {
+      if (w >= (uint64_t)W0 / 2) return false;
+      const U4 Y = philox4x32_10(p_lo, p_hi, e | 0x80000000u, P.stream_id, k0, k1);
+      if ((uint64_t)Y.w < w) { C.roulette_gained += W0 - (int64_t)w; ++C.n_roulette_kept; w = (uint64_t)W0; return false; }
+      C.roulette_lost += (int64_t)w; ++C.n_roulette_killed; fate = ORC_ROULETTE; term = where;
+      return true;
+    };
 
     // ---- step 4: draw for event e -------------------------------------------
     R tau;
@@ -367,7 +380,17 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
         ++n_ev; ++C.n_events;                  // step 6
         // ---- step 8: classify ----------------------------------------------
         R xi = u1 * kh;
-        if (xi < vx.c1) {
+        if (P.weighted) {
+          // §3.14: deposit w * P(absorbed), P = c1 / k_hat as a 24-bit fixed-point number; the rest goes on
+          const R f = vx.c1 * rk;
+          const uint64_t pq = std::min<uint64_t>((uint64_t)1 << 24, (uint64_t)(f * (R)16777216.0));
+          const uint64_t a = (w * pq) >> 24;
+          if (a) add64(&P.atm_abs[vox], (int64_t)a);
+          w -= a;
+          if (w == 0) { ++C.n_atm_abs; fate = ORC_ATM_ABS; term = (uint32_t)vox; break; }
+          xi = E::fma(u1, kh - vx.c1, vx.c1);     // what happens instead: uniform on [c1, k_hat)
+        }
+        if (!P.weighted && xi < vx.c1) {
           add64(&P.atm_abs[vox], W0); ++C.n_atm_abs;
           fate = ORC_ATM_ABS; term = (uint32_t)vox; break;
         } else if (xi < vx.c2) {               // cloud droplet: Henyey-Greenstein
@@ -383,9 +406,10 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
         } else {
           ++C.n_null;                          // null collision: direction unchanged
         }
+        if (P.weighted && roulette((uint32_t)vox)) break;
         ++e;
         if (e > EVENT_CAP) {                   // step 12
-          ++C.n_capped; C.capped_energy += W0; fate = ORC_CAPPED; term = 0; break;
+          ++C.n_capped; C.capped_energy += P.weighted ? (int64_t)w : W0; fate = ORC_CAPPED; term = 0; break;
         }
         draw();
       } else {
@@ -408,13 +432,26 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
           int hy = c[1] * by + std::min((int)(qy * rdy), (lev ? P.my : 1) * by - 1);
           size_t col = (size_t)hy * nx + hx;
           if (at_top) {                        // step 11
-            add64(&P.toa_up[col], W0); ++C.n_toa;
+            add64(&P.toa_up[col], P.weighted ? (int64_t)w : W0); ++C.n_toa;
             fate = ORC_TOD_EXIT; term = (uint32_t)col; break;
           }
           // ---- step 10: Lambertian surface ---------------------------------
           ++C.n_sfc_hits; ++n_sfc;
-          add64(direct ? &P.sfc_dir[col] : &P.sfc_dif[col], W0);
-          if (u1 < (R)P.albedo[col]) {
+          add64(direct ? &P.sfc_dir[col] : &P.sfc_dif[col], P.weighted ? (int64_t)w : W0);
+          bool reflect;
+          if (P.weighted) {
+            // §3.14: the albedo reduces the weight, 24-bit fixed point; always reflect
+            const uint64_t aq = std::min<uint64_t>((uint64_t)1 << 24, (uint64_t)((R)P.albedo[col] * (R)16777216.0));
+            const uint64_t refl = (w * aq) >> 24;
+            if (w - refl) add64(&P.sfc_abs[col], (int64_t)(w - refl));
+            w = refl;
+            if (w == 0) { ++C.n_sfc_abs; fate = ORC_SFC_ABS; term = (uint32_t)col; break; }
+            if (roulette((uint32_t)col)) break;
+            reflect = true;
+          } else {
+            reflect = u1 < (R)P.albedo[col];
+          }
+          if (reflect) {
             R mu = std::sqrt((R)1 - u2), s = std::sqrt(u2);
             R sp, cp; E::sincos_2pi(u3, sp, cp);
             d[0] = s * cp; d[1] = s * sp; d[2] = mu; set_dir();
@@ -423,7 +460,7 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
             place(q);
             ++e;
             if (e > EVENT_CAP) {
-              ++C.n_capped; C.capped_energy += W0; fate = ORC_CAPPED; term = 0; break;
+              ++C.n_capped; C.capped_energy += P.weighted ? (int64_t)w : W0; fate = ORC_CAPPED; term = 0; break;
             }
             draw();
           } else {
@@ -520,7 +557,7 @@ extern "C" {
 // Returns 0 on success, -1 on bad arguments.  Tallies and counters are ADDED to.
 // elapsed_s (may be NULL) receives the wall time of the photon loop only.
 int orc_trace(int precision, int nx, int ny, int nz, float dx, float dy, float dz, int bx, int by,
-              int bz, int mx, int my, int mz, float merge_ratio, const float* k_ext, const float* k_ext_cloud, const float* ssa, const float* g,
+              int bz, int mx, int my, int mz, float merge_ratio, int weighted, const float* k_ext, const float* k_ext_cloud, const float* ssa, const float* g,
               const float* sfc_albedo, double zenith_deg, double azimuth_deg, uint64_t n_photons,
               uint64_t first_photon_id, uint64_t seed, uint32_t stream_id, int64_t* atm_abs,
               int64_t* sfc_dir, int64_t* sfc_dif, int64_t* sfc_abs, int64_t* toa_up,
@@ -530,7 +567,7 @@ int orc_trace(int precision, int nx, int ny, int nz, float dx, float dy, float d
   if (mx <= 0 || my <= 0 || mz <= 0 || (nx / bx) % mx || (ny / by) % my || (nz / bz) % mz) return -1;
   if (!(zenith_deg >= 0.0 && zenith_deg < 90.0)) return -1;
   if (precision != 32 && precision != 64) return -1;
-  Problem P{nx, ny, nz, bx, by, bz, mx, my, mz, merge_ratio, dx, dy, dz, k_ext, k_ext_cloud, ssa, g, sfc_albedo,
+  Problem P{nx, ny, nz, bx, by, bz, mx, my, mz, merge_ratio, weighted ? 1 : 0, dx, dy, dz, k_ext, k_ext_cloud, ssa, g, sfc_albedo,
             zenith_deg, azimuth_deg, n_photons, first_photon_id, seed, stream_id,
             atm_abs, sfc_dir, sfc_dif, sfc_abs, toa_up, records};
   std::vector<float> khat = build_majorant(P);
