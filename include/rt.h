@@ -48,8 +48,10 @@ typedef struct rt_ctx rt_ctx; /* opaque; owned by the library; one CUDA device p
  * the "collision events" of BASELINE.json's metric. */
 typedef struct {
   uint64_t n_photons, n_events, n_null, n_rayleigh, n_hg, n_atm_abs, n_sfc_hits, n_sfc_abs, n_toa,
-      n_capped, n_cell_steps, n_relevel;
-  int64_t capped_energy; /* quanta of photons stopped by the event cap; 0 on all shipped configs */
+      n_capped, n_cell_steps, n_relevel, n_roulette_killed, n_roulette_kept;
+  int64_t capped_energy;   /* quanta of photons stopped by the event cap; 0 on all shipped configs */
+  int64_t roulette_lost;   /* weighted mode: quanta of photons ended by the roulette ... */
+  int64_t roulette_gained; /* ... and quanta given to its survivors (weight reset to RT_W0) */
 } rt_counters;
 
 /* Allocate a context for an nx*ny*nz grid of dx*dy*dz metre voxels with an acceleration grid
@@ -104,6 +106,20 @@ int rt_read_tallies(rt_ctx* ctx, int64_t* atm_abs, int64_t* sfc_dir, int64_t* sf
  * a context that already holds optics must be given them again before the next rt_trace
  * (RT_ESTATE otherwise).  Errors: RT_EINVAL. */
 int rt_set_merge(rt_ctx* ctx, int mx, int my, int mz, float merge_ratio);
+
+/* Absorption scheme of the following rt_trace calls.
+ * RT_MODE_ANALOG (default; BASELINE.json north_star): a photon is absorbed with probability c1 / k_hat at a
+ * tentative collision and (1 - albedo) at the surface, and ends in exactly one bin with RT_W0 quanta.
+ * RT_MODE_WEIGHTED (the paper's scheme): the photon carries an integer weight w (RT_W0
+ * at launch); every tentative collision deposits floor(w pq / 2^24) quanta in atm_abs[voxel], pq =
+ * floor(c1 / k_hat 2^24), and continues with the rest; a surface arrival adds w to sfc_dir/sfc_dif, the
+ * albedo splits it into sfc_abs and the reflected weight; a photon leaving through the top adds w to toa_up;
+ * below RT_W0 / 2 the photon survives with probability w / RT_W0 and weight RT_W0, else it ends (fate 5).
+ * Closure: sum(atm_abs) + sum(sfc_abs) + sum(toa_up) + capped_energy + roulette_lost - roulette_gained ==
+ * n_photons * RT_W0 exactly.  Tallies of both modes may be accumulated in one context.  Errors: RT_EINVAL. */
+#define RT_MODE_ANALOG 0
+#define RT_MODE_WEIGHTED 1
+int rt_set_mode(rt_ctx* ctx, int mode);
 
 /* Zero tallies and counters on `cuda_stream`. */
 int rt_reset_tallies(rt_ctx* ctx, void* cuda_stream);

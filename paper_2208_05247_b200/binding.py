@@ -9,14 +9,17 @@ import torch
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "librt_b200.so")
 W0 = 1 << 32
-FATE_ATM_ABS, FATE_SFC_ABS, FATE_TOD_EXIT, FATE_CAPPED = 1, 2, 3, 4
+FATE_ATM_ABS, FATE_SFC_ABS, FATE_TOD_EXIT, FATE_CAPPED, FATE_ROULETTE = 1, 2, 3, 4, 5
+MODE_ANALOG, MODE_WEIGHTED = 0, 1
 
-EXPORTS = ("rt_create_grid", "rt_set_merge", "rt_set_optics", "rt_trace", "rt_trace_records", "rt_read_tallies",
+EXPORTS = ("rt_create_grid", "rt_set_merge", "rt_set_mode", "rt_set_optics", "rt_trace", "rt_trace_records", "rt_read_tallies",
            "rt_reset_tallies", "rt_read_majorant", "rt_read_packed_optics", "rt_gather_bench",
            "rt_last_trace_ms", "rt_launch_count", "rt_philox_words", "rt_last_error", "rt_destroy")
 
 COUNTER_FIELDS = ("n_photons", "n_events", "n_null", "n_rayleigh", "n_hg", "n_atm_abs", "n_sfc_hits",
-                  "n_sfc_abs", "n_toa", "n_capped", "n_cell_steps", "n_relevel", "capped_energy")
+                  "n_sfc_abs", "n_toa", "n_capped", "n_cell_steps", "n_relevel", "n_roulette_killed", "n_roulette_kept",
+                  "capped_energy", "roulette_lost", "roulette_gained")
+N_SIGNED = 3
 
 
 class RtError(RuntimeError):
@@ -24,7 +27,7 @@ class RtError(RuntimeError):
 
 
 class rt_counters(C.Structure):
-    _fields_ = [(n, C.c_uint64) for n in COUNTER_FIELDS[:-1]] + [("capped_energy", C.c_int64)]
+    _fields_ = [(n, C.c_uint64) for n in COUNTER_FIELDS[:-N_SIGNED]] + [(n, C.c_int64) for n in COUNTER_FIELDS[-N_SIGNED:]]
 
     def asdict(self):
         return {n: int(getattr(self, n)) for n in COUNTER_FIELDS}
@@ -45,6 +48,7 @@ def lib():
     vp, i32, u32, u64, f32, f64 = C.c_void_p, C.c_int, C.c_uint32, C.c_uint64, C.c_float, C.c_double
     L.rt_create_grid.argtypes = [C.POINTER(vp), i32, i32, i32, f32, f32, f32, i32, i32, i32, i32]
     L.rt_set_merge.argtypes = [vp, i32, i32, i32, f32]
+    L.rt_set_mode.argtypes = [vp, i32]
     L.rt_set_optics.argtypes = [vp, vp, vp, vp, vp, vp, vp]
     L.rt_trace.argtypes = [vp, f64, f64, u64, u64, u64, u32, vp]
     L.rt_trace_records.argtypes = [vp, f64, f64, u64, u64, u64, u32, vp, vp]
@@ -85,7 +89,8 @@ class Tallies:
 
     def closure(self):
         return (int(self.atm_abs.sum()) + int(self.sfc_abs.sum()) + int(self.toa_up.sum())
-                + int(self.counters.capped_energy))
+                + int(self.counters.capped_energy) + int(self.counters.roulette_lost)
+                - int(self.counters.roulette_gained))
 
 
 class Grid:
@@ -127,6 +132,10 @@ class Grid:
         if t.numel() != n:
             raise RtError("field has %d elements, expected %d" % (t.numel(), n))
         return t
+
+    def set_mode(self, weighted):
+        """Absorption scheme of the following traces: analog (False) or the paper's weights + roulette (True)."""
+        self._check(self.L.rt_set_mode(self.ctx, MODE_WEIGHTED if weighted else MODE_ANALOG), "rt_set_mode")
 
     def set_optics(self, k_ext, k_ext_cloud, ssa, g, sfc_albedo):
         nz, ny, nx = self.shape

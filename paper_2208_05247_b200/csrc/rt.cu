@@ -16,6 +16,7 @@ struct rt_ctx {
   float dx = 0, dy = 0, dz = 0;
   int mx = 1, my = 1, mz = 1;             // merged-cell factors (rt_set_merge)
   float merge_ratio = 1.25f;
+  int weighted = 0;                       // rt_set_mode: 0 analog absorption, 1 weights + roulette
   float* kmin = nullptr;                  // per-cell minimum extinction; allocated when merging is on
   size_t nvox = 0, ncol = 0, ncell = 0;
   float4* optics = nullptr;
@@ -28,7 +29,8 @@ struct rt_ctx {
   float* stage = nullptr;                 // 4 nvox + ncol floats; only allocated when a caller passes host fields
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   bool have_optics = false, have_trace = false;
-  int trace_blocks = 0, trace_blocks_rec = 0, sm_count = 0;
+  int trace_blocks[2][2] = {{0, 0}, {0, 0}};   // persistent grid size, [records][weighted]
+  int sm_count = 0;
   uint64_t launches = 0;
   std::string err;
 };
@@ -111,7 +113,7 @@ int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photon
   {
     // ids per work-counter atomic: 128, or fewer (a multiple of 32) when the launch has under ~8 chunks per warp,
     // so that short launches (one spectral point of config 4) balance over all resident warps
-    const unsigned long long warps = (unsigned long long)(records ? c->trace_blocks_rec : c->trace_blocks) * (rt::kTraceThreads / 32);
+    const unsigned long long warps = (unsigned long long)c->trace_blocks[records ? 1 : 0][c->weighted] * (rt::kTraceThreads / 32);
     unsigned long long ch = n_photons / (warps * 8ull);
     ch = (ch / 32ull) * 32ull;
     A.chunk = (unsigned)(ch < 32ull ? 32ull : (ch > (unsigned long long)rt::kChunk ? (unsigned long long)rt::kChunk : ch));
@@ -121,13 +123,16 @@ int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photon
   RT_CUDA(c, cudaEventRecord(c->ev0, st));
   if (n_photons > 0) {
     const bool pow2 = !(c->ncx & (c->ncx - 1)) && !(c->ncy & (c->ncy - 1));
-    if (records) {
-      if (pow2) rt::trace_kernel<true, true><<<c->trace_blocks_rec, rt::kTraceThreads, 0, st>>>(A);
-      else      rt::trace_kernel<true, false><<<c->trace_blocks_rec, rt::kTraceThreads, 0, st>>>(A);
+    const int blocks = c->trace_blocks[records ? 1 : 0][c->weighted];
+#define RT_LAUNCH(R, P, W) rt::trace_kernel<R, P, W><<<blocks, rt::kTraceThreads, 0, st>>>(A)
+    if (c->weighted) {
+      if (records) { if (pow2) RT_LAUNCH(true, true, true); else RT_LAUNCH(true, false, true); }
+      else         { if (pow2) RT_LAUNCH(false, true, true); else RT_LAUNCH(false, false, true); }
     } else {
-      if (pow2) rt::trace_kernel<false, true><<<c->trace_blocks, rt::kTraceThreads, 0, st>>>(A);
-      else      rt::trace_kernel<false, false><<<c->trace_blocks, rt::kTraceThreads, 0, st>>>(A);
+      if (records) { if (pow2) RT_LAUNCH(true, true, false); else RT_LAUNCH(true, false, false); }
+      else         { if (pow2) RT_LAUNCH(false, true, false); else RT_LAUNCH(false, false, false); }
     }
+#undef RT_LAUNCH
     ++c->launches;
   }
   RT_CUDA(c, cudaEventRecord(c->ev1, st));
@@ -171,17 +176,29 @@ int rt_create_grid(rt_ctx** out, int nx, int ny, int nz, float dx, float dy, flo
   RT_CUDA(c, cudaEventCreate(&c->ev0));
   RT_CUDA(c, cudaEventCreate(&c->ev1));
   RT_CUDA(c, cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, cuda_device));
-  int per_sm = 0;
-  // persistent grid: resident blocks per SM (the smaller of the two wrap variants) x SM count
-  int per_sm2 = 0;
-  RT_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rt::trace_kernel<false, false>, rt::kTraceThreads, 0));
-  RT_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm2, rt::trace_kernel<false, true>, rt::kTraceThreads, 0));
-  per_sm = per_sm < per_sm2 ? per_sm : per_sm2;
-  c->trace_blocks = c->sm_count * (per_sm > 0 ? per_sm : 1);
-  RT_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rt::trace_kernel<true, false>, rt::kTraceThreads, 0));
-  RT_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm2, rt::trace_kernel<true, true>, rt::kTraceThreads, 0));
-  per_sm = per_sm < per_sm2 ? per_sm : per_sm2;
-  c->trace_blocks_rec = c->sm_count * (per_sm > 0 ? per_sm : 1);
+  // persistent grid: resident blocks per SM (the smallest over the wrap and absorption-mode variants) x SM count
+  auto occupancy = [&](int* out, auto... kernels) {
+    int best = 1 << 30;
+    cudaError_t err = cudaSuccess;
+    auto one = [&](auto k) {
+      int v = 0;
+      cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, k, rt::kTraceThreads, 0);
+      if (e != cudaSuccess) err = e;
+      if (v < best) best = v;
+    };
+    (one(kernels), ...);
+    *out = best > 0 && best < (1 << 30) ? best : 1;
+    return err;
+  };
+  int per_sm = 1;
+  RT_CUDA(c, occupancy(&per_sm, rt::trace_kernel<false, false, false>, rt::trace_kernel<false, true, false>));
+  c->trace_blocks[0][0] = c->sm_count * per_sm;
+  RT_CUDA(c, occupancy(&per_sm, rt::trace_kernel<false, false, true>, rt::trace_kernel<false, true, true>));
+  c->trace_blocks[0][1] = c->sm_count * per_sm;
+  RT_CUDA(c, occupancy(&per_sm, rt::trace_kernel<true, false, false>, rt::trace_kernel<true, true, false>));
+  c->trace_blocks[1][0] = c->sm_count * per_sm;
+  RT_CUDA(c, occupancy(&per_sm, rt::trace_kernel<true, false, true>, rt::trace_kernel<true, true, true>));
+  c->trace_blocks[1][1] = c->sm_count * per_sm;
   return RT_OK;
 }
 
@@ -258,9 +275,12 @@ int rt_read_tallies(rt_ctx* c, int64_t* atm_abs, int64_t* sfc_dir, int64_t* sfc_
     counters->n_null = h[rt::C_NULL]; counters->n_rayleigh = h[rt::C_RAY]; counters->n_hg = h[rt::C_HG];
     counters->n_atm_abs = h[rt::C_ATM_ABS]; counters->n_sfc_hits = h[rt::C_SFC_HITS];
     counters->n_sfc_abs = h[rt::C_SFC_ABS]; counters->n_toa = h[rt::C_TOA]; counters->n_capped = h[rt::C_CAPPED];
-    counters->n_cell_steps = h[rt::C_CELLS]; counters->n_relevel = h[rt::C_RELEVEL]; counters->capped_energy = (int64_t)h[rt::C_CAPPED_E];
+    counters->n_cell_steps = h[rt::C_CELLS]; counters->n_relevel = h[rt::C_RELEVEL];
+    counters->n_roulette_killed = h[rt::C_ROUL_KILLED]; counters->n_roulette_kept = h[rt::C_ROUL_KEPT];
+    counters->roulette_lost = (int64_t)h[rt::C_ROUL_LOST]; counters->roulette_gained = (int64_t)h[rt::C_ROUL_GAINED];
+    counters->capped_energy = (int64_t)h[rt::C_CAPPED_E];
     counters->n_events = h[rt::C_NULL] + h[rt::C_RAY] + h[rt::C_HG] + h[rt::C_ATM_ABS];
-    counters->n_photons = h[rt::C_ATM_ABS] + h[rt::C_SFC_ABS] + h[rt::C_TOA] + h[rt::C_CAPPED];
+    counters->n_photons = h[rt::C_ATM_ABS] + h[rt::C_SFC_ABS] + h[rt::C_TOA] + h[rt::C_CAPPED] + h[rt::C_ROUL_KILLED];
   }
   return RT_OK;
 }
@@ -273,6 +293,13 @@ int rt_set_merge(rt_ctx* c, int mx, int my, int mz, float merge_ratio) {
   if (!(merge_ratio >= 1.0f) || !std::isfinite(merge_ratio)) return fail(c, RT_EINVAL, "rt_set_merge: merge_ratio must be >= 1");
   c->mx = mx; c->my = my; c->mz = mz; c->merge_ratio = merge_ratio;
   c->have_optics = false;                 // the majorant table is rebuilt by the next rt_set_optics
+  return RT_OK;
+}
+
+int rt_set_mode(rt_ctx* c, int mode) {
+  if (!c) return RT_EINVAL;
+  if (mode != RT_MODE_ANALOG && mode != RT_MODE_WEIGHTED) return fail(c, RT_EINVAL, "rt_set_mode: unknown mode");
+  c->weighted = (mode == RT_MODE_WEIGHTED);
   return RT_OK;
 }
 

@@ -58,7 +58,7 @@ constexpr int kMoveSteps = RT_MOVE_STEPS;         // MOVE steps between two vote
 constexpr int kMoveMin = RT_MOVE_MIN;             // ... cut short when fewer lanes than this still move (0: never)
 
 enum Counter { C_NULL = 0, C_RAY, C_HG, C_ATM_ABS, C_SFC_HITS, C_SFC_ABS, C_TOA, C_CAPPED, C_CELLS,
-               C_CAPPED_E, C_RELEVEL, C_COUNT };
+               C_CAPPED_E, C_RELEVEL, C_ROUL_KILLED, C_ROUL_KEPT, C_ROUL_LOST, C_ROUL_GAINED, C_COUNT };
 
 enum : uint32_t { ST_DEAD = 0, ST_MOVE = 1, ST_COLLIDE = 2, ST_SCATTER = 3, ST_BOUNDARY = 4 };
 
@@ -101,7 +101,9 @@ __device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
 
 
 // kPow2: the acceleration grid's x and y extents are powers of two, so the periodic wrap is a mask.
-template <bool kRecords, bool kPow2>
+// kWeighted: the paper's absorption weights + Russian roulette instead of analog
+// absorption: integer weight wq (tally quanta), deposits at every tentative collision, roulette ledger.
+template <bool kRecords, bool kPow2, bool kWeighted>
 __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(const TraceArgs A) {
   __shared__ unsigned long long s_cnt[C_COUNT];
   if (threadIdx.x < C_COUNT) s_cnt[threadIdx.x] = 0ull;
@@ -131,6 +133,9 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
                                           // cell), top byte: axis of the crossing that asked for a change of level
   // event counts: running totals of this thread; a photon's own counts are differences (records)
   uint32_t t_ev = 0, t_sc = 0, t_hg = 0, t_sfc = 0, t_cells = 0, t_relevel = 0;
+  unsigned long long wq = kW0;            // weighted mode: the photon's weight in tally quanta
+  unsigned long long t_rlost = 0, t_rgain = 0;   // roulette ledger of this thread
+  uint32_t t_rkept = 0;
   uint32_t b_ev = 0, b_sc = 0, b_sfc = 0;  // totals when the current photon was launched (records only)
 
   auto draw = [&]() {
@@ -161,8 +166,25 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
     rz = ((vc > 0.0f ? Lz : 0.0f) - qz) * ic;
   };
   auto cell_of = [&]() { return ((unsigned)cz * (unsigned)A.ncy + (unsigned)cy) * (unsigned)A.ncx + (unsigned)cx; };
+  // §3.14 roulette: below W0/2 survive with probability wq / W0 exactly (32-bit word of the Philox block at
+  // counter e | 2^31 against wq) and continue with W0, else end; both branches go to the ledger
+  int fate = 0;
+  uint32_t term = 0;
+  auto roulette = [&](uint32_t where) {
+    if (wq >= kW0 / 2) return false;
+    const unsigned long long pid = A.first_id + i;
+    const uint4 Y = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), e | 0x80000000u, A.stream_id, A.keys);
+    if ((unsigned long long)Y.w < wq) { t_rgain += kW0 - wq; ++t_rkept; wq = kW0; return false; }
+    t_rlost += wq; fate = 5; term = where;
+    return true;
+  };
   auto flush_thread_counters = [&]() {
     unsigned long long v;
+    if (kWeighted) {
+      if (t_rlost) atomicAdd(&s_cnt[C_ROUL_LOST], t_rlost);
+      if (t_rgain) atomicAdd(&s_cnt[C_ROUL_GAINED], t_rgain);
+      v = warp_sum(t_rkept);    if (lane == 0 && v) atomicAdd(&s_cnt[C_ROUL_KEPT], v);
+    }
     v = warp_sum(t_sc - t_hg);  if (lane == 0 && v) atomicAdd(&s_cnt[C_RAY], v);
     v = warp_sum(t_hg);         if (lane == 0 && v) atomicAdd(&s_cnt[C_HG], v);
     v = warp_sum(t_sfc);        if (lane == 0 && v) atomicAdd(&s_cnt[C_SFC_HITS], v);
@@ -211,6 +233,7 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
         flush_thread_counters();                   // keep the 32-bit running totals far from overflow
         if (kRecords) { b_ev -= t_ev; b_sc -= t_sc; b_sfc -= t_sfc; }
         t_ev = t_sc = t_hg = t_sfc = t_cells = t_relevel = 0;
+        t_rlost = t_rgain = 0; t_rkept = 0;
       }
       if (got) {
         // ---- §3.6 launch, event index 0 ------------------------------------------------------
@@ -244,6 +267,7 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
         ry = ((A.sun_iy > 0.0f ? Ly : 0.0f) - ((float)(iy % wy) + u24(X.y)) * A.dy) * A.sun_iy;
         rz = ((A.sun_iz > 0.0f ? Lz : 0.0f) - Lz) * A.sun_iz;
         direct = true;
+        wq = kW0;
         e = 1;
         if (kRecords) { b_ev = t_ev; b_sc = t_sc; b_sfc = t_sfc; }
         draw();
@@ -328,15 +352,16 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
       continue;
     }
 
-    int fate = 0;
-    uint32_t term = 0;
+    fate = 0;
+    term = 0;
     unsigned long long* tally_a = nullptr;  // arrival / terminal bin
     unsigned long long* tally_b = nullptr;  // surface absorption after an arrival tally
     if (phase == ST_COLLIDE) {
       // ---- COLLIDE: fetch the voxel, classify, draw the next event (§3.8) --------------------------
       if (st == ST_COLLIDE) {
         const bool lev = __float_as_int(kh) < 0;
-        const float s = tau * (1.0f / fabsf(kh));
+        const float rk = 1.0f / fabsf(kh);
+        const float s = tau * rk;
         rx = fmaxf(0.0f, rx - s); ry = fmaxf(0.0f, ry - s); rz = fmaxf(0.0f, rz - s);
         const float qx = local(da, rx, lev ? A.Lx1 : A.Lx), qy = local(db, ry, lev ? A.Ly1 : A.Ly),
                     qz = local(dc, rz, lev ? A.Lz1 : A.Lz);
@@ -348,23 +373,37 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
                              + (unsigned)(cx * A.bx + lx);
         const float4 v = __ldg(&A.optics[vox]);
         ++t_ev;
-        const float xi = u1 * fabsf(kh);
+        float xi = u1 * fabsf(kh);
         st = ST_MOVE;
-        if (xi < v.x) {                             // absorbed by the gas / droplet
+        if (kWeighted) {
+          // §3.14: deposit wq * P(absorbed), P = c1 / k_hat as a 24-bit fixed-point number; the rest goes on
+          const float f = v.x * rk;
+          const unsigned long long pq = min(1u << 24, (unsigned)(f * 16777216.0f));
+          const unsigned long long a = (wq * pq) >> 24;
+          if (a) atomicAdd(A.atm_abs + vox, a);
+          wq -= a;
+          if (wq == 0) { fate = 1; term = (uint32_t)vox; }
+          xi = fmaf(u1, fabsf(kh) - v.x, v.x);      // what happens instead: uniform on [c1, k_hat)
+        } else if (xi < v.x) {                      // absorbed by the gas / droplet
           tally_a = A.atm_abs + vox;
           fate = 1; term = (uint32_t)vox;
-        } else {
+        }
+        if (fate == 0) {
           if (xi < v.z) {                           // real scattering: angle and rotation in SCATTER
             st = ST_SCATTER;
             sg = (xi < v.y) ? v.w : 2.0f;
             sw2 = w2; sw3 = w3;
           }
-          ++e;
-          if (e > kEventCap) {                      // §3.12 (the capped event itself is still counted)
-            if (st == ST_SCATTER) { ++t_sc; if (sg < 1.5f) ++t_hg; }
-            fate = 4; term = 0;
+          if (kWeighted && roulette((uint32_t)vox)) {
+            if (st == ST_SCATTER) { ++t_sc; if (sg < 1.5f) ++t_hg; }   // the event itself is still counted
           } else {
-            draw();
+            ++e;
+            if (e > kEventCap) {                    // §3.12 (the capped event itself is still counted)
+              if (st == ST_SCATTER) { ++t_sc; if (sg < 1.5f) ++t_hg; }
+              fate = 4; term = 0;
+            } else {
+              draw();
+            }
           }
         }
       }
@@ -408,12 +447,26 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
         const int hy = cy * A.by + min((int)(qy * A.rdy), (lev ? A.my * A.by : A.by) - 1);
         const unsigned col = (unsigned)hy * (unsigned)A.nx + (unsigned)hx;
         if (cz >= 0) {                              // left through the domain top
-          tally_a = A.toa_up + col;
+          if (kWeighted) atomicAdd(A.toa_up + col, wq); else tally_a = A.toa_up + col;
           fate = 3; term = (uint32_t)col;
         } else {                                    // Lambertian surface
           ++t_sfc;
-          tally_a = (direct ? A.sfc_dir : A.sfc_dif) + col;
-          if (u1 < __ldg(&A.albedo[col])) {
+          bool reflect;
+          if (kWeighted) {
+            // §3.14: arrival tallied with the weight; the albedo reduces the weight, 24-bit fixed point
+            atomicAdd((direct ? A.sfc_dir : A.sfc_dif) + col, wq);
+            const unsigned long long aq = min(1u << 24, (unsigned)(__ldg(&A.albedo[col]) * 16777216.0f));
+            const unsigned long long refl = (wq * aq) >> 24;
+            if (wq - refl) atomicAdd(A.sfc_abs + col, wq - refl);
+            wq = refl;
+            if (wq == 0) { fate = 2; term = (uint32_t)col; reflect = false; }
+            else reflect = !roulette((uint32_t)col);
+          } else {
+            tally_a = (direct ? A.sfc_dir : A.sfc_dif) + col;
+            reflect = u1 < __ldg(&A.albedo[col]);
+            if (!reflect) { tally_b = A.sfc_abs + col; fate = 2; term = (uint32_t)col; }
+          }
+          if (reflect) {
             const float u2 = u24(w2);
             const float mu = sqrtf(1.0f - u2), sn = sqrtf(u2);
             float sp, cp;
@@ -427,9 +480,6 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
               draw();
               st = ST_MOVE;
             }
-          } else {
-            tally_b = A.sfc_abs + col;
-            fate = 2; term = (uint32_t)col;
           }
         }
       }
@@ -447,13 +497,18 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
       // photons finished: count their fates per warp, write their records
       const unsigned f1 = __ballot_sync(0xffffffffu, fate == 1), f2 = __ballot_sync(0xffffffffu, fate == 2);
       const unsigned f3 = __ballot_sync(0xffffffffu, fate == 3), f4 = __ballot_sync(0xffffffffu, fate == 4);
+      if (kWeighted) {
+        const unsigned f5 = __ballot_sync(0xffffffffu, fate == 5);
+        if (lane == 0 && f5) atomicAdd(&s_cnt[C_ROUL_KILLED], (unsigned long long)__popc(f5));
+        if (fate == 4) atomicAdd(&s_cnt[C_CAPPED_E], wq);
+      }
       if (lane == 0) {
         if (f1) atomicAdd(&s_cnt[C_ATM_ABS], (unsigned long long)__popc(f1));
         if (f2) atomicAdd(&s_cnt[C_SFC_ABS], (unsigned long long)__popc(f2));
         if (f3) atomicAdd(&s_cnt[C_TOA], (unsigned long long)__popc(f3));
         if (f4) {
           atomicAdd(&s_cnt[C_CAPPED], (unsigned long long)__popc(f4));
-          atomicAdd(&s_cnt[C_CAPPED_E], kW0 * (unsigned long long)__popc(f4));
+          if (!kWeighted) atomicAdd(&s_cnt[C_CAPPED_E], kW0 * (unsigned long long)__popc(f4));
         }
       }
       if (kRecords && fate != 0) {

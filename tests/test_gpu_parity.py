@@ -271,3 +271,53 @@ def test_bad_inputs_fail_loudly():
     with pytest.raises(rt.RtError):
         g.trace(95.0, 0.0, 16)
     g.close()
+
+
+def _compare_weighted(cfg, opt, n, zen=None, azi=None):
+    """Weighted mode against the oracle in kernel precision: records, every tally quantum,
+    every counter including the roulette ledger; exact closure with the ledger."""
+    rt = _rt()
+    zen = cfg.zenith_deg if zen is None else zen
+    azi = cfg.azimuth_deg if azi is None else azi
+    g = rt.Grid(*cfg.grid, device=0, **cfg.accel)
+    g.set_mode(weighted=True)
+    g.set_optics(opt["k_ext"], opt["k_ext_cloud"], opt["ssa"], opt["g"], opt["sfc_albedo"])
+    rec = g.trace(zen, azi, n, seed=cfg.seed, records=True).cpu().numpy().view(np.uint32)
+    t = g.read_tallies()
+    g.close()
+    o32, rec32, _ = O.trace(cfg.grid, opt, zen, azi, n, seed=cfg.seed, precision=32, records=True, n_threads=8,
+                            weighted=True, **cfg.accel)
+    assert t.closure() == n * rt.W0 and o32.closure() == n * rt.W0
+    assert np.array_equal(rec, rec32)
+    for name in ("atm_abs", "sfc_dir", "sfc_dif", "sfc_abs", "toa_up"):
+        assert np.array_equal(getattr(t, name).numpy(), getattr(o32, name)), name
+    assert t.counters.asdict() == o32.counters.asdict()
+    assert t.counters.n_roulette_killed > 0 and t.counters.n_roulette_kept > 0
+    return t
+
+
+def test_weighted_mode_config1_and_config2():
+    from dataclasses import replace
+    cfg = CONFIGS[1]
+    _compare_weighted(cfg, make_optics(cfg), cfg.n_photons)
+    cfg = replace(CONFIGS[2], block=(2, 2, 2), merge=(8, 8, 4))
+    t = _compare_weighted(cfg, make_optics(cfg), (1 << 20) + 13)
+    assert t.counters.n_relevel > 0
+
+
+def test_weighted_mode_config3_sample_and_mixed_accumulation():
+    """Config 3 in the bench launch configuration, weighted; then an analog and a weighted launch accumulated in
+    one context: the closure identity covers both."""
+    rt = _rt()
+    cfg = CONFIGS[3]
+    opt = make_optics(cfg)
+    _compare_weighted(cfg, opt, 1 << 19)
+    g = rt.Grid(*cfg.grid, device=0, **cfg.accel)
+    g.set_optics(opt["k_ext"], opt["k_ext_cloud"], opt["ssa"], opt["g"], opt["sfc_albedo"])
+    n = 1 << 22
+    g.trace(cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed)
+    g.set_mode(weighted=True)
+    g.trace(cfg.zenith_deg, cfg.azimuth_deg, n, first_photon_id=n, seed=cfg.seed)
+    t = g.read_tallies()
+    g.close()
+    assert t.closure() == 2 * n * rt.W0 and t.counters.n_photons == 2 * n and t.counters.n_capped == 0
