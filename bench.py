@@ -111,7 +111,7 @@ def run_reference(args):
     times, events = [], 0
     for step in range(args.warmup + args.steps):
         t, _, el = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, first_photon_id=step * n,
-                           seed=cfg.seed, precision=64, n_threads=cores, **cfg.accel)
+                           seed=cfg.seed, precision=64, n_threads=cores, weighted=(args.mode == "weighted"), **cfg.accel)
         assert t.closure() == n * O.W0
         if step >= args.warmup:
             times.append(el)
@@ -182,6 +182,7 @@ def run_ours(args):
     host = [torch.from_numpy(opt[k]).pin_memory() for k in names] if not spectral else None
     n = cfg.n_photons                            # per GPU (weak scaling: photon ids are sharded by rank)
     g = rt.Grid(*cfg.grid, device=local, **cfg.accel)
+    g.set_mode(weighted=(args.mode == "weighted"))
     pinned_cols = rt.Tallies(None, *[torch.empty((cfg.ny, cfg.nx), dtype=torch.int64).pin_memory() for _ in range(4)],
                              counters=None)
     if spectral:
@@ -248,7 +249,12 @@ def run_ours(args):
     elapsed_ms = max_over_ranks(e0.elapsed_time(e1))
     launches = g.launch_count() - launches0
     clocks = sampler.stop() if sampler else None
-    closure_ok = (int(t.sfc_abs.sum()) + int(t.toa_up.sum()) + t.counters.n_atm_abs * rt.W0 == n * rt.W0)
+    closure_ok = (args.mode == "analog" and
+                  int(t.sfc_abs.sum()) + int(t.toa_up.sum()) + t.counters.n_atm_abs * rt.W0 == n * rt.W0)
+    if args.mode == "weighted":     # atm_abs stays on the device in this leg: sum it there
+        ta = g.read_tallies(host=False)
+        closure_ok = ta.closure() == n * rt.W0
+        del ta
 
     total_photons = n * world * args.steps
     total_events = sum_over_ranks(events)
@@ -312,7 +318,7 @@ def run_ours(args):
         import oracle as O
         cores = O.hardware_threads()
         ot, _, el = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, CPU_BASELINE_PHOTONS, seed=cfg.seed,
-                            precision=64, n_threads=cores, **cfg.accel)
+                            precision=64, n_threads=cores, weighted=(args.mode == "weighted"), **cfg.accel)
         cpu = {"value": CPU_BASELINE_PHOTONS / el, "unit": UNIT, "cores": cores, "kind": "oracle",
                "collision_events_per_s": ot.counters.n_events / el,
                "sample": "photon ids [0, %d) (%d per column) of the %d-photon workload, photon loop only" % (
@@ -327,6 +333,7 @@ def run_ours(args):
         "trace_kernel": {"ms": ms_avg, "paths_per_s": n / (ms_avg * 1e-3), "events_per_s": trace_events_per_s},
         "config": {"workload": cfg.name, "grid": [cfg.nx, cfg.ny, cfg.nz], "photons_per_gpu_per_step": n,
                    "block": list(cfg.block), "merge": list(cfg.merge), "merge_ratio": cfg.merge_ratio,
+                   "mode": args.mode,
                    "zenith_deg": cfg.zenith_deg, "azimuth_deg": cfg.azimuth_deg,
                    "parallelism": "photon-id ranges per GPU, no collective" if world > 1 else "1 GPU",
                    "l2": ("inputs exceed L2 (%d MiB packed optics + %d MiB tallies vs 126 MB)" % (
@@ -371,6 +378,8 @@ def main():
     ap.add_argument("--workload", type=int, choices=(1, 2, 3, 4, 5), default=WORKLOAD,
                     help="BASELINE.json configs[N-1]; the default (3) is the configuration the metric is quoted on")
     ap.add_argument("--block", default=None, help="acceleration-grid block bx,by,bz (default: the config's)")
+    ap.add_argument("--mode", choices=("analog", "weighted"), default="analog",
+                    help="absorption scheme: analog (the metric's, default) or the paper's weights + roulette")
     ap.add_argument("--merge", default=None, help="merged-cell factors mx,my,mz (default: the config's; 1,1,1 = off)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing (used under ncu)")
     args = ap.parse_args()
