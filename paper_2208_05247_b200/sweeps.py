@@ -23,6 +23,45 @@ def spectral_sweep(grid, fields_of_point, counts, zenith_deg, azimuth_deg, seed=
     return total
 
 
+def spectral_sweep_overlapped(grids, streams, fields_of_point, counts, zenith_deg, azimuth_deg, seed=1,
+                              first_photon_id=0):
+    """The same sweep over several contexts of the same grid (normally two), point j going to context j mod
+    len(grids) on that context's own stream: while the persistent trace kernel of one point drains (a point
+    of config 4 is only ~6e5 photons, so its tail is a large part of its launch), the next point's pack and
+    trace already fill the freed SMs.  Each context accumulates its own tallies; their sum (exact, int64) is
+    the sweep's result: `sum_tallies`.  The streams wait for the caller's current stream first."""
+    ready = torch.cuda.Event()
+    ready.record()
+    for st in streams:
+        st.wait_event(ready)
+    total = 0
+    k = 0
+    for j, n in enumerate(counts):
+        if n == 0:
+            continue
+        g, st = grids[k % len(grids)], streams[k % len(grids)]
+        k += 1
+        with torch.cuda.stream(st):
+            g.set_optics(*fields_of_point(j))
+            g.trace(zenith_deg, azimuth_deg, n, first_photon_id=first_photon_id, seed=seed, stream_id=j)
+        total += n
+    for st in streams:
+        torch.cuda.current_stream().wait_stream(st)
+    return total
+
+
+def sum_tallies(grids, host=False):
+    """Sum of the contexts' tallies and counters (integers: exact and order-independent)."""
+    from .binding import Tallies, rt_counters
+    ts = [g.read_tallies(host=host) for g in grids]
+    cnt = rt_counters()
+    for name, _ in rt_counters._fields_:
+        setattr(cnt, name, sum(int(getattr(t.counters, name)) for t in ts))
+    fields = [sum(getattr(t, f) for t in ts[1:]) + getattr(ts[0], f) if len(ts) > 1 else getattr(ts[0], f)
+              for f in ("atm_abs", "sfc_dir", "sfc_dif", "sfc_abs", "toa_up")]
+    return Tallies(*fields, counters=cnt)
+
+
 def _block_sums(t, blk):
     """Sums over blocks of blk voxels/columns of an integer tensor whose shape is a multiple of blk."""
     shp = []

@@ -70,6 +70,21 @@ def test_config4_spectral_sweep():
     assert int(t.atm_abs.sum()) == c.n_atm_abs * rt.W0 and int(t.toa_up.sum()) == c.n_toa * rt.W0
     # a sweep in which many points absorb strongly: broadband absorption well above the single-point config 3
     assert 0.05 < c.n_atm_abs / total < 0.9
+
+    # the same sweep over two contexts on two streams (points alternate, launches overlap): the summed integer
+    # tallies and counters must equal the one-context sweep's exactly
+    from paper_2208_05247_b200.sweeps import spectral_sweep_overlapped, sum_tallies
+    g2 = rt.Grid(*cfg.grid, device=0, **cfg.accel)
+    g.reset_tallies()
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    total2 = spectral_sweep_overlapped([g, g2], streams, lambda j: [make_optics_torch(cfg, pts[j])[k] for k in NAMES],
+                                       counts, cfg.zenith_deg, cfg.azimuth_deg, seed=cfg.seed)
+    torch.cuda.synchronize()
+    t2 = sum_tallies([g, g2], host=True)
+    assert total2 == total and t2.counters.asdict() == c.asdict()
+    for name in TALLIES:
+        assert torch.equal(getattr(t2, name), getattr(t, name)), name
+    g2.close()
     g.close()
 
 
