@@ -3,6 +3,7 @@
 #include "../../include/rt.h"
 
 #include <cmath>
+#include <cstdint>
 #include <cstdio>
 #include <cstring>
 #include <string>
@@ -224,9 +225,15 @@ int rt_set_optics(rt_ctx* c, const float* k_ext, const float* k_ext_cloud, const
     if (!c->kmin) RT_CUDA(c, cudaMalloc(&c->kmin, c->ncell * sizeof(float)));
     RT_CUDA(c, cudaMemsetAsync(c->kmin, 0x7f, c->ncell * sizeof(float), st));   // 0x7f7f7f7f: above any finite input's bits that matter (3.4e38)
   }
-  rt::pack_optics_kernel<<<blocks, 256, 0, st>>>(k_ext, k_ext_cloud, ssa, g, c->optics, (int*)c->khat,
-                                                merging ? (int*)c->kmin : nullptr, c->nx,
-                                                c->ny, c->nz, c->bx, c->by, c->bz, c->bad);
+  const bool rows = (c->nx % 4 == 0) && !(((uintptr_t)k_ext | (uintptr_t)k_ext_cloud | (uintptr_t)ssa | (uintptr_t)g) & 15u);
+  if (rows)
+    rt::pack_optics_rows_kernel<<<c->sm_count * 16, 128, 0, st>>>(
+        (const float4*)k_ext, (const float4*)k_ext_cloud, (const float4*)ssa, (const float4*)g, c->optics,
+        (int*)c->khat, merging ? (int*)c->kmin : nullptr, c->nx, c->ny, c->nz, c->bx, c->by, c->bz, c->bad);
+  else
+    rt::pack_optics_kernel<<<blocks, 256, 0, st>>>(k_ext, k_ext_cloud, ssa, g, c->optics, (int*)c->khat,
+                                                  merging ? (int*)c->kmin : nullptr, c->nx,
+                                                  c->ny, c->nz, c->bx, c->by, c->bz, c->bad);
   rt::check_albedo_kernel<<<c->sm_count, 256, 0, st>>>(c->albedo, c->ncol, c->bad);
   c->launches += 2;
   if (merging) {
