@@ -37,7 +37,7 @@ def lib():
         _lib.orc_trace.restype = C.c_int
         _lib.orc_trace.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float,
                                    C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_float, C.c_int,
-                                   fp, fp, fp, fp, fp, C.c_double, C.c_double,
+                                   C.c_float, C.c_int, fp, fp, fp, fp, fp, C.c_double, C.c_double,
                                    C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint32, ip, ip, ip, ip, ip,
                                    C.POINTER(Counters), C.POINTER(C.c_uint32), C.c_int,
                                    C.POINTER(C.c_double)]
@@ -71,11 +71,12 @@ class Tallies:
 
 def trace(grid, optics, zenith_deg, azimuth_deg, n_photons, first_photon_id=0, seed=1, stream_id=0,
           precision=64, tallies=None, records=False, n_threads=1, merge=(1, 1, 1), merge_ratio=1.25,
-          weighted=False):
+          weighted=False, diffuse_fraction=0.0, sobol=False):
     """Run the oracle.  grid = (nx, ny, nz, dx, dy, dz, bx, by, bz); optics = dict with
     k_ext, k_ext_cloud, ssa, g ([nz][ny][nx] fp32) and sfc_albedo ([ny][nx] fp32); merge = merged-cell
     factors ((1, 1, 1) = single-level acceleration grid); weighted = the paper's absorption
-    weights + Russian roulette instead of analog absorption.
+    weights + Russian roulette instead of analog absorption; diffuse_fraction and
+    sobol = the paper's top-of-domain source.
     Returns (tallies, records or None, elapsed seconds of the photon loop)."""
     nx, ny, nz, dx, dy, dz, bx, by, bz = grid
     k, kp = _f32(optics["k_ext"])
@@ -89,7 +90,7 @@ def trace(grid, optics, zenith_deg, azimuth_deg, n_photons, first_photon_id=0, s
     ip = C.POINTER(C.c_int64)
     el = C.c_double(0.0)
     rc = lib().orc_trace(int(precision), nx, ny, nz, dx, dy, dz, bx, by, bz, int(merge[0]), int(merge[1]),
-                         int(merge[2]), float(merge_ratio), int(bool(weighted)), kp, kcp, wp, gp, alp,
+                         int(merge[2]), float(merge_ratio), int(bool(weighted)), float(diffuse_fraction), int(bool(sobol)), kp, kcp, wp, gp, alp,
                          float(zenith_deg), float(azimuth_deg), int(n_photons), int(first_photon_id),
                          int(seed), int(stream_id), t.atm_abs.ctypes.data_as(ip),
                          t.sfc_dir.ctypes.data_as(ip), t.sfc_dif.ctypes.data_as(ip),
@@ -170,6 +171,16 @@ def majorant(nx, ny, nz, bx, by, bz, k_ext, merge=(1, 1, 1), merge_ratio=1.25):
     lib().orc_majorant(nx, ny, nz, bx, by, bz, int(merge[0]), int(merge[1]), int(merge[2]),
                        C.c_float(merge_ratio), kp, out.ctypes.data_as(C.POINTER(C.c_float)))
     return out
+
+
+def sobol2(k):
+    """Points k of the 2-D Sobol sequence as two uint32 arrays of 32-bit fractions."""
+    k = np.ascontiguousarray(k, dtype=np.uint32)
+    x1 = np.empty_like(k)
+    x2 = np.empty_like(k)
+    up = C.POINTER(C.c_uint32)
+    lib().orc_sobol2(k.ctypes.data_as(up), x1.ctypes.data_as(up), x2.ctypes.data_as(up), C.c_uint64(k.size))
+    return x1, x2
 
 
 def hardware_threads():

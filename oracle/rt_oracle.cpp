@@ -224,6 +224,8 @@ struct Problem {
   int mx, my, mz;            // §3.5b: merged cells of mx x my x mz acceleration cells (1,1,1 = none)
   float merge_ratio;         // §3.5b: merged iff max c3 <= merge_ratio * min c3 over the merged cell's voxels
   int weighted;              // §3.14: 0 = analog absorption, 1 = the paper's weights + Russian roulette
+  float diffuse_fraction;    // §3.15: share of photons launched diffusely (isotropic downwelling radiance)
+  int sobol;                 // §3.15: entry points from a scrambled 2-D Sobol sequence instead of Philox
   float dx, dy, dz;
   const float *k_ext, *k_cloud, *ssa, *g, *albedo;
   double zenith_deg, azimuth_deg;
@@ -249,6 +251,17 @@ inline Vox<R> pack_voxel(float kf, float kcf, float wf, float gf) {
   v.c1 = std::min(v.c1, v.c2);
   v.g = (R)gf;
   return v;
+}
+
+// §3.15 point k of the 2-D Sobol sequence as 32-bit fractions: x1 = radical inverse of k in base 2,
+// x2 = XOR of the direction numbers V0 = 2^31, Vj = Vj-1 ^ (Vj-1 >> 1) over the set bits j of k.
+inline void sobol2(uint32_t k, uint32_t& x1, uint32_t& x2) {
+  x1 = 0; x2 = 0;
+  uint32_t V = 0x80000000u;
+  for (int j = 0; j < 32; ++j) {
+    if ((k >> j) & 1u) { x1 ^= 0x80000000u >> j; x2 ^= V; }
+    V ^= V >> 1;
+  }
 }
 
 template <class R>
@@ -291,6 +304,18 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
       ix = std::min((int)(u2 * (R)nx), nx - 1);
       iy = std::min((int)(u3 * (R)ny), ny - 1);
     }
+    if (P.sobol && i < n_full) {
+      // §3.15 ("initialized at the domain top following a scrambled Sobol sequence"): within its column
+      // the photon of pass k enters at point k of the 2-D Sobol sequence (radical inverse in base 2; second
+      // coordinate from the direction numbers V0 = 2^31, Vj = Vj-1 ^ (Vj-1 >> 1)), scrambled by a random
+      // digital shift (XOR) drawn per column, stream and call from Philox under the key (k0, k1 ^ 'SOBL')
+      const uint32_t k = (uint32_t)(i / ncol), col32 = (uint32_t)(i % ncol);
+      const U4 S = philox4x32_10(col32, P.stream_id, (uint32_t)P.first_id, (uint32_t)(P.first_id >> 32),
+                                 k0, k1 ^ 0x534F424Cu);
+      uint32_t x1, x2;
+      sobol2(k, x1, x2);
+      u0 = uni24<R>(x1 ^ S.x); u1 = uni24<R>(x2 ^ S.y);
+    }
     int c[3] = {ix / bx, iy / by, ncz - 1};    // acceleration-cell index (at level 1: the merged cell's origin)
     // §3.5b: the sign bit of the stored majorant says whether the cell belongs to a merged cell
     auto load = [&](R& kh_out) {
@@ -307,6 +332,20 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
     // magnitudes never grow and rounding does not accumulate along a path.  Local coordinates are
     // recovered when needed as q = face - v r.
     R d[3] = {sun_x, sun_y, sun_z};            // unit direction
+    bool direct = true;
+    if (P.diffuse_fraction > 0.0f) {
+      // §3.15 ("either along the sun beam or randomly generated, assuming isotropic downwelling diffuse
+      // radiation at the TOD"): words of the Philox block at counter (id, 0 | 2^31): 0 decides, 1 and 2 give a
+      // cosine-weighted downward direction (isotropic radiance: pdf(mu) = 2 mu)
+      const U4 D = philox4x32_10(p_lo, p_hi, 0x80000000u, P.stream_id, k0, k1);
+      if (uni24<R>(D.x) < (R)P.diffuse_fraction) {
+        const R v1 = uni24<R>(D.y);
+        const R mu = std::sqrt((R)1 - v1), sn = std::sqrt(v1);
+        R sp, cp; E::sincos_2pi(uni24<R>(D.z), sp, cp);
+        d[0] = sn * cp; d[1] = sn * sp; d[2] = -mu;
+        direct = false;
+      }
+    }
     R v[3], iv[3];                             // nudged components and reciprocals
     R del[2][3];                               // distance between successive faces, per level and axis
     R r[3];                                    // remaining distance to the next face on each axis
@@ -331,7 +370,6 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
                       ((R)(iy % ((lev ? P.my : 1) * by)) + u1) * dy, Lv[lev][2]};
       place(q);
     }
-    bool direct = true;
     uint32_t e = 1, n_ev = 0, n_sc = 0, n_sfc = 0;
     int fate = 0; uint32_t term = 0;
     // §3.14 weighted mode: integer weight in tally quanta, W0 at launch.  Roulette (Iwabuchi 2006
@@ -557,7 +595,8 @@ extern "C" {
 // Returns 0 on success, -1 on bad arguments.  Tallies and counters are ADDED to.
 // elapsed_s (may be NULL) receives the wall time of the photon loop only.
 int orc_trace(int precision, int nx, int ny, int nz, float dx, float dy, float dz, int bx, int by,
-              int bz, int mx, int my, int mz, float merge_ratio, int weighted, const float* k_ext, const float* k_ext_cloud, const float* ssa, const float* g,
+              int bz, int mx, int my, int mz, float merge_ratio, int weighted, float diffuse_fraction,
+              int sobol, const float* k_ext, const float* k_ext_cloud, const float* ssa, const float* g,
               const float* sfc_albedo, double zenith_deg, double azimuth_deg, uint64_t n_photons,
               uint64_t first_photon_id, uint64_t seed, uint32_t stream_id, int64_t* atm_abs,
               int64_t* sfc_dir, int64_t* sfc_dif, int64_t* sfc_abs, int64_t* toa_up,
@@ -567,7 +606,8 @@ int orc_trace(int precision, int nx, int ny, int nz, float dx, float dy, float d
   if (mx <= 0 || my <= 0 || mz <= 0 || (nx / bx) % mx || (ny / by) % my || (nz / bz) % mz) return -1;
   if (!(zenith_deg >= 0.0 && zenith_deg < 90.0)) return -1;
   if (precision != 32 && precision != 64) return -1;
-  Problem P{nx, ny, nz, bx, by, bz, mx, my, mz, merge_ratio, weighted ? 1 : 0, dx, dy, dz, k_ext, k_ext_cloud, ssa, g, sfc_albedo,
+  if (!(diffuse_fraction >= 0.0f && diffuse_fraction <= 1.0f)) return -1;
+  Problem P{nx, ny, nz, bx, by, bz, mx, my, mz, merge_ratio, weighted ? 1 : 0, diffuse_fraction, sobol ? 1 : 0, dx, dy, dz, k_ext, k_ext_cloud, ssa, g, sfc_albedo,
             zenith_deg, azimuth_deg, n_photons, first_photon_id, seed, stream_id,
             atm_abs, sfc_dir, sfc_dif, sfc_abs, toa_up, records};
   std::vector<float> khat = build_majorant(P);
@@ -643,6 +683,9 @@ void orc_majorant(int nx, int ny, int nz, int bx, int by, int bz, int mx, int my
   P.mx = mx; P.my = my; P.mz = mz; P.merge_ratio = merge_ratio;
   std::vector<float> kh = build_majorant(P);
   std::memcpy(out, kh.data(), kh.size() * sizeof(float));
+}
+void orc_sobol2(const uint32_t* k, uint32_t* x1, uint32_t* x2, uint64_t n) {
+  for (uint64_t i = 0; i < n; ++i) sobol2(k[i], x1[i], x2[i]);
 }
 int orc_hardware_threads() { return (int)std::thread::hardware_concurrency(); }
 
