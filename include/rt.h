@@ -121,6 +121,19 @@ int rt_set_merge(rt_ctx* ctx, int mx, int my, int mz, float merge_ratio);
 #define RT_MODE_WEIGHTED 1
 int rt_set_mode(rt_ctx* ctx, int mode);
 
+/* Top-of-domain source of the following rt_trace calls.  Default: every photon on the
+ * sun beam, sub-pixel entry point from Philox (BASELINE.json north_star).
+ * diffuse_fraction in [0, 1]: that share of the photons (decided per photon by a Philox word) starts diffuse:
+ * direction drawn for isotropic downwelling radiance (pdf(mu) = 2 mu), counted as diffuse light from the start
+ * ("the initial direction of each photon is either along the sun beam or randomly generated").
+ * sampler RT_SAMPLER_SOBOL: within its column the photon of pass k (k = index in the call / ncol) enters at
+ * point k of the 2-D Sobol sequence under a random digital shift per column, stream_id and first_photon_id
+ * ("initialized ... following a scrambled Sobol sequence"); photons of the remainder pass keep Philox.
+ * Errors: RT_EINVAL. */
+#define RT_SAMPLER_PHILOX 0
+#define RT_SAMPLER_SOBOL 1
+int rt_set_source(rt_ctx* ctx, float diffuse_fraction, int sampler);
+
 /* Zero tallies and counters on `cuda_stream`. */
 int rt_reset_tallies(rt_ctx* ctx, void* cuda_stream);
 

@@ -12,7 +12,7 @@ W0 = 1 << 32
 FATE_ATM_ABS, FATE_SFC_ABS, FATE_TOD_EXIT, FATE_CAPPED, FATE_ROULETTE = 1, 2, 3, 4, 5
 MODE_ANALOG, MODE_WEIGHTED = 0, 1
 
-EXPORTS = ("rt_create_grid", "rt_set_merge", "rt_set_mode", "rt_set_optics", "rt_trace", "rt_trace_records", "rt_read_tallies",
+EXPORTS = ("rt_create_grid", "rt_set_merge", "rt_set_mode", "rt_set_source", "rt_set_optics", "rt_trace", "rt_trace_records", "rt_read_tallies",
            "rt_reset_tallies", "rt_read_majorant", "rt_read_packed_optics", "rt_gather_bench",
            "rt_last_trace_ms", "rt_launch_count", "rt_philox_words", "rt_last_error", "rt_destroy")
 
@@ -49,6 +49,7 @@ def lib():
     L.rt_create_grid.argtypes = [C.POINTER(vp), i32, i32, i32, f32, f32, f32, i32, i32, i32, i32]
     L.rt_set_merge.argtypes = [vp, i32, i32, i32, f32]
     L.rt_set_mode.argtypes = [vp, i32]
+    L.rt_set_source.argtypes = [vp, f32, i32]
     L.rt_set_optics.argtypes = [vp, vp, vp, vp, vp, vp, vp]
     L.rt_trace.argtypes = [vp, f64, f64, u64, u64, u64, u32, vp]
     L.rt_trace_records.argtypes = [vp, f64, f64, u64, u64, u64, u32, vp, vp]
@@ -136,6 +137,10 @@ class Grid:
     def set_mode(self, weighted):
         """Absorption scheme of the following traces: analog (False) or the paper's weights + roulette (True)."""
         self._check(self.L.rt_set_mode(self.ctx, MODE_WEIGHTED if weighted else MODE_ANALOG), "rt_set_mode")
+
+    def set_source(self, diffuse_fraction=0.0, sobol=False):
+        """Top-of-domain source of the following traces (include/rt.h rt_set_source)."""
+        self._check(self.L.rt_set_source(self.ctx, float(diffuse_fraction), 1 if sobol else 0), "rt_set_source")
 
     def set_optics(self, k_ext, k_ext_cloud, ssa, g, sfc_albedo):
         nz, ny, nx = self.shape

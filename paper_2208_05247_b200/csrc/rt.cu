@@ -18,6 +18,8 @@ struct rt_ctx {
   int mx = 1, my = 1, mz = 1;             // merged-cell factors (rt_set_merge)
   float merge_ratio = 1.25f;
   int weighted = 0;                       // rt_set_mode: 0 analog absorption, 1 weights + roulette
+  float diffuse_fraction = 0.0f;          // rt_set_source
+  int sobol = 0;
   float* kmin = nullptr;                  // per-cell minimum extinction; allocated when merging is on
   size_t nvox = 0, ncol = 0, ncell = 0;
   float4* optics = nullptr;
@@ -120,6 +122,8 @@ int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photon
     A.chunk = (unsigned)(ch < 32ull ? 32ull : (ch > (unsigned long long)rt::kChunk ? (unsigned long long)rt::kChunk : ch));
   }
   A.keys = rt::philox_round_keys((uint32_t)seed, (uint32_t)(seed >> 32)); A.stream_id = stream_id;
+  A.keys_sobol = rt::philox_round_keys((uint32_t)seed, (uint32_t)(seed >> 32) ^ 0x534F424Cu);
+  A.diffuse_fraction = c->diffuse_fraction; A.sobol = c->sobol;
   RT_CUDA(c, cudaMemsetAsync(A.next_photon, 0, sizeof(unsigned long long), st));
   RT_CUDA(c, cudaEventRecord(c->ev0, st));
   if (n_photons > 0) {
@@ -300,6 +304,14 @@ int rt_set_merge(rt_ctx* c, int mx, int my, int mz, float merge_ratio) {
   if (!(merge_ratio >= 1.0f) || !std::isfinite(merge_ratio)) return fail(c, RT_EINVAL, "rt_set_merge: merge_ratio must be >= 1");
   c->mx = mx; c->my = my; c->mz = mz; c->merge_ratio = merge_ratio;
   c->have_optics = false;                 // the majorant table is rebuilt by the next rt_set_optics
+  return RT_OK;
+}
+
+int rt_set_source(rt_ctx* c, float diffuse_fraction, int sampler) {
+  if (!c) return RT_EINVAL;
+  if (!(diffuse_fraction >= 0.0f && diffuse_fraction <= 1.0f)) return fail(c, RT_EINVAL, "rt_set_source: diffuse_fraction must be in [0, 1]");
+  if (sampler != RT_SAMPLER_PHILOX && sampler != RT_SAMPLER_SOBOL) return fail(c, RT_EINVAL, "rt_set_source: unknown sampler");
+  c->diffuse_fraction = diffuse_fraction; c->sobol = (sampler == RT_SAMPLER_SOBOL);
   return RT_OK;
 }
 

@@ -80,6 +80,9 @@ struct TraceArgs {
   unsigned long long n_photons, first_id, n_full, ncol;
   unsigned chunk;                      // photon ids per global atomic: kChunk, or less so that a small launch still spreads over all warps
   PhiloxKeys keys;                     // round keys of the Philox key (seed)
+  PhiloxKeys keys_sobol;               // ... of (seed low, seed high ^ 'SOBL'): digital shifts of §3.15
+  float diffuse_fraction;              // §3.15: share of photons launched diffusely (0: none)
+  int sobol;                           // §3.15: entry points from the scrambled 2-D Sobol sequence
   uint32_t stream_id;
 };
 
@@ -240,11 +243,21 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
         const unsigned long long pid = A.first_id + i;
         const uint4 X = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), 0u, A.stream_id, A.keys);
         int ix, iy;
+        float e0 = u24(X.x), e1 = u24(X.y);   // sub-pixel entry point
         if (i < A.n_full) {
           // column = i mod ncol; 32-bit arithmetic whenever the index allows it
           const uint32_t col = (i >> 32) ? (uint32_t)(i % A.ncol) : (uint32_t)i % (uint32_t)A.ncol;
           ix = (int)(col % (uint32_t)A.nx);
           iy = (int)(col / (uint32_t)A.nx);
+          if (A.sobol) {
+            // §3.15: point k = pass number of the 2-D Sobol sequence, XORed with the column's digital shift
+            const uint32_t k = (i >> 32) ? (uint32_t)(i / A.ncol) : (uint32_t)i / (uint32_t)A.ncol;
+            const uint4 S = philox4x32_10(col, A.stream_id, (uint32_t)A.first_id, (uint32_t)(A.first_id >> 32),
+                                          A.keys_sobol);
+            uint32_t x1 = __brev(k), x2 = 0, V = 0x80000000u;
+            for (uint32_t kk = k; kk; kk >>= 1) { if (kk & 1u) x2 ^= V; V ^= V >> 1; }
+            e0 = u24(x1 ^ S.x); e1 = u24(x2 ^ S.y);
+          }
         } else {
           ix = min((int)(u24(X.z) * (float)A.nx), A.nx - 1);
           iy = min((int)(u24(X.w) * (float)A.ny), A.ny - 1);
@@ -261,12 +274,29 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
           cx &= -A.mx; cy &= -A.my; cz &= -A.mz;      // merged-cell origin (factors are powers of two)
           wx *= A.mx; wy *= A.my; Lx = A.Lx1; Ly = A.Ly1; Lz = A.Lz1;
         }
-        // place() with the beam's host-computed reciprocals (same IEEE operations)
-        delx = Lx * fabsf(A.sun_ix); dely = Ly * fabsf(A.sun_iy); delz = Lz * fabsf(A.sun_iz);
-        rx = ((A.sun_ix > 0.0f ? Lx : 0.0f) - ((float)(ix % wx) + u24(X.x)) * A.dx) * A.sun_ix;
-        ry = ((A.sun_iy > 0.0f ? Ly : 0.0f) - ((float)(iy % wy) + u24(X.y)) * A.dy) * A.sun_iy;
-        rz = ((A.sun_iz > 0.0f ? Lz : 0.0f) - Lz) * A.sun_iz;
+        const float qx = ((float)(ix % wx) + e0) * A.dx, qy = ((float)(iy % wy) + e1) * A.dy;
         direct = true;
+        if (A.diffuse_fraction > 0.0f) {
+          // §3.15: block (id, 0 | 2^31): word 0 decides, words 1, 2 give a cosine-weighted downward direction
+          const uint4 D = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), 0x80000000u, A.stream_id, A.keys);
+          if (u24(D.x) < A.diffuse_fraction) {
+            const float v1 = u24(D.y);
+            const float mu = sqrtf(1.0f - v1), sn = sqrtf(v1);
+            float sp, cp;
+            sincos_2pi(u24(D.z), sp, cp);
+            da = sn * cp; db = sn * sp; dc = -mu;
+            direct = false;
+          }
+        }
+        if (direct) {
+          // place() with the beam's host-computed reciprocals (same IEEE operations)
+          delx = Lx * fabsf(A.sun_ix); dely = Ly * fabsf(A.sun_iy); delz = Lz * fabsf(A.sun_iz);
+          rx = ((A.sun_ix > 0.0f ? Lx : 0.0f) - qx) * A.sun_ix;
+          ry = ((A.sun_iy > 0.0f ? Ly : 0.0f) - qy) * A.sun_iy;
+          rz = ((A.sun_iz > 0.0f ? Lz : 0.0f) - Lz) * A.sun_iz;
+        } else {
+          place(qx, qy, Lz);
+        }
         wq = kW0;
         e = 1;
         if (kRecords) { b_ev = t_ev; b_sc = t_sc; b_sfc = t_sfc; }

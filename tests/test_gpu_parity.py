@@ -321,3 +321,32 @@ def test_weighted_mode_config3_sample_and_mixed_accumulation():
     t = g.read_tallies()
     g.close()
     assert t.closure() == 2 * n * rt.W0 and t.counters.n_photons == 2 * n and t.counters.n_capped == 0
+
+
+def test_source_options_sobol_and_diffuse_fraction():
+    """rt_set_source: scrambled Sobol entry points and a diffuse fraction, alone and
+    together, in both absorption modes, with merged cells, against the oracle in kernel precision."""
+    rt = _rt()
+    from dataclasses import replace
+    cfg = replace(CONFIGS[2], block=(2, 2, 2), merge=(8, 8, 4))
+    opt = make_optics(cfg)
+    n = cfg.ncol * 9 + 1234                                # nine full passes + a remainder pass
+    g = rt.Grid(*cfg.grid, device=0, **cfg.accel)
+    g.set_optics(opt["k_ext"], opt["k_ext_cloud"], opt["ssa"], opt["g"], opt["sfc_albedo"])
+    for f, sobol, weighted, first in ((0.0, True, False, 0), (0.35, False, False, 0), (0.2, True, True, (1 << 34) + 3)):
+        g.reset_tallies()
+        g.set_mode(weighted)
+        g.set_source(f, sobol)
+        rec = g.trace(cfg.zenith_deg, cfg.azimuth_deg, n, first_photon_id=first, seed=cfg.seed, stream_id=5,
+                      records=True).cpu().numpy().view(np.uint32)
+        t = g.read_tallies()
+        o32, rec32, _ = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, first_photon_id=first, seed=cfg.seed,
+                                stream_id=5, precision=32, records=True, n_threads=8, weighted=weighted,
+                                diffuse_fraction=f, sobol=sobol, **cfg.accel)
+        assert np.array_equal(rec, rec32), (f, sobol, weighted)
+        for name in ("atm_abs", "sfc_dir", "sfc_dif", "sfc_abs", "toa_up"):
+            assert np.array_equal(getattr(t, name).numpy(), getattr(o32, name)), (name, f, sobol)
+        assert t.counters.asdict() == o32.counters.asdict() and t.closure() == n * rt.W0
+    g.close()
+    with pytest.raises(rt.RtError):
+        rt.Grid(*CONFIGS[1].grid, device=0).set_source(1.5, False)
