@@ -134,6 +134,17 @@ int rt_set_mode(rt_ctx* ctx, int mode);
 #define RT_SAMPLER_SOBOL 1
 int rt_set_source(rt_ctx* ctx, float diffuse_fraction, int sampler);
 
+/* S11, host helper ("The mean weight of all rays hitting the surface or leaving the domain top is then used
+ * to compute surface and TOD radiative fluxes"; heating from the absorbed weight).  Converts `count` tally
+ * quanta (HOST pointer, as read by rt_read_tallies) to physical units in double: every photon of the
+ * n_photons traced into these tallies carries tod_flux * (domain area) / n_photons watts, where tod_flux is the
+ * downward flux through the horizontal domain top in W m^-2 (the paper takes it from a two-stream
+ * pre-computation, out of scope), so out[i] = tally[i] / RT_W0 * tod_flux * ncol / n_photons [W m^-2 per
+ * column], divided by `depth` (the voxel depth dz in metres) when depth > 0 [W m^-3 for atm_abs].
+ * Errors: RT_EINVAL (NULL, n_photons = 0, negative or non-finite arguments).  Runs on the host. */
+int rt_tally_to_flux(const int64_t* tally, double* out, uint64_t count, uint64_t n_photons, uint64_t ncol,
+                     double tod_flux, double depth);
+
 /* Zero tallies and counters on `cuda_stream`. */
 int rt_reset_tallies(rt_ctx* ctx, void* cuda_stream);
 

@@ -13,7 +13,7 @@ FATE_ATM_ABS, FATE_SFC_ABS, FATE_TOD_EXIT, FATE_CAPPED, FATE_ROULETTE = 1, 2, 3,
 MODE_ANALOG, MODE_WEIGHTED = 0, 1
 
 EXPORTS = ("rt_create_grid", "rt_set_merge", "rt_set_mode", "rt_set_source", "rt_set_optics", "rt_trace", "rt_trace_records", "rt_read_tallies",
-           "rt_reset_tallies", "rt_read_majorant", "rt_read_packed_optics", "rt_gather_bench",
+           "rt_reset_tallies", "rt_tally_to_flux", "rt_read_majorant", "rt_read_packed_optics", "rt_gather_bench",
            "rt_last_trace_ms", "rt_launch_count", "rt_philox_words", "rt_last_error", "rt_destroy")
 
 COUNTER_FIELDS = ("n_photons", "n_events", "n_null", "n_rayleigh", "n_hg", "n_atm_abs", "n_sfc_hits",
@@ -55,6 +55,7 @@ def lib():
     L.rt_trace_records.argtypes = [vp, f64, f64, u64, u64, u64, u32, vp, vp]
     L.rt_read_tallies.argtypes = [vp, vp, vp, vp, vp, vp, C.POINTER(rt_counters)]
     L.rt_reset_tallies.argtypes = [vp, vp]
+    L.rt_tally_to_flux.argtypes = [vp, vp, u64, u64, u64, f64, f64]
     L.rt_read_majorant.argtypes = [vp, vp]
     L.rt_read_packed_optics.argtypes = [vp, vp]
     L.rt_gather_bench.argtypes = [vp, u32, u64, vp, C.POINTER(f32), C.POINTER(u64)]
@@ -92,6 +93,18 @@ class Tallies:
         return (int(self.atm_abs.sum()) + int(self.sfc_abs.sum()) + int(self.toa_up.sum())
                 + int(self.counters.capped_energy) + int(self.counters.roulette_lost)
                 - int(self.counters.roulette_gained))
+
+
+def tally_to_flux(tally, n_photons, ncol, tod_flux, depth=0.0):
+    """rt_tally_to_flux on a host int64 tensor: W m^-2 per column (depth = 0) or W m^-3 (depth = dz)."""
+    t = tally.contiguous()
+    if t.is_cuda or t.dtype != torch.int64:
+        raise RtError("tally_to_flux: a host int64 tensor (as rt_read_tallies returns) is required")
+    out = torch.empty(t.shape, dtype=torch.float64)
+    rc = lib().rt_tally_to_flux(_ptr(t), _ptr(out), t.numel(), int(n_photons), int(ncol), float(tod_flux), float(depth))
+    if rc != 0:
+        raise RtError("rt_tally_to_flux failed (%d)" % rc)
+    return out
 
 
 class Grid:

@@ -322,6 +322,15 @@ int rt_set_mode(rt_ctx* c, int mode) {
   return RT_OK;
 }
 
+int rt_tally_to_flux(const int64_t* tally, double* out, uint64_t count, uint64_t n_photons, uint64_t ncol,
+                     double tod_flux, double depth) {
+  if (!tally || !out || n_photons == 0 || ncol == 0) return RT_EINVAL;
+  if (!(tod_flux >= 0.0) || !std::isfinite(tod_flux) || !(depth >= 0.0) || !std::isfinite(depth)) return RT_EINVAL;
+  const double per_quantum = tod_flux * (double)ncol / (double)n_photons / (double)RT_W0 / (depth > 0.0 ? depth : 1.0);
+  for (uint64_t k = 0; k < count; ++k) out[k] = (double)tally[k] * per_quantum;
+  return RT_OK;
+}
+
 int rt_reset_tallies(rt_ctx* c, void* cuda_stream) {
   if (!c) return RT_EINVAL;
   DeviceGuard guard(c->device);

@@ -99,3 +99,25 @@ def test_two_rank_sharding_closes_energy_exactly(tmp_path):
     m = np.load(out)
     assert int(m["atm_abs"].sum()) + int(m["sfc_abs"].sum()) + int(m["toa_up"].sum()) == n_total * O.W0
     assert int(m["sfc_dir"].sum()) % O.W0 == 0 and int(m["sfc_dir"].sum()) > 0
+
+
+def test_tally_to_flux_host_helper():
+    """S11: quanta -> W m^-2 / W m^-3 on the host; needs no GPU.  Vacuum over a black surface from the
+    oracle: every photon arrives, so the domain-mean surface flux is the top-of-domain flux; a Beer-Lambert slab:
+    the column-integrated heating plus the surface flux give back the top-of-domain flux (energy in watts)."""
+    import oracle as O
+    import paper_2208_05247_b200 as rt
+    from rt_inputs import plane_parallel
+    n, F = 1 << 14, 812.5
+    cfg, opt = plane_parallel(8, 8, 8, 100.0, 100.0, 50.0, 0.0, 0.0, albedo=0.0)
+    t, _, _ = O.trace(cfg.grid, opt, 30.0, 0.0, n, seed=1)
+    flux = rt.tally_to_flux(torch.from_numpy(t.sfc_dir), n, cfg.ncol, F)
+    assert flux.shape == (8, 8) and abs(float(flux.mean()) - F) < 1e-9 * F
+    cfg, opt = plane_parallel(8, 8, 8, 100.0, 100.0, 50.0, 2e-3, 0.0, albedo=0.0)
+    t, _, _ = O.trace(cfg.grid, opt, 30.0, 0.0, n, seed=1)
+    heat = rt.tally_to_flux(torch.from_numpy(t.atm_abs), n, cfg.ncol, F, depth=cfg.dz)      # W m^-3
+    sfc = rt.tally_to_flux(torch.from_numpy(t.sfc_abs), n, cfg.ncol, F)
+    assert abs(float((heat.sum(dim=0) * cfg.dz + sfc).mean()) - F) < 1e-9 * F
+    assert 0.1 * F < float(sfc.mean()) < 0.9 * F
+    with pytest.raises(rt.RtError):
+        rt.tally_to_flux(torch.from_numpy(t.sfc_abs), 0, cfg.ncol, F)
