@@ -38,7 +38,7 @@ def lib():
         _lib.orc_trace.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float,
                                    C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_float, C.c_int,
                                    C.c_float, C.c_int, fp, fp, fp, fp, fp, C.c_double, C.c_double,
-                                   C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint32, ip, ip, ip, ip, ip,
+                                   C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint32, ip, ip, ip, ip, ip, ip,
                                    C.POINTER(Counters), C.POINTER(C.c_uint32), C.c_int,
                                    C.POINTER(C.c_double)]
         _lib.orc_hardware_threads.restype = C.c_int
@@ -71,7 +71,7 @@ class Tallies:
 
 def trace(grid, optics, zenith_deg, azimuth_deg, n_photons, first_photon_id=0, seed=1, stream_id=0,
           precision=64, tallies=None, records=False, n_threads=1, merge=(1, 1, 1), merge_ratio=1.25,
-          weighted=False, diffuse_fraction=0.0, sobol=False):
+          weighted=False, diffuse_fraction=0.0, sobol=False, heating_split=False):
     """Run the oracle.  grid = (nx, ny, nz, dx, dy, dz, bx, by, bz); optics = dict with
     k_ext, k_ext_cloud, ssa, g ([nz][ny][nx] fp32) and sfc_albedo ([ny][nx] fp32); merge = merged-cell
     factors ((1, 1, 1) = single-level acceleration grid); weighted = the paper's absorption
@@ -88,13 +88,16 @@ def trace(grid, optics, zenith_deg, azimuth_deg, n_photons, first_photon_id=0, s
     t = tallies if tallies is not None else Tallies(nx, ny, nz)
     rec = np.zeros((n_photons, 4), dtype=np.uint32) if records else None
     ip = C.POINTER(C.c_int64)
+    if heating_split and getattr(t, "atm_abs_direct", None) is None:
+        t.atm_abs_direct = np.zeros((nz, ny, nx), dtype=np.int64)   # heating by never-scattered photons
     el = C.c_double(0.0)
     rc = lib().orc_trace(int(precision), nx, ny, nz, dx, dy, dz, bx, by, bz, int(merge[0]), int(merge[1]),
                          int(merge[2]), float(merge_ratio), int(bool(weighted)), float(diffuse_fraction), int(bool(sobol)), kp, kcp, wp, gp, alp,
                          float(zenith_deg), float(azimuth_deg), int(n_photons), int(first_photon_id),
                          int(seed), int(stream_id), t.atm_abs.ctypes.data_as(ip),
                          t.sfc_dir.ctypes.data_as(ip), t.sfc_dif.ctypes.data_as(ip),
-                         t.sfc_abs.ctypes.data_as(ip), t.toa_up.ctypes.data_as(ip), C.byref(t.counters),
+                         t.sfc_abs.ctypes.data_as(ip), t.toa_up.ctypes.data_as(ip),
+                         t.atm_abs_direct.ctypes.data_as(ip) if heating_split else None, C.byref(t.counters),
                          rec.ctypes.data_as(C.POINTER(C.c_uint32)) if records else None,
                          int(n_threads), C.byref(el))
     if rc != 0:

@@ -232,6 +232,7 @@ struct Problem {
   uint64_t n_photons, first_id, seed;
   uint32_t stream_id;
   int64_t *atm_abs, *sfc_dir, *sfc_dif, *sfc_abs, *toa_up;
+  int64_t* atm_abs_direct;   // optional (may be null): the part of atm_abs deposited by never-scattered photons
   uint32_t* records;
 };
 
@@ -424,12 +425,14 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
           const uint64_t pq = std::min<uint64_t>((uint64_t)1 << 24, (uint64_t)(f * (R)16777216.0));
           const uint64_t a = (w * pq) >> 24;
           if (a) add64(&P.atm_abs[vox], (int64_t)a);
+          if (a && direct && P.atm_abs_direct) add64(&P.atm_abs_direct[vox], (int64_t)a);
           w -= a;
           if (w == 0) { ++C.n_atm_abs; fate = ORC_ATM_ABS; term = (uint32_t)vox; break; }
           xi = E::fma(u1, kh - vx.c1, vx.c1);     // what happens instead: uniform on [c1, k_hat)
         }
         if (!P.weighted && xi < vx.c1) {
           add64(&P.atm_abs[vox], W0); ++C.n_atm_abs;
+          if (direct && P.atm_abs_direct) add64(&P.atm_abs_direct[vox], W0);
           fate = ORC_ATM_ABS; term = (uint32_t)vox; break;
         } else if (xi < vx.c2) {               // cloud droplet: Henyey-Greenstein
           R mu = sample_hg<R>(vx.g, u2);
@@ -600,7 +603,7 @@ int orc_trace(int precision, int nx, int ny, int nz, float dx, float dy, float d
               const float* sfc_albedo, double zenith_deg, double azimuth_deg, uint64_t n_photons,
               uint64_t first_photon_id, uint64_t seed, uint32_t stream_id, int64_t* atm_abs,
               int64_t* sfc_dir, int64_t* sfc_dif, int64_t* sfc_abs, int64_t* toa_up,
-              orc_counters* counters, uint32_t* records, int n_threads, double* elapsed_s) {
+              int64_t* atm_abs_direct, orc_counters* counters, uint32_t* records, int n_threads, double* elapsed_s) {
   if (nx <= 0 || ny <= 0 || nz <= 0 || bx <= 0 || by <= 0 || bz <= 0) return -1;
   if (nx % bx || ny % by || nz % bz) return -1;
   if (mx <= 0 || my <= 0 || mz <= 0 || (nx / bx) % mx || (ny / by) % my || (nz / bz) % mz) return -1;
@@ -609,7 +612,7 @@ int orc_trace(int precision, int nx, int ny, int nz, float dx, float dy, float d
   if (!(diffuse_fraction >= 0.0f && diffuse_fraction <= 1.0f)) return -1;
   Problem P{nx, ny, nz, bx, by, bz, mx, my, mz, merge_ratio, weighted ? 1 : 0, diffuse_fraction, sobol ? 1 : 0, dx, dy, dz, k_ext, k_ext_cloud, ssa, g, sfc_albedo,
             zenith_deg, azimuth_deg, n_photons, first_photon_id, seed, stream_id,
-            atm_abs, sfc_dir, sfc_dif, sfc_abs, toa_up, records};
+            atm_abs, sfc_dir, sfc_dif, sfc_abs, toa_up, atm_abs_direct, records};
   std::vector<float> khat = build_majorant(P);
   if (n_threads < 1) n_threads = 1;
   std::vector<orc_counters> cs(n_threads);

@@ -134,3 +134,31 @@ def test_weighted_reduces_heating_noise():
     mean_a = 0.5 * (runs[(False, 31)] + runs[(False, 32)])
     mean_w = 0.5 * (runs[(True, 31)] + runs[(True, 32)])
     assert np.sqrt(np.mean((mean_a - mean_w) ** 2)) < 3 * d_analog
+
+
+def test_direct_part_of_heating():
+    """P:82 reports heating by direct and by diffuse radiation separately.  The optional tally of heating by
+    never-scattered photons has a closed form in a homogeneous scattering slab: level j absorbs
+    (1 - omega0) (T_{j-1} - T_j) of the incident power directly, T = exp(-k_ext s) along the slant beam
+    (extinction removes photons from the direct beam, a share 1 - omega0 of each removal is absorption).
+    Both absorption modes; pure absorber: direct = total exactly; fully diffuse source: no direct heating."""
+    nz, dz, zen, k, w0 = 16, 100.0, 40.0, 1.1e-3, 0.55
+    cfg, opt = plane_parallel(8, 8, nz, 100.0, 100.0, dz, k, w0, g=0.5, cloud_frac=0.6, albedo=0.3)
+    n = 1 << 19
+    mu0 = np.cos(np.radians(zen))
+    k32, w32 = float(opt["k_ext"][0, 0, 0]), float(opt["ssa"][0, 0, 0])
+    trans = np.exp(-k32 * dz * np.arange(nz + 1) / mu0)
+    expect = (1 - w32) * (trans[:-1] - trans[1:])                       # top level first
+    for wt in (False, True):
+        t, _, _ = O.trace(cfg.grid, opt, zen, 100.0, n, seed=9, n_threads=T, weighted=wt, heating_split=True)
+        assert t.closure() == n * W0
+        assert (t.atm_abs_direct <= t.atm_abs).all() and 0 < int(t.atm_abs_direct.sum()) < int(t.atm_abs.sum())
+        layer = t.atm_abs_direct.sum(axis=(1, 2))[::-1] / (n * W0)
+        chi2 = float(((layer - expect) ** 2 * n / expect).sum())
+        assert chi2 < nz + 4 * np.sqrt(2 * nz), (wt, chi2)
+        d, _, _ = O.trace(cfg.grid, opt, zen, 100.0, 1 << 14, seed=9, n_threads=T, weighted=wt, heating_split=True,
+                          diffuse_fraction=1.0)
+        assert int(d.atm_abs_direct.sum()) == 0 and int(d.atm_abs.sum()) > 0
+    cfg, opt = plane_parallel(8, 8, nz, 100.0, 100.0, dz, k, 0.0, albedo=0.0)
+    t, _, _ = O.trace(cfg.grid, opt, zen, 100.0, 1 << 15, seed=9, n_threads=T, heating_split=True)
+    assert np.array_equal(t.atm_abs_direct, t.atm_abs)
