@@ -134,6 +134,14 @@ int rt_set_mode(rt_ctx* ctx, int mode);
 #define RT_SAMPLER_SOBOL 1
 int rt_set_source(rt_ctx* ctx, float diffuse_fraction, int sampler);
 
+/* Direct part of the heating (P:82 reports heating by direct and by diffuse radiation).  With on != 0 the
+ * following rt_trace calls also add every quantum that a never-scattered photon deposits in atm_abs to a
+ * second nvox-word tally (allocated at the first call, zeroed by rt_reset_tallies); atm_abs stays the total,
+ * the diffuse part is the difference.  rt_read_heating_direct copies it out ([z][y][x], DEVICE or HOST
+ * pointer) and synchronises.  Errors: RT_EINVAL, RT_ENOMEM, RT_ESTATE (read before enabling). */
+int rt_set_heating_split(rt_ctx* ctx, int on);
+int rt_read_heating_direct(rt_ctx* ctx, int64_t* atm_abs_direct);
+
 /* S11, host helper ("The mean weight of all rays hitting the surface or leaving the domain top is then used
  * to compute surface and TOD radiative fluxes"; heating from the absorbed weight).  Converts `count` tally
  * quanta (HOST pointer, as read by rt_read_tallies) to physical units in double: every photon of the

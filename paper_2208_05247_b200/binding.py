@@ -13,7 +13,7 @@ FATE_ATM_ABS, FATE_SFC_ABS, FATE_TOD_EXIT, FATE_CAPPED, FATE_ROULETTE = 1, 2, 3,
 MODE_ANALOG, MODE_WEIGHTED = 0, 1
 
 EXPORTS = ("rt_create_grid", "rt_set_merge", "rt_set_mode", "rt_set_source", "rt_set_optics", "rt_trace", "rt_trace_records", "rt_read_tallies",
-           "rt_reset_tallies", "rt_tally_to_flux", "rt_read_majorant", "rt_read_packed_optics", "rt_gather_bench",
+           "rt_reset_tallies", "rt_set_heating_split", "rt_read_heating_direct", "rt_tally_to_flux", "rt_read_majorant", "rt_read_packed_optics", "rt_gather_bench",
            "rt_last_trace_ms", "rt_launch_count", "rt_philox_words", "rt_last_error", "rt_destroy")
 
 COUNTER_FIELDS = ("n_photons", "n_events", "n_null", "n_rayleigh", "n_hg", "n_atm_abs", "n_sfc_hits",
@@ -55,6 +55,8 @@ def lib():
     L.rt_trace_records.argtypes = [vp, f64, f64, u64, u64, u64, u32, vp, vp]
     L.rt_read_tallies.argtypes = [vp, vp, vp, vp, vp, vp, C.POINTER(rt_counters)]
     L.rt_reset_tallies.argtypes = [vp, vp]
+    L.rt_set_heating_split.argtypes = [vp, i32]
+    L.rt_read_heating_direct.argtypes = [vp, vp]
     L.rt_tally_to_flux.argtypes = [vp, vp, u64, u64, u64, f64, f64]
     L.rt_read_majorant.argtypes = [vp, vp]
     L.rt_read_packed_optics.argtypes = [vp, vp]
@@ -185,6 +187,16 @@ class Grid:
         cnt = rt_counters()
         self._check(self.L.rt_read_tallies(self.ctx, _ptr(a), *[_ptr(t) for t in cols], C.byref(cnt)), "rt_read_tallies")
         return Tallies(a, cols[0], cols[1], cols[2], cols[3], cnt)
+
+    def set_heating_split(self, on=True):
+        """Also tally the heating by never-scattered photons (include/rt.h rt_set_heating_split)."""
+        self._check(self.L.rt_set_heating_split(self.ctx, 1 if on else 0), "rt_set_heating_split")
+
+    def read_heating_direct(self, host=True):
+        nz, ny, nx = self.shape
+        out = torch.empty((nz, ny, nx), dtype=torch.int64, device="cpu" if host else self.device)
+        self._check(self.L.rt_read_heating_direct(self.ctx, _ptr(out)), "rt_read_heating_direct")
+        return out
 
     def reset_tallies(self):
         self._check(self.L.rt_reset_tallies(self.ctx, _stream(self.device)), "rt_reset_tallies")

@@ -20,6 +20,8 @@ struct rt_ctx {
   int weighted = 0;                       // rt_set_mode: 0 analog absorption, 1 weights + roulette
   float diffuse_fraction = 0.0f;          // rt_set_source
   int sobol = 0;
+  unsigned long long* atm_dir = nullptr;  // rt_set_heating_split: heating by never-scattered photons, nvox words
+  bool split = false;
   float* kmin = nullptr;                  // per-cell minimum extinction; allocated when merging is on
   size_t nvox = 0, ncol = 0, ncell = 0;
   float4* optics = nullptr;
@@ -107,6 +109,7 @@ int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photon
   auto inv = [](float d) { return 1.0f / (std::fabs(d) < rt::kTiny ? rt::kTiny : d); };  // IEEE fp32, as set_inverse
   A.sun_ix = inv(A.sun_x); A.sun_iy = inv(A.sun_y); A.sun_iz = inv(A.sun_z);
   A.optics = c->optics; A.khat = c->khat; A.albedo = c->albedo;
+  A.atm_dir = c->split ? c->atm_dir : nullptr;
   A.atm_abs = tally_ptr(c, 0); A.sfc_dir = tally_ptr(c, 1); A.sfc_dif = tally_ptr(c, 2);
   A.sfc_abs = tally_ptr(c, 3); A.toa_up = tally_ptr(c, 4);
   A.counters = c->counters; A.next_photon = c->counters + rt::C_COUNT;
@@ -315,6 +318,26 @@ int rt_set_source(rt_ctx* c, float diffuse_fraction, int sampler) {
   return RT_OK;
 }
 
+int rt_set_heating_split(rt_ctx* c, int on) {
+  if (!c) return RT_EINVAL;
+  DeviceGuard guard(c->device);
+  if (on && !c->atm_dir) {
+    RT_CUDA(c, cudaMalloc(&c->atm_dir, c->nvox * sizeof(unsigned long long)));
+    RT_CUDA(c, cudaMemset(c->atm_dir, 0, c->nvox * sizeof(unsigned long long)));
+  }
+  c->split = on != 0;
+  return RT_OK;
+}
+
+int rt_read_heating_direct(rt_ctx* c, int64_t* out) {
+  if (!c || !out) return RT_EINVAL;
+  if (!c->atm_dir) return fail(c, RT_ESTATE, "rt_read_heating_direct: call rt_set_heating_split(ctx, 1) first");
+  DeviceGuard guard(c->device);
+  RT_CUDA(c, cudaDeviceSynchronize());
+  RT_CUDA(c, cudaMemcpy(out, c->atm_dir, c->nvox * sizeof(int64_t), cudaMemcpyDefault));
+  return RT_OK;
+}
+
 int rt_set_mode(rt_ctx* c, int mode) {
   if (!c) return RT_EINVAL;
   if (mode != RT_MODE_ANALOG && mode != RT_MODE_WEIGHTED) return fail(c, RT_EINVAL, "rt_set_mode: unknown mode");
@@ -337,6 +360,7 @@ int rt_reset_tallies(rt_ctx* c, void* cuda_stream) {
   cudaStream_t st = (cudaStream_t)cuda_stream;
   RT_CUDA(c, cudaMemsetAsync(c->tallies, 0, (c->nvox + 4 * c->ncol) * sizeof(unsigned long long), st));
   RT_CUDA(c, cudaMemsetAsync(c->counters, 0, (rt::C_COUNT + 1) * sizeof(unsigned long long), st));
+  if (c->atm_dir) RT_CUDA(c, cudaMemsetAsync(c->atm_dir, 0, c->nvox * sizeof(unsigned long long), st));
   return RT_OK;
 }
 
@@ -408,7 +432,7 @@ void rt_destroy(rt_ctx* c) {
   {
     DeviceGuard guard(c->device);
     cudaDeviceSynchronize();
-    cudaFree(c->optics); cudaFree(c->khat); cudaFree(c->kmin); cudaFree(c->albedo); cudaFree(c->tallies);
+    cudaFree(c->optics); cudaFree(c->khat); cudaFree(c->kmin); cudaFree(c->atm_dir); cudaFree(c->albedo); cudaFree(c->tallies);
     cudaFree(c->counters); cudaFree(c->bad); cudaFree(c->sink); cudaFree(c->stage);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);

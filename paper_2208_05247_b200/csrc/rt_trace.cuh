@@ -73,6 +73,7 @@ struct TraceArgs {
   const float* __restrict__ khat;      // [cz][cy][cx]
   const float* __restrict__ albedo;    // [y][x]
   unsigned long long* atm_abs;         // [z][y][x]
+  unsigned long long* atm_dir;         // [z][y][x] or nullptr: the part of atm_abs from never-scattered photons
   unsigned long long *sfc_dir, *sfc_dif, *sfc_abs, *toa_up;  // [y][x]
   unsigned long long* counters;        // C_COUNT words
   unsigned long long* next_photon;     // work counter, zeroed before launch
@@ -411,11 +412,13 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
           const unsigned long long pq = min(1u << 24, (unsigned)(f * 16777216.0f));
           const unsigned long long a = (wq * pq) >> 24;
           if (a) atomicAdd(A.atm_abs + vox, a);
+          if (a && direct && A.atm_dir) atomicAdd(A.atm_dir + vox, a);
           wq -= a;
           if (wq == 0) { fate = 1; term = (uint32_t)vox; }
           xi = fmaf(u1, fabsf(kh) - v.x, v.x);      // what happens instead: uniform on [c1, k_hat)
         } else if (xi < v.x) {                      // absorbed by the gas / droplet
           tally_a = A.atm_abs + vox;
+          if (direct && A.atm_dir) atomicAdd(A.atm_dir + vox, kW0);
           fate = 1; term = (uint32_t)vox;
         }
         if (fate == 0) {

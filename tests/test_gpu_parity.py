@@ -350,3 +350,28 @@ def test_source_options_sobol_and_diffuse_fraction():
     g.close()
     with pytest.raises(rt.RtError):
         rt.Grid(*CONFIGS[1].grid, device=0).set_source(1.5, False)
+
+
+def test_direct_part_of_heating_on_gpu():
+    """rt_set_heating_split / rt_read_heating_direct against the oracle's optional tally, both modes."""
+    rt = _rt()
+    from dataclasses import replace
+    cfg = replace(CONFIGS[2], block=(2, 2, 2), merge=(8, 8, 4))
+    opt = make_optics(cfg)
+    n = 1 << 19
+    g = rt.Grid(*cfg.grid, device=0, **cfg.accel)
+    g.set_optics(opt["k_ext"], opt["k_ext_cloud"], opt["ssa"], opt["g"], opt["sfc_albedo"])
+    with pytest.raises(rt.RtError):
+        g.read_heating_direct()
+    g.set_heating_split(True)
+    for weighted in (False, True):
+        g.reset_tallies()
+        g.set_mode(weighted)
+        g.trace(cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed)
+        t = g.read_tallies()
+        d = g.read_heating_direct().numpy()
+        o32, _, _ = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed, precision=32, n_threads=8,
+                            weighted=weighted, heating_split=True, **cfg.accel)
+        assert np.array_equal(d, o32.atm_abs_direct) and np.array_equal(t.atm_abs.numpy(), o32.atm_abs)
+        assert 0 < int(d.sum()) < int(t.atm_abs.sum()) and (d <= t.atm_abs.numpy()).all()
+    g.close()
