@@ -196,10 +196,14 @@ def run_ours(args):
         pinned_all = None
         # two contexts on two streams, points alternating, so that one point's pack and trace fill the SMs the
         # previous point's draining persistent kernel frees; the integer tallies of the two are summed
-        extra = [rt.Grid(*cfg.grid, device=local, **cfg.accel) for _ in range(args.contexts - 1)]
+        from paper_2208_05247_b200.sweeps import spectral_sweep_batched
+        batched = args.contexts == 0       # all points' optics in HBM slots, one launch (rt_trace_batch)
+        if batched:
+            g.set_slots(len(pts))
+        extra = [rt.Grid(*cfg.grid, device=local, **cfg.accel) for _ in range(max(args.contexts, 1) - 1)]
         for gx in extra:
             gx.set_mode(weighted=(args.mode == "weighted"))
-        sweep_streams = [torch.cuda.Stream(dev) for _ in range(args.contexts)]
+        sweep_streams = [torch.cuda.Stream(dev) for _ in range(max(args.contexts, 2))]
         pinned_cols2 = rt.Tallies(None, *[torch.empty((cfg.ny, cfg.nx), dtype=torch.int64).pin_memory()
                                           for _ in range(4)], counters=None)
     else:
@@ -217,8 +221,12 @@ def run_ours(args):
                 gx.reset_tallies()
             ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             ea.record()
-            spectral_sweep_overlapped([g] + extra, sweep_streams, lambda j: fields[j], counts, cfg.zenith_deg,
-                                      cfg.azimuth_deg, seed=cfg.seed, first_photon_id=first)   # 112 x (S0, S1, S2-S10)
+            if batched:
+                spectral_sweep_batched(g, lambda j: fields[j], counts, cfg.zenith_deg, cfg.azimuth_deg,
+                                       seed=cfg.seed, first_photon_id=first)       # 112 x (S0, S1), one S2-S10 launch
+            else:
+                spectral_sweep_overlapped([g] + extra, sweep_streams, lambda j: fields[j], counts, cfg.zenith_deg,
+                                          cfg.azimuth_deg, seed=cfg.seed, first_photon_id=first)   # 112 x (S0, S1, S2-S10)
             eb.record()
             t = g.read_tallies(out=out)                          # S11, both contexts
             for gx in extra:
@@ -359,8 +367,10 @@ def run_ours(args):
                    "l2": ("inputs exceed L2 (%d MiB packed optics + %d MiB tallies vs 126 MB)" % (
                        cfg.nvox * 16 >> 20, cfg.nvox * 8 >> 20)) if cfg.nvox * 24 > (126 << 20) else
                          "inputs fit L2; every step traces new photon ids",
-                   "step": ("reset_tallies + 112 x (set_optics + trace, stream_id = point; two contexts on two "
-                            "streams by default, points alternating) + read_tallies of all"
+                   "step": ("reset_tallies + 112 x set_optics_slot + one trace_batch launch (stream_id = point) + "
+                            "read_tallies" if spectral and args.contexts == 0 else
+                            "reset_tallies + 112 x (set_optics + trace, stream_id = point; points alternating over "
+                            "--contexts contexts and streams) + read_tallies of all"
                             if spectral else
                             "reset_tallies + set_optics + trace + read_tallies(column tallies, counters)")},
         "e2e": e2e,
@@ -401,8 +411,9 @@ def main():
     ap.add_argument("--block", default=None, help="acceleration-grid block bx,by,bz (default: the config's)")
     ap.add_argument("--mode", choices=("analog", "weighted"), default="analog",
                     help="absorption scheme: analog (the metric's, default) or the paper's weights + roulette")
-    ap.add_argument("--contexts", type=int, default=2,
-                    help="workload 4: contexts (streams) the spectral points alternate over")
+    ap.add_argument("--contexts", type=int, default=0,
+                    help="workload 4: 0 (default) = all points' optics in HBM slots and one launch (rt_trace_batch); "
+                         "N >= 1 = one rt_trace per point, points alternating over N contexts on N streams")
     ap.add_argument("--merge", default=None, help="merged-cell factors mx,my,mz (default: the config's; 1,1,1 = off)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing (used under ncu)")
     args = ap.parse_args()

@@ -134,6 +134,29 @@ int rt_set_mode(rt_ctx* ctx, int mode);
 #define RT_SAMPLER_SOBOL 1
 int rt_set_source(rt_ctx* ctx, float diffuse_fraction, int sampler);
 
+/* Batched spectral points (BASELINE.json configs[3]; "Ray tracing is then performed independently for each
+ * quadrature point"): the context holds n_slots packed-optics, majorant and albedo slots in HBM (16 B per voxel
+ * and slot: 112 points of the 512x512x128 grid = 57 GB of the B200's 180 GB), and ONE launch traces the photons
+ * of all points, so that no launch drains between points and the host does not wait per point.
+ * rt_set_slots: (re)allocates the slots (n_slots * nvox < 2^32); slot 0 is the one rt_set_optics and rt_trace
+ *   use; every slot must be given optics again afterwards.  Synchronises the device.
+ * rt_set_optics_slot: rt_set_optics into slot `slot`, asynchronous on `cuda_stream`: range errors accumulate on
+ *   the device and are reported by the next rt_trace_batch (RT_EOPTICS).  Host fields are accepted but make
+ *   the call wait for the stream.
+ * rt_trace_batch: point j (first_point <= j < first_point + n_points <= n_slots) is traced with
+ *   counts[j - first_point] photons (HOST array), stream id j, slot j, global photon ids first_photon_id + (index within the point), its own column stratification
+ *   (full passes over the columns + remainder), i.e. exactly what rt_trace(..., counts[j], first_photon_id, seed,
+ *   stream_id = j) on slot j's optics would trace; tallies accumulate.  records_out: NULL or 16 B per photon in
+ *   the order of the points.  Reads the error mask and uploads the offsets before launching (waits for the
+ *   stream once).  At most two rt_trace_batch launches of a context may be in flight (on different streams,
+ *   e.g. the second half of the points packing while the first half traces).  Errors: RT_EINVAL, RT_ESTATE (a slot without optics), RT_EOPTICS, RT_ENOMEM, RT_ECUDA. */
+int rt_set_slots(rt_ctx* ctx, int n_slots);
+int rt_set_optics_slot(rt_ctx* ctx, int slot, const float* k_ext, const float* k_ext_cloud, const float* ssa,
+                       const float* g, const float* sfc_albedo, void* cuda_stream);
+int rt_trace_batch(rt_ctx* ctx, double zenith_deg, double azimuth_deg, int first_point, int n_points,
+                   const uint64_t* counts, uint64_t first_photon_id, uint64_t seed, void* cuda_stream,
+                   uint32_t* records_out);
+
 /* Direct part of the heating (P:82 reports heating by direct and by diffuse radiation).  With on != 0 the
  * following rt_trace calls also add every quantum that a never-scattered photon deposits in atm_abs to a
  * second nvox-word tally (allocated at the first call, zeroed by rt_reset_tallies); atm_abs stays the total,

@@ -12,7 +12,7 @@ W0 = 1 << 32
 FATE_ATM_ABS, FATE_SFC_ABS, FATE_TOD_EXIT, FATE_CAPPED, FATE_ROULETTE = 1, 2, 3, 4, 5
 MODE_ANALOG, MODE_WEIGHTED = 0, 1
 
-EXPORTS = ("rt_create_grid", "rt_set_merge", "rt_set_mode", "rt_set_source", "rt_set_optics", "rt_trace", "rt_trace_records", "rt_read_tallies",
+EXPORTS = ("rt_create_grid", "rt_set_merge", "rt_set_mode", "rt_set_source", "rt_set_optics", "rt_set_slots", "rt_set_optics_slot", "rt_trace_batch", "rt_trace", "rt_trace_records", "rt_read_tallies",
            "rt_reset_tallies", "rt_set_heating_split", "rt_read_heating_direct", "rt_tally_to_flux", "rt_read_majorant", "rt_read_packed_optics", "rt_gather_bench",
            "rt_last_trace_ms", "rt_launch_count", "rt_philox_words", "rt_last_error", "rt_destroy")
 
@@ -51,6 +51,9 @@ def lib():
     L.rt_set_mode.argtypes = [vp, i32]
     L.rt_set_source.argtypes = [vp, f32, i32]
     L.rt_set_optics.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+    L.rt_set_slots.argtypes = [vp, i32]
+    L.rt_set_optics_slot.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp]
+    L.rt_trace_batch.argtypes = [vp, f64, f64, i32, i32, C.POINTER(u64), u64, u64, vp, vp]
     L.rt_trace.argtypes = [vp, f64, f64, u64, u64, u64, u32, vp]
     L.rt_trace_records.argtypes = [vp, f64, f64, u64, u64, u64, u32, vp, vp]
     L.rt_read_tallies.argtypes = [vp, vp, vp, vp, vp, vp, C.POINTER(rt_counters)]
@@ -163,6 +166,28 @@ class Grid:
         ts = [self._f32(k_ext, nvox), self._f32(k_ext_cloud, nvox), self._f32(ssa, nvox),
               self._f32(g, nvox), self._f32(sfc_albedo, ncol)]
         self._check(self.L.rt_set_optics(self.ctx, *[_ptr(t) for t in ts], _stream(self.device)), "rt_set_optics")
+
+    def set_slots(self, n_slots):
+        """Optics / majorant / albedo slots for batched spectral points (include/rt.h rt_set_slots)."""
+        self._check(self.L.rt_set_slots(self.ctx, int(n_slots)), "rt_set_slots")
+
+    def set_optics_slot(self, slot, k_ext, k_ext_cloud, ssa, g, sfc_albedo):
+        nz, ny, nx = self.shape
+        nvox, ncol = nx * ny * nz, nx * ny
+        ts = [self._f32(k_ext, nvox), self._f32(k_ext_cloud, nvox), self._f32(ssa, nvox),
+              self._f32(g, nvox), self._f32(sfc_albedo, ncol)]
+        self._check(self.L.rt_set_optics_slot(self.ctx, int(slot), *[_ptr(t) for t in ts], _stream(self.device)),
+                    "rt_set_optics_slot")
+
+    def trace_batch(self, zenith_deg, azimuth_deg, counts, first_photon_id=0, seed=1, records=False, first_point=0):
+        """One launch for the spectral points first_point .. first_point + len(counts) - 1 (slot = stream id =
+        point, counts[j - first_point] photons)."""
+        arr = (C.c_uint64 * len(counts))(*[int(x) for x in counts])
+        total = sum(int(x) for x in counts)
+        rec = torch.zeros((max(total, 1), 4), dtype=torch.int32, device=self.device) if records else None
+        self._check(self.L.rt_trace_batch(self.ctx, zenith_deg, azimuth_deg, int(first_point), len(counts), arr, int(first_photon_id),
+                                          int(seed), _stream(self.device), _ptr(rec)), "rt_trace_batch")
+        return rec[:total] if records else None
 
     def trace(self, zenith_deg, azimuth_deg, n_photons, first_photon_id=0, seed=1, stream_id=0, records=False):
         if records:

@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstring>
 #include <string>
+#include <vector>
 
 #include "rt_setup.cuh"
 #include "rt_trace.cuh"
@@ -17,6 +18,10 @@ struct rt_ctx {
   float dx = 0, dy = 0, dz = 0;
   int mx = 1, my = 1, mz = 1;             // merged-cell factors (rt_set_merge)
   float merge_ratio = 1.25f;
+  int n_slots = 1;                        // rt_set_slots: optics / majorant / albedo slots (spectral points)
+  std::vector<char> slot_ok = std::vector<char>(1, 0);
+  unsigned batch_calls = 0;
+  unsigned long long* batch_tab = nullptr; // device: offsets (n_slots + 1) then nfull (n_slots), for rt_trace_batch
   int weighted = 0;                       // rt_set_mode: 0 analog absorption, 1 weights + roulette
   float diffuse_fraction = 0.0f;          // rt_set_source
   int sobol = 0;
@@ -84,9 +89,10 @@ const float* stage_input(rt_ctx* c, const float* p, size_t n, size_t slot_offset
 }
 
 int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photons, uint64_t first_id,
-             uint64_t seed, uint32_t stream_id, void* stream_v, uint32_t* records) {
+             uint64_t seed, uint32_t stream_id, void* stream_v, uint32_t* records, int n_points = 0, int first_point = 0,
+             const unsigned long long* tab = nullptr) {
   if (!c) return RT_EINVAL;
-  if (!c->have_optics) return fail(c, RT_ESTATE, "rt_trace: call rt_set_optics first");
+  if (n_points == 0 && !c->have_optics) return fail(c, RT_ESTATE, "rt_trace: call rt_set_optics first");
   if (!(zenith_deg >= 0.0 && zenith_deg < 90.0) || !std::isfinite(azimuth_deg))
     return fail(c, RT_EINVAL, "rt_trace: zenith must be in [0, 90) degrees and azimuth finite");
   DeviceGuard guard(c->device);
@@ -127,13 +133,24 @@ int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photon
   A.keys = rt::philox_round_keys((uint32_t)seed, (uint32_t)(seed >> 32)); A.stream_id = stream_id;
   A.keys_sobol = rt::philox_round_keys((uint32_t)seed, (uint32_t)(seed >> 32) ^ 0x534F424Cu);
   A.diffuse_fraction = c->diffuse_fraction; A.sobol = c->sobol;
+  A.n_points = n_points; A.first_point = first_point; A.offsets = tab; A.nfull = tab ? tab + c->n_slots + 1 : nullptr;
+  A.nvox32 = (unsigned)c->nvox; A.ncell32 = (unsigned)c->ncell; A.ncol32 = (unsigned)c->ncol;
   RT_CUDA(c, cudaMemsetAsync(A.next_photon, 0, sizeof(unsigned long long), st));
   RT_CUDA(c, cudaEventRecord(c->ev0, st));
   if (n_photons > 0) {
     const bool pow2 = !(c->ncx & (c->ncx - 1)) && !(c->ncy & (c->ncy - 1));
     const int blocks = c->trace_blocks[records ? 1 : 0][c->weighted];
 #define RT_LAUNCH(R, P, W) rt::trace_kernel<R, P, W><<<blocks, rt::kTraceThreads, 0, st>>>(A)
-    if (c->weighted) {
+#define RT_LAUNCH_B(R, P, W) rt::trace_kernel<R, P, W, true><<<blocks, rt::kTraceThreads, 0, st>>>(A)
+    if (n_points > 0) {
+      if (c->weighted) {
+        if (records) { if (pow2) RT_LAUNCH_B(true, true, true); else RT_LAUNCH_B(true, false, true); }
+        else         { if (pow2) RT_LAUNCH_B(false, true, true); else RT_LAUNCH_B(false, false, true); }
+      } else {
+        if (records) { if (pow2) RT_LAUNCH_B(true, true, false); else RT_LAUNCH_B(true, false, false); }
+        else         { if (pow2) RT_LAUNCH_B(false, true, false); else RT_LAUNCH_B(false, false, false); }
+      }
+    } else if (c->weighted) {
       if (records) { if (pow2) RT_LAUNCH(true, true, true); else RT_LAUNCH(true, false, true); }
       else         { if (pow2) RT_LAUNCH(false, true, true); else RT_LAUNCH(false, false, true); }
     } else {
@@ -141,6 +158,7 @@ int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photon
       else         { if (pow2) RT_LAUNCH(false, true, false); else RT_LAUNCH(false, false, false); }
     }
 #undef RT_LAUNCH
+#undef RT_LAUNCH_B
     ++c->launches;
   }
   RT_CUDA(c, cudaEventRecord(c->ev1, st));
@@ -210,22 +228,32 @@ int rt_create_grid(rt_ctx** out, int nx, int ny, int nz, float dx, float dy, flo
   return RT_OK;
 }
 
-int rt_set_optics(rt_ctx* c, const float* k_ext, const float* k_ext_cloud, const float* ssa, const float* g,
-                  const float* sfc_albedo, void* cuda_stream) {
-  if (!c) return RT_EINVAL;
+}  // extern "C" (reopened below)
+
+namespace {
+
+// S0 + S1 into optics / majorant / albedo slot `slot`.  sync: wait for the kernels and report range errors now
+// (rt_set_optics); otherwise the error mask accumulates on the device until rt_trace_batch reads it.
+int set_optics_impl(rt_ctx* c, int slot, const float* k_ext, const float* k_ext_cloud, const float* ssa,
+                    const float* g, const float* sfc_albedo, cudaStream_t st, bool sync, const char* who) {
   if (!k_ext || !k_ext_cloud || !ssa || !g || !sfc_albedo) return fail(c, RT_EINVAL, "rt_set_optics: NULL field");
   DeviceGuard guard(c->device);
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  c->have_optics = false;
+  c->slot_ok[slot] = 0;
+  if (slot == 0) c->have_optics = false;
   int rc = RT_OK;
+  const float* in[5] = {k_ext, k_ext_cloud, ssa, g, sfc_albedo};
   k_ext = stage_input(c, k_ext, c->nvox, 0, st, &rc);                      if (!k_ext) return rc;
   k_ext_cloud = stage_input(c, k_ext_cloud, c->nvox, c->nvox, st, &rc);    if (!k_ext_cloud) return rc;
   ssa = stage_input(c, ssa, c->nvox, 2 * c->nvox, st, &rc);                if (!ssa) return rc;
   g = stage_input(c, g, c->nvox, 3 * c->nvox, st, &rc);                    if (!g) return rc;
   sfc_albedo = stage_input(c, sfc_albedo, c->ncol, 4 * c->nvox, st, &rc);  if (!sfc_albedo) return rc;
-  RT_CUDA(c, cudaMemsetAsync(c->bad, 0, sizeof(int), st));
-  RT_CUDA(c, cudaMemsetAsync(c->khat, 0, c->ncell * sizeof(float), st));
-  RT_CUDA(c, cudaMemcpyAsync(c->albedo, sfc_albedo, c->ncol * sizeof(float), cudaMemcpyDeviceToDevice, st));
+  const bool staged = in[0] != k_ext || in[1] != k_ext_cloud || in[2] != ssa || in[3] != g || in[4] != sfc_albedo;
+  float4* optics = c->optics + (size_t)slot * c->nvox;
+  float* khat = c->khat + (size_t)slot * c->ncell;
+  float* albedo = c->albedo + (size_t)slot * c->ncol;
+  if (sync) RT_CUDA(c, cudaMemsetAsync(c->bad, 0, sizeof(int), st));
+  RT_CUDA(c, cudaMemsetAsync(khat, 0, c->ncell * sizeof(float), st));
+  RT_CUDA(c, cudaMemcpyAsync(albedo, sfc_albedo, c->ncol * sizeof(float), cudaMemcpyDeviceToDevice, st));
   const int blocks = c->sm_count * 8;
   const bool merging = c->mx * c->my * c->mz > 1;
   if (merging) {
@@ -235,31 +263,107 @@ int rt_set_optics(rt_ctx* c, const float* k_ext, const float* k_ext_cloud, const
   const bool rows = (c->nx % 4 == 0) && !(((uintptr_t)k_ext | (uintptr_t)k_ext_cloud | (uintptr_t)ssa | (uintptr_t)g) & 15u);
   if (rows)
     rt::pack_optics_rows_kernel<<<c->sm_count * 16, 128, 0, st>>>(
-        (const float4*)k_ext, (const float4*)k_ext_cloud, (const float4*)ssa, (const float4*)g, c->optics,
-        (int*)c->khat, merging ? (int*)c->kmin : nullptr, c->nx, c->ny, c->nz, c->bx, c->by, c->bz, c->bad);
+        (const float4*)k_ext, (const float4*)k_ext_cloud, (const float4*)ssa, (const float4*)g, optics,
+        (int*)khat, merging ? (int*)c->kmin : nullptr, c->nx, c->ny, c->nz, c->bx, c->by, c->bz, c->bad);
   else
-    rt::pack_optics_kernel<<<blocks, 256, 0, st>>>(k_ext, k_ext_cloud, ssa, g, c->optics, (int*)c->khat,
+    rt::pack_optics_kernel<<<blocks, 256, 0, st>>>(k_ext, k_ext_cloud, ssa, g, optics, (int*)khat,
                                                   merging ? (int*)c->kmin : nullptr, c->nx,
                                                   c->ny, c->nz, c->bx, c->by, c->bz, c->bad);
-  rt::check_albedo_kernel<<<c->sm_count, 256, 0, st>>>(c->albedo, c->ncol, c->bad);
+  rt::check_albedo_kernel<<<c->sm_count, 256, 0, st>>>(albedo, c->ncol, c->bad);
   c->launches += 2;
   if (merging) {
     const size_t nblk = c->ncell / ((size_t)c->mx * c->my * c->mz);
-    rt::merge_cells_kernel<<<(unsigned)((nblk + 127) / 128), 128, 0, st>>>(c->khat, c->kmin, c->ncx, c->ncy, c->ncz,
+    rt::merge_cells_kernel<<<(unsigned)((nblk + 127) / 128), 128, 0, st>>>(khat, c->kmin, c->ncx, c->ncy, c->ncz,
                                                                             c->mx, c->my, c->mz, c->merge_ratio);
     ++c->launches;
   }
   RT_CUDA(c, cudaGetLastError());
+  if (sync) {
+    int bad = 0;
+    RT_CUDA(c, cudaMemcpyAsync(&bad, c->bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+    RT_CUDA(c, cudaStreamSynchronize(st));
+    if (bad) {
+      char msg[176];
+      snprintf(msg, sizeof msg, "%s: input out of range (mask 0x%x: 1 k_ext, 2 k_ext_cloud, 4 ssa, 8 g, 16 albedo)", who, bad);
+      return fail(c, RT_EOPTICS, msg);
+    }
+  } else if (staged) {
+    RT_CUDA(c, cudaStreamSynchronize(st));   // the one staging buffer is about to be reused
+  }
+  c->slot_ok[slot] = 1;
+  if (slot == 0 && sync) c->have_optics = true;
+  return RT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int rt_set_optics(rt_ctx* c, const float* k_ext, const float* k_ext_cloud, const float* ssa, const float* g,
+                  const float* sfc_albedo, void* cuda_stream) {
+  if (!c) return RT_EINVAL;
+  return set_optics_impl(c, 0, k_ext, k_ext_cloud, ssa, g, sfc_albedo, (cudaStream_t)cuda_stream, true, "rt_set_optics");
+}
+
+int rt_set_slots(rt_ctx* c, int n_slots) {
+  if (!c) return RT_EINVAL;
+  if (n_slots < 1 || (unsigned long long)n_slots * c->nvox >= (1ull << 32))
+    return fail(c, RT_EINVAL, "rt_set_slots: need 1 <= n_slots and n_slots * nvox < 2^32");
+  DeviceGuard guard(c->device);
+  RT_CUDA(c, cudaDeviceSynchronize());
+  cudaFree(c->optics); cudaFree(c->khat); cudaFree(c->albedo); cudaFree(c->batch_tab);
+  c->optics = nullptr; c->khat = nullptr; c->albedo = nullptr; c->batch_tab = nullptr;
+  c->have_optics = false;
+  c->n_slots = n_slots;
+  c->slot_ok.assign((size_t)n_slots, 0);
+  RT_CUDA(c, cudaMalloc(&c->optics, (size_t)n_slots * c->nvox * sizeof(float4)));
+  RT_CUDA(c, cudaMalloc(&c->khat, (size_t)n_slots * c->ncell * sizeof(float)));
+  RT_CUDA(c, cudaMalloc(&c->albedo, (size_t)n_slots * c->ncol * sizeof(float)));
+  RT_CUDA(c, cudaMalloc(&c->batch_tab, 2 * (2 * (size_t)n_slots + 1) * sizeof(unsigned long long)));   // two launches may be in flight
+  RT_CUDA(c, cudaMemset(c->bad, 0, sizeof(int)));
+  return RT_OK;
+}
+
+int rt_set_optics_slot(rt_ctx* c, int slot, const float* k_ext, const float* k_ext_cloud, const float* ssa,
+                       const float* g, const float* sfc_albedo, void* cuda_stream) {
+  if (!c) return RT_EINVAL;
+  if (slot < 0 || slot >= c->n_slots) return fail(c, RT_EINVAL, "rt_set_optics_slot: slot out of range (rt_set_slots)");
+  return set_optics_impl(c, slot, k_ext, k_ext_cloud, ssa, g, sfc_albedo, (cudaStream_t)cuda_stream, false,
+                         "rt_set_optics_slot");
+}
+
+int rt_trace_batch(rt_ctx* c, double zenith_deg, double azimuth_deg, int first_point, int n_points,
+                   const uint64_t* counts, uint64_t first_photon_id, uint64_t seed, void* cuda_stream,
+                   uint32_t* records_out) {
+  if (!c) return RT_EINVAL;
+  if (first_point < 0 || n_points < 1 || first_point + n_points > c->n_slots || !counts || !c->batch_tab)
+    return fail(c, RT_EINVAL, "rt_trace_batch: points must lie within the slots (rt_set_slots), counts not NULL");
+  for (int j = first_point; j < first_point + n_points; ++j)
+    if (!c->slot_ok[j]) return fail(c, RT_ESTATE, "rt_trace_batch: a slot below n_points has no optics (rt_set_optics_slot)");
+  DeviceGuard guard(c->device);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  // range errors of the slots' fields, accumulated on the device since rt_set_slots
   int bad = 0;
   RT_CUDA(c, cudaMemcpyAsync(&bad, c->bad, sizeof(int), cudaMemcpyDeviceToHost, st));
   RT_CUDA(c, cudaStreamSynchronize(st));
   if (bad) {
-    char msg[160];
-    snprintf(msg, sizeof msg, "rt_set_optics: input out of range (mask 0x%x: 1 k_ext, 2 k_ext_cloud, 4 ssa, 8 g, 16 albedo)", bad);
+    char msg[176];
+    snprintf(msg, sizeof msg, "rt_trace_batch: a slot's input is out of range (mask 0x%x: 1 k_ext, 2 k_ext_cloud, 4 ssa, 8 g, 16 albedo)", bad);
     return fail(c, RT_EOPTICS, msg);
   }
-  c->have_optics = true;
-  return RT_OK;
+  std::vector<unsigned long long> tab(2 * (size_t)c->n_slots + 1, 0ull);
+  unsigned long long total = 0;
+  for (int j = 0; j < n_points; ++j) {
+    tab[j] = total;
+    tab[(size_t)c->n_slots + 1 + j] = (counts[j] / c->ncol) * c->ncol;
+    total += counts[j];
+  }
+  for (int j = n_points; j <= c->n_slots; ++j) tab[j] = total;
+  unsigned long long* dtab = c->batch_tab + (c->batch_calls++ & 1u) * tab.size();   // alternate: two launches in flight
+  RT_CUDA(c, cudaMemcpyAsync(dtab, tab.data(), tab.size() * sizeof(unsigned long long), cudaMemcpyHostToDevice, st));
+  RT_CUDA(c, cudaStreamSynchronize(st));   // tab is a stack vector
+  return do_trace(c, zenith_deg, azimuth_deg, total, first_photon_id, seed, 0u, cuda_stream, records_out, n_points,
+                  first_point, dtab);
 }
 
 int rt_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photons, uint64_t first_photon_id,
@@ -433,7 +537,7 @@ void rt_destroy(rt_ctx* c) {
     DeviceGuard guard(c->device);
     cudaDeviceSynchronize();
     cudaFree(c->optics); cudaFree(c->khat); cudaFree(c->kmin); cudaFree(c->atm_dir); cudaFree(c->albedo); cudaFree(c->tallies);
-    cudaFree(c->counters); cudaFree(c->bad); cudaFree(c->sink); cudaFree(c->stage);
+    cudaFree(c->counters); cudaFree(c->bad); cudaFree(c->batch_tab); cudaFree(c->sink); cudaFree(c->stage);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
   }

@@ -82,6 +82,12 @@ struct TraceArgs {
   unsigned chunk;                      // photon ids per global atomic: kChunk, or less so that a small launch still spreads over all warps
   PhiloxKeys keys;                     // round keys of the Philox key (seed)
   PhiloxKeys keys_sobol;               // ... of (seed low, seed high ^ 'SOBL'): digital shifts of §3.15
+  // batched launch (kBatch; rt_trace_batch): photons of n_points spectral points in one launch; point j owns
+  // the launch indices [offsets[j], offsets[j+1]), reads optics slot j and majorant slot j, draws on stream j
+  const unsigned long long* offsets;   // n_points + 1 prefix sums (device)
+  const unsigned long long* nfull;     // per point: ncol * floor(count / ncol) (device)
+  int n_points, first_point;           // points first_point .. first_point + n_points - 1 (slot = stream id = point)
+  unsigned nvox32, ncell32, ncol32;    // slot strides of optics, majorant and albedo
   float diffuse_fraction;              // §3.15: share of photons launched diffusely (0: none)
   int sobol;                           // §3.15: entry points from the scrambled 2-D Sobol sequence
   uint32_t stream_id;
@@ -107,7 +113,8 @@ __device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
 // kPow2: the acceleration grid's x and y extents are powers of two, so the periodic wrap is a mask.
 // kWeighted: the paper's absorption weights + Russian roulette instead of analog
 // absorption: integer weight wq (tally quanta), deposits at every tentative collision, roulette ledger.
-template <bool kRecords, bool kPow2, bool kWeighted>
+// kBatch: several spectral points in one launch, each with its own optics and majorant slot (see TraceArgs).
+template <bool kRecords, bool kPow2, bool kWeighted, bool kBatch = false>
 __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(const TraceArgs A) {
   __shared__ unsigned long long s_cnt[C_COUNT];
   if (threadIdx.x < C_COUNT) s_cnt[threadIdx.x] = 0ull;
@@ -120,7 +127,9 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
 
   // photon state
   uint32_t st = ST_DEAD;
-  unsigned long long i = 0;
+  unsigned long long i = 0;               // index in the call (kBatch: in the photon's point)
+  uint32_t jpt = 0;                       // kBatch: the photon's point = its stream id and slot
+  unsigned long long ig = 0;              // kBatch: index in the launch (records)
   uint32_t e = 0;
   int cx = 0, cy = 0, cz = 0;
   float da = 0, db = 0, dc = -1;          // unit direction
@@ -142,9 +151,10 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
   uint32_t t_rkept = 0;
   uint32_t b_ev = 0, b_sc = 0, b_sfc = 0;  // totals when the current photon was launched (records only)
 
+  auto sid = [&]() { return kBatch ? jpt : A.stream_id; };
   auto draw = [&]() {
     const unsigned long long pid = A.first_id + i;
-    const uint4 X = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), e, A.stream_id, A.keys);
+    const uint4 X = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), e, sid(), A.keys);
     tau = neg_log(1.0f - u24(X.x)); u1 = u24(X.y); w2 = X.z; w3 = X.w;
   };
   // local coordinate from a remaining distance: q = face - v r, face = L if v > 0 else 0
@@ -169,7 +179,10 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
     ry = ((vb > 0.0f ? Ly : 0.0f) - qy) * ib;
     rz = ((vc > 0.0f ? Lz : 0.0f) - qz) * ic;
   };
-  auto cell_of = [&]() { return ((unsigned)cz * (unsigned)A.ncy + (unsigned)cy) * (unsigned)A.ncx + (unsigned)cx; };
+  auto cell_of = [&]() {
+    const unsigned c = ((unsigned)cz * (unsigned)A.ncy + (unsigned)cy) * (unsigned)A.ncx + (unsigned)cx;
+    return kBatch ? c + jpt * A.ncell32 : c;
+  };
   // §3.14 roulette: below W0/2 survive with probability wq / W0 exactly (32-bit word of the Philox block at
   // counter e | 2^31 against wq) and continue with W0, else end; both branches go to the ledger
   int fate = 0;
@@ -177,7 +190,7 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
   auto roulette = [&](uint32_t where) {
     if (wq >= kW0 / 2) return false;
     const unsigned long long pid = A.first_id + i;
-    const uint4 Y = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), e | 0x80000000u, A.stream_id, A.keys);
+    const uint4 Y = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), e | 0x80000000u, sid(), A.keys);
     if ((unsigned long long)Y.w < wq) { t_rgain += kW0 - wq; ++t_rkept; wq = kW0; return false; }
     t_rlost += wq; fate = 5; term = where;
     return true;
@@ -241,11 +254,24 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
       }
       if (got) {
         // ---- §3.6 launch, event index 0 ------------------------------------------------------
+        unsigned long long n_full = A.n_full;
+        if (kBatch) {
+          // which point owns launch index i: last j with offsets[j] <= i
+          ig = i;
+          int lo = 0, hi = A.n_points;
+          while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (__ldg(A.offsets + mid) <= i) lo = mid; else hi = mid;
+          }
+          jpt = (uint32_t)(lo + A.first_point);
+          i -= __ldg(A.offsets + lo);
+          n_full = __ldg(A.nfull + lo);
+        }
         const unsigned long long pid = A.first_id + i;
-        const uint4 X = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), 0u, A.stream_id, A.keys);
+        const uint4 X = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), 0u, sid(), A.keys);
         int ix, iy;
         float e0 = u24(X.x), e1 = u24(X.y);   // sub-pixel entry point
-        if (i < A.n_full) {
+        if (i < n_full) {
           // column = i mod ncol; 32-bit arithmetic whenever the index allows it
           const uint32_t col = (i >> 32) ? (uint32_t)(i % A.ncol) : (uint32_t)i % (uint32_t)A.ncol;
           ix = (int)(col % (uint32_t)A.nx);
@@ -253,7 +279,7 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
           if (A.sobol) {
             // §3.15: point k = pass number of the 2-D Sobol sequence, XORed with the column's digital shift
             const uint32_t k = (i >> 32) ? (uint32_t)(i / A.ncol) : (uint32_t)i / (uint32_t)A.ncol;
-            const uint4 S = philox4x32_10(col, A.stream_id, (uint32_t)A.first_id, (uint32_t)(A.first_id >> 32),
+            const uint4 S = philox4x32_10(col, sid(), (uint32_t)A.first_id, (uint32_t)(A.first_id >> 32),
                                           A.keys_sobol);
             uint32_t x1 = __brev(k), x2 = 0, V = 0x80000000u;
             for (uint32_t kk = k; kk; kk >>= 1) { if (kk & 1u) x2 ^= V; V ^= V >> 1; }
@@ -279,7 +305,7 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
         direct = true;
         if (A.diffuse_fraction > 0.0f) {
           // §3.15: block (id, 0 | 2^31): word 0 decides, words 1, 2 give a cosine-weighted downward direction
-          const uint4 D = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), 0x80000000u, A.stream_id, A.keys);
+          const uint4 D = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), 0x80000000u, sid(), A.keys);
           if (u24(D.x) < A.diffuse_fraction) {
             const float v1 = u24(D.y);
             const float mu = sqrtf(1.0f - v1), sn = sqrtf(v1);
@@ -402,7 +428,7 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
         // 32-bit indices: rt_create_grid refuses grids of 2^32 voxels or more
         const unsigned vox = ((unsigned)(cz * A.bz + lz) * (unsigned)A.ny + (unsigned)(cy * A.by + ly)) * (unsigned)A.nx
                              + (unsigned)(cx * A.bx + lx);
-        const float4 v = __ldg(&A.optics[vox]);
+        const float4 v = __ldg(&A.optics[kBatch ? vox + jpt * A.nvox32 : vox]);
         ++t_ev;
         float xi = u1 * fabsf(kh);
         st = ST_MOVE;
@@ -488,7 +514,7 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
           if (kWeighted) {
             // §3.14: arrival tallied with the weight; the albedo reduces the weight, 24-bit fixed point
             atomicAdd((direct ? A.sfc_dir : A.sfc_dif) + col, wq);
-            const unsigned long long aq = min(1u << 24, (unsigned)(__ldg(&A.albedo[col]) * 16777216.0f));
+            const unsigned long long aq = min(1u << 24, (unsigned)(__ldg(&A.albedo[kBatch ? col + jpt * A.ncol32 : col]) * 16777216.0f));
             const unsigned long long refl = (wq * aq) >> 24;
             if (wq - refl) atomicAdd(A.sfc_abs + col, wq - refl);
             wq = refl;
@@ -496,7 +522,7 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
             else reflect = !roulette((uint32_t)col);
           } else {
             tally_a = (direct ? A.sfc_dir : A.sfc_dif) + col;
-            reflect = u1 < __ldg(&A.albedo[col]);
+            reflect = u1 < __ldg(&A.albedo[kBatch ? col + jpt * A.ncol32 : col]);
             if (!reflect) { tally_b = A.sfc_abs + col; fate = 2; term = (uint32_t)col; }
           }
           if (reflect) {
@@ -548,7 +574,7 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
         uint4 r;
         r.x = (uint32_t)fate | (min(t_sfc - b_sfc, 0xFFFFFFu) << 8);
         r.y = term; r.z = t_ev - b_ev; r.w = t_sc - b_sc;
-        reinterpret_cast<uint4*>(A.records)[i] = r;
+        reinterpret_cast<uint4*>(A.records)[kBatch ? ig : i] = r;
       }
     }
   }

@@ -85,6 +85,26 @@ def test_config4_spectral_sweep():
     for name in TALLIES:
         assert torch.equal(getattr(t2, name), getattr(t, name)), name
     g2.close()
+
+    # ... and with all 112 points' optics resident in HBM slots and ONE launch (rt_trace_batch)
+    from paper_2208_05247_b200.sweeps import spectral_sweep_batched
+    g.set_slots(112)
+    g.reset_tallies()
+    total3 = spectral_sweep_batched(g, lambda j: [make_optics_torch(cfg, pts[j])[k] for k in NAMES], counts,
+                                    cfg.zenith_deg, cfg.azimuth_deg, seed=cfg.seed)
+    t3 = g.read_tallies()
+    assert total3 == total and t3.counters.asdict() == c.asdict()
+    for name in TALLIES:
+        assert torch.equal(getattr(t3, name), getattr(t, name)), name
+    # ... in two halves on two streams (the second half packs while the first traces)
+    g.reset_tallies()
+    spectral_sweep_batched(g, lambda j: [make_optics_torch(cfg, pts[j])[k] for k in NAMES], counts,
+                           cfg.zenith_deg, cfg.azimuth_deg, seed=cfg.seed, streams=streams)
+    torch.cuda.synchronize()
+    t4 = g.read_tallies()
+    assert t4.counters.asdict() == c.asdict()
+    for name in TALLIES:
+        assert torch.equal(getattr(t4, name), getattr(t, name)), name
     g.close()
 
 
@@ -124,3 +144,47 @@ def test_config5_convergence_sweep():
         c = [r[key] / np.sqrt(1.0 / r["photons_per_column"] + 1.0 / ref["photons_per_column"]) for r in rows]
         assert max(c) / min(c) < 1.15, (key, c)
         assert rows[0][key] > 4 * rows[3][key]        # 64x the photons: ~ sqrt((1+1/256)/(1/64+1/256)) = 7.2
+
+
+def test_batched_points_equal_separate_traces():
+    """rt_trace_batch (one launch, slots in HBM) traces exactly what separate rt_trace calls per point would:
+    records per point against the oracle in kernel precision (own optics, stream id = point, ragged counts incl.
+    0 and a remainder pass), accumulated tallies and counters = the sum over the points."""
+    rt = _rt()
+    from dataclasses import replace
+    cfg = replace(CONFIGS[2], block=(2, 2, 2), merge=(8, 8, 4))
+    pts = spectral_points(112)
+    sel = (3, 40, 77, 111, 5)
+    counts = [cfg.ncol * 2 + 77, 0, 1000, cfg.ncol, 33]
+    g = rt.Grid(*cfg.grid, device=0, **cfg.accel)
+    g.set_slots(len(sel))
+    opts = [make_optics(cfg, pts[j]) for j in sel]
+    for k, opt in enumerate(opts):
+        g.set_optics_slot(k, *[opt[n] for n in NAMES])
+    first = (1 << 33) + 11
+    rec = g.trace_batch(cfg.zenith_deg, cfg.azimuth_deg, counts, first_photon_id=first, seed=cfg.seed,
+                        records=True).cpu().numpy().view(np.uint32)
+    t = g.read_tallies()
+    total = O.Tallies(cfg.nx, cfg.ny, cfg.nz)
+    off = 0
+    for k, (opt, n) in enumerate(zip(opts, counts)):
+        if n == 0:
+            continue
+        _, rec32, _ = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, first_photon_id=first, seed=cfg.seed,
+                              stream_id=k, precision=32, records=True, n_threads=8, tallies=total, **cfg.accel)
+        assert np.array_equal(rec[off:off + n], rec32), k
+        off += n
+    for name in TALLIES:
+        assert np.array_equal(getattr(t, name).numpy(), getattr(total, name)), name
+    assert t.counters.asdict() == total.counters.asdict() and t.closure() == sum(counts) * rt.W0
+    # errors: a slot without optics, a bad field reported at the batch trace
+    g.set_slots(2)
+    g.set_optics_slot(0, *[opts[0][n] for n in NAMES])
+    with pytest.raises(rt.RtError):
+        g.trace_batch(cfg.zenith_deg, cfg.azimuth_deg, [10, 10])
+    bad = opts[0]["ssa"].copy()
+    bad[1, 2, 3] = -0.5
+    g.set_optics_slot(1, opts[0]["k_ext"], opts[0]["k_ext_cloud"], bad, opts[0]["g"], opts[0]["sfc_albedo"])
+    with pytest.raises(rt.RtError):
+        g.trace_batch(cfg.zenith_deg, cfg.azimuth_deg, [10, 10])
+    g.close()
