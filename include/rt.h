@@ -7,8 +7,11 @@
  * fine grid, scatter by Rayleigh or Henyey-Greenstein with the cloud/gas split
  * k_ext,cloud/k_ext, reflect at a Lambertian surface with local albedo and
  * are tallied as surface flux (direct = never scattered), domain-top upward flux
- * and 3D absorbed power.  Absorption is analog (BASELINE.json north_star): each
- * photon carries RT_W0 = 2^32 integer quanta and ends in exactly one bin.
+ * and 3D absorbed power.  Absorption is analog by default (BASELINE.json north_star):
+ * each photon carries RT_W0 = 2^32 integer quanta and ends in exactly one bin.  Options, all off
+ * after rt_create_grid: merged acceleration cells (rt_set_merge), the paper's weights + Russian
+ * roulette (rt_set_mode), its top-of-domain source (rt_set_source), the direct part of the heating
+ * (rt_set_heating_split), many spectral points in one launch (rt_set_slots, rt_trace_batch).
  *
  * Every step runs in CUDA kernels for sm_100a; there is no CPU fallback.  All functions
  * return 0 (RT_OK) or a negative RT_E* code; no exception crosses this boundary;
@@ -40,6 +43,7 @@ extern "C" {
 #define RT_FATE_SFC_ABS 2
 #define RT_FATE_TOD_EXIT 3
 #define RT_FATE_CAPPED 4
+#define RT_FATE_ROULETTE 5 /* weighted mode only */
 
 typedef struct rt_ctx rt_ctx; /* opaque; owned by the library; one CUDA device per context */
 
