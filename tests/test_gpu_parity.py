@@ -375,3 +375,52 @@ def test_direct_part_of_heating_on_gpu():
         assert np.array_equal(d, o32.atm_abs_direct) and np.array_equal(t.atm_abs.numpy(), o32.atm_abs)
         assert 0 < int(d.sum()) < int(t.atm_abs.sum()) and (d <= t.atm_abs.numpy()).all()
     g.close()
+
+
+def test_random_small_configurations():
+    """Seeded random small problems: anisotropic voxels, non-cubic acceleration cells, merged or not, every
+    option combination, grazing and overhead sun, odd photon counts: records, tallies and counters against the
+    oracle in kernel precision each time."""
+    rt = _rt()
+    rng = np.random.default_rng(20260811)
+    for case in range(10):
+        bx, by, bz = (int(rng.choice([1, 2, 4])) for _ in range(3))
+        mx, my, mz = (int(rng.choice([1, 2, 4])) for _ in range(3))
+        ncx, ncy, ncz = (int(rng.choice([4, 8, 12])) * m for m in (mx, my, mz))
+        nx, ny, nz = ncx * bx, ncy * by, ncz * bz
+        dx, dy, dz = (float(rng.choice([20.0, 37.5, 100.0])) for _ in range(3))
+        k = np.full((nz, ny, nx), float(rng.choice([0.0, 3e-5, 4e-4])))
+        for _ in range(int(rng.integers(0, 5))):
+            z0, y0, x0 = (int(rng.integers(0, max(1, n_ - 3))) for n_ in (nz, ny, nx))
+            k[z0:z0 + 3, y0:y0 + 4, x0:x0 + 3] += rng.uniform(1e-3, 5e-2, size=k[z0:z0 + 3, y0:y0 + 4, x0:x0 + 3].shape)
+        cloudy = k > 1e-3
+        cfg, opt = plane_parallel(nx, ny, nz, dx, dy, dz, 0.0, 0.0, albedo=0.0, block=(bx, by, bz))
+        opt["k_ext"] = k.astype(np.float32)
+        opt["k_ext_cloud"] = np.where(cloudy, 0.97 * k, 0.0).astype(np.float32)
+        opt["ssa"] = np.where(cloudy, 0.995, float(rng.uniform(0.0, 1.0))).astype(np.float32)
+        opt["g"] = np.full((nz, ny, nx), float(rng.uniform(-0.3, 0.9)), dtype=np.float32)
+        opt["sfc_albedo"] = rng.uniform(0.0, 1.0, size=(ny, nx)).astype(np.float32)
+        accel = {"merge": (mx, my, mz), "merge_ratio": float(rng.choice([1.0, 1.25, 3.0]))}
+        zen, azi = float(rng.choice([0.0, 25.0, 70.0, 88.0])), float(rng.uniform(0.0, 360.0))
+        weighted, sobol = bool(rng.integers(0, 2)), bool(rng.integers(0, 2))
+        f = float(rng.choice([0.0, 0.0, 0.4, 1.0]))
+        n = int(rng.integers(1, 3 * nx * ny + 2000))
+        first, sid, seed = int(rng.integers(0, 1 << 40)), int(rng.integers(0, 1 << 20)), int(rng.integers(1, 1 << 50))
+        g = rt.Grid(*cfg.grid, device=0, **accel)
+        g.set_mode(weighted)
+        g.set_source(f, sobol)
+        g.set_heating_split(True)
+        g.set_optics(*[opt[k_] for k_ in ("k_ext", "k_ext_cloud", "ssa", "g", "sfc_albedo")])
+        rec = g.trace(zen, azi, n, first_photon_id=first, seed=seed, stream_id=sid, records=True).cpu().numpy().view(np.uint32)
+        t = g.read_tallies()
+        d = g.read_heating_direct().numpy()
+        g.close()
+        o, orec, _ = O.trace(cfg.grid, opt, zen, azi, n, first_photon_id=first, seed=seed, stream_id=sid, precision=32,
+                             records=True, n_threads=4, weighted=weighted, diffuse_fraction=f, sobol=sobol,
+                             heating_split=True, **accel)
+        tag = (case, (nx, ny, nz), (bx, by, bz), accel, zen, weighted, sobol, f)
+        assert np.array_equal(rec, orec), tag
+        for name in ("atm_abs", "sfc_dir", "sfc_dif", "sfc_abs", "toa_up"):
+            assert np.array_equal(getattr(t, name).numpy(), getattr(o, name)), (name,) + tag
+        assert np.array_equal(d, o.atm_abs_direct), tag
+        assert t.counters.asdict() == o.counters.asdict() and t.closure() == n * rt.W0, tag
