@@ -100,6 +100,13 @@ int rt_trace_records(rt_ctx* ctx, double zenith_deg, double azimuth_deg, uint64_
 int rt_read_tallies(rt_ctx* ctx, int64_t* atm_abs, int64_t* sfc_dir, int64_t* sfc_dif, int64_t* sfc_abs,
                     int64_t* toa_up, rt_counters* counters);
 
+/* rt_read_tallies without the wait: the copies (and a one-thread kernel that assembles the counters) are queued
+ * on `cuda_stream` after the work already queued there; the outputs are valid once the caller has synchronised
+ * that stream.  HOST outputs should be pinned, or the copies serialise with the host.  Lets a caller upload the
+ * next step's fields and download the last step's tallies while another context traces (bench.py's e2e leg). */
+int rt_read_tallies_async(rt_ctx* ctx, int64_t* atm_abs, int64_t* sfc_dir, int64_t* sfc_dif, int64_t* sfc_abs,
+                          int64_t* toa_up, rt_counters* counters, void* cuda_stream);
+
 /* Merged acceleration cells (P:54 leaves the acceleration grid's resolution open).
  * Blocks of mx*my*mz acceleration cells in which the extinction is nearly uniform (max k_ext <=
  * merge_ratio * min k_ext over the block's voxels) are traversed as ONE cell with the block's maximum as

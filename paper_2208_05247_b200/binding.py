@@ -12,7 +12,7 @@ W0 = 1 << 32
 FATE_ATM_ABS, FATE_SFC_ABS, FATE_TOD_EXIT, FATE_CAPPED, FATE_ROULETTE = 1, 2, 3, 4, 5
 MODE_ANALOG, MODE_WEIGHTED = 0, 1
 
-EXPORTS = ("rt_create_grid", "rt_set_merge", "rt_set_mode", "rt_set_source", "rt_set_optics", "rt_set_slots", "rt_set_optics_slot", "rt_trace_batch", "rt_trace", "rt_trace_records", "rt_read_tallies",
+EXPORTS = ("rt_create_grid", "rt_set_merge", "rt_set_mode", "rt_set_source", "rt_set_optics", "rt_set_slots", "rt_set_optics_slot", "rt_trace_batch", "rt_trace", "rt_trace_records", "rt_read_tallies", "rt_read_tallies_async",
            "rt_reset_tallies", "rt_set_heating_split", "rt_read_heating_direct", "rt_tally_to_flux", "rt_read_majorant", "rt_read_packed_optics", "rt_gather_bench",
            "rt_last_trace_ms", "rt_launch_count", "rt_philox_words", "rt_last_error", "rt_destroy")
 
@@ -57,6 +57,7 @@ def lib():
     L.rt_trace.argtypes = [vp, f64, f64, u64, u64, u64, u32, vp]
     L.rt_trace_records.argtypes = [vp, f64, f64, u64, u64, u64, u32, vp, vp]
     L.rt_read_tallies.argtypes = [vp, vp, vp, vp, vp, vp, C.POINTER(rt_counters)]
+    L.rt_read_tallies_async.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
     L.rt_reset_tallies.argtypes = [vp, vp]
     L.rt_set_heating_split.argtypes = [vp, i32]
     L.rt_read_heating_direct.argtypes = [vp, vp]
@@ -98,6 +99,11 @@ class Tallies:
         return (int(self.atm_abs.sum()) + int(self.sfc_abs.sum()) + int(self.toa_up.sum())
                 + int(self.counters.capped_energy) + int(self.counters.roulette_lost)
                 - int(self.counters.roulette_gained))
+
+
+def counters_of(buf):
+    """rt_counters from the pinned byte buffer filled by Grid.read_tallies_async (after a stream sync)."""
+    return rt_counters.from_buffer_copy(bytes(buf.cpu().numpy().tobytes()))
 
 
 def tally_to_flux(tally, n_photons, ncol, tod_flux, depth=0.0):
@@ -222,6 +228,14 @@ class Grid:
         out = torch.empty((nz, ny, nx), dtype=torch.int64, device="cpu" if host else self.device)
         self._check(self.L.rt_read_heating_direct(self.ctx, _ptr(out)), "rt_read_heating_direct")
         return out
+
+    def read_tallies_async(self, out, counters_buf):
+        """rt_read_tallies_async into the (pinned) buffers of `out` (a Tallies; None fields are skipped) and
+        into `counters_buf`, a pinned uint8 tensor of ctypes.sizeof(rt_counters) bytes.  Valid after the current
+        stream has been synchronised; `counters_of(counters_buf)` then gives the rt_counters."""
+        self._check(self.L.rt_read_tallies_async(self.ctx, _ptr(out.atm_abs), _ptr(out.sfc_dir), _ptr(out.sfc_dif),
+                                                 _ptr(out.sfc_abs), _ptr(out.toa_up), _ptr(counters_buf),
+                                                 _stream(self.device)), "rt_read_tallies_async")
 
     def reset_tallies(self):
         self._check(self.L.rt_reset_tallies(self.ctx, _stream(self.device)), "rt_reset_tallies")

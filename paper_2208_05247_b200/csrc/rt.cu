@@ -20,6 +20,7 @@ struct rt_ctx {
   float merge_ratio = 1.25f;
   int n_slots = 1;                        // rt_set_slots: optics / majorant / albedo slots (spectral points)
   std::vector<char> slot_ok = std::vector<char>(1, 0);
+  rt_counters* d_counters = nullptr;      // rt_read_tallies_async: counters assembled on the device
   unsigned batch_calls = 0;
   unsigned long long* batch_tab = nullptr; // device: offsets (n_slots + 1) then nfull (n_slots), for rt_trace_batch
   int weighted = 0;                       // rt_set_mode: 0 analog absorption, 1 weights + roulette
@@ -403,6 +404,45 @@ int rt_read_tallies(rt_ctx* c, int64_t* atm_abs, int64_t* sfc_dir, int64_t* sfc_
   return RT_OK;
 }
 
+}  // extern "C" (reopened below)
+
+namespace {
+__global__ void assemble_counters_kernel(const unsigned long long* __restrict__ h, rt_counters* __restrict__ out) {
+  rt_counters r;
+  r.n_null = h[rt::C_NULL]; r.n_rayleigh = h[rt::C_RAY]; r.n_hg = h[rt::C_HG];
+  r.n_atm_abs = h[rt::C_ATM_ABS]; r.n_sfc_hits = h[rt::C_SFC_HITS];
+  r.n_sfc_abs = h[rt::C_SFC_ABS]; r.n_toa = h[rt::C_TOA]; r.n_capped = h[rt::C_CAPPED];
+  r.n_cell_steps = h[rt::C_CELLS]; r.n_relevel = h[rt::C_RELEVEL];
+  r.n_roulette_killed = h[rt::C_ROUL_KILLED]; r.n_roulette_kept = h[rt::C_ROUL_KEPT];
+  r.roulette_lost = (int64_t)h[rt::C_ROUL_LOST]; r.roulette_gained = (int64_t)h[rt::C_ROUL_GAINED];
+  r.capped_energy = (int64_t)h[rt::C_CAPPED_E];
+  r.n_events = h[rt::C_NULL] + h[rt::C_RAY] + h[rt::C_HG] + h[rt::C_ATM_ABS];
+  r.n_photons = h[rt::C_ATM_ABS] + h[rt::C_SFC_ABS] + h[rt::C_TOA] + h[rt::C_CAPPED] + h[rt::C_ROUL_KILLED];
+  *out = r;
+}
+}  // namespace
+
+extern "C" {
+
+int rt_read_tallies_async(rt_ctx* c, int64_t* atm_abs, int64_t* sfc_dir, int64_t* sfc_dif, int64_t* sfc_abs,
+                          int64_t* toa_up, rt_counters* counters, void* cuda_stream) {
+  if (!c) return RT_EINVAL;
+  DeviceGuard guard(c->device);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int64_t* outs[5] = {atm_abs, sfc_dir, sfc_dif, sfc_abs, toa_up};
+  for (int k = 0; k < 5; ++k)
+    if (outs[k])
+      RT_CUDA(c, cudaMemcpyAsync(outs[k], tally_ptr(c, k), (k == 0 ? c->nvox : c->ncol) * sizeof(int64_t), cudaMemcpyDefault, st));
+  if (counters) {
+    if (!c->d_counters) RT_CUDA(c, cudaMalloc(&c->d_counters, sizeof(rt_counters)));
+    assemble_counters_kernel<<<1, 1, 0, st>>>(c->counters, c->d_counters);
+    ++c->launches;
+    RT_CUDA(c, cudaMemcpyAsync(counters, c->d_counters, sizeof(rt_counters), cudaMemcpyDefault, st));
+  }
+  RT_CUDA(c, cudaGetLastError());
+  return RT_OK;
+}
+
 int rt_set_merge(rt_ctx* c, int mx, int my, int mz, float merge_ratio) {
   if (!c) return RT_EINVAL;
   auto pow2 = [](int v) { return v > 0 && !(v & (v - 1)); };
@@ -537,7 +577,7 @@ void rt_destroy(rt_ctx* c) {
     DeviceGuard guard(c->device);
     cudaDeviceSynchronize();
     cudaFree(c->optics); cudaFree(c->khat); cudaFree(c->kmin); cudaFree(c->atm_dir); cudaFree(c->albedo); cudaFree(c->tallies);
-    cudaFree(c->counters); cudaFree(c->bad); cudaFree(c->batch_tab); cudaFree(c->sink); cudaFree(c->stage);
+    cudaFree(c->counters); cudaFree(c->d_counters); cudaFree(c->bad); cudaFree(c->batch_tab); cudaFree(c->sink); cudaFree(c->stage);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
   }

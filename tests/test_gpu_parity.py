@@ -424,3 +424,25 @@ def test_random_small_configurations():
             assert np.array_equal(getattr(t, name).numpy(), getattr(o, name)), (name,) + tag
         assert np.array_equal(d, o.atm_abs_direct), tag
         assert t.counters.asdict() == o.counters.asdict() and t.closure() == n * rt.W0, tag
+
+
+def test_read_tallies_async_matches_synchronous_read():
+    rt = _rt()
+    import ctypes
+    cfg = CONFIGS[1]
+    opt = make_optics(cfg)
+    g = rt.Grid(*cfg.grid, device=0)
+    g.set_optics(opt["k_ext"], opt["k_ext_cloud"], opt["ssa"], opt["g"], opt["sfc_albedo"])
+    st = torch.cuda.Stream()
+    out = rt.Tallies(torch.empty((cfg.nz, cfg.ny, cfg.nx), dtype=torch.int64).pin_memory(),
+                     *[torch.empty((cfg.ny, cfg.nx), dtype=torch.int64).pin_memory() for _ in range(4)], counters=None)
+    cbuf = torch.zeros(ctypes.sizeof(rt.rt_counters), dtype=torch.uint8).pin_memory()
+    with torch.cuda.stream(st):
+        g.trace(cfg.zenith_deg, cfg.azimuth_deg, 1 << 16, seed=cfg.seed)
+        g.read_tallies_async(out, cbuf)
+    st.synchronize()
+    t = g.read_tallies()
+    for name in ("atm_abs", "sfc_dir", "sfc_dif", "sfc_abs", "toa_up"):
+        assert torch.equal(getattr(out, name), getattr(t, name)), name
+    assert rt.counters_of(cbuf).asdict() == t.counters.asdict() and t.counters.n_photons == 1 << 16
+    g.close()
