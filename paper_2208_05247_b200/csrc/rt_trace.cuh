@@ -30,7 +30,7 @@ constexpr float kTiny = 1e-30f;                 // direction components are nudg
 constexpr int kTraceThreads = 256;
 constexpr int kChunk = 128;                     // photon ids a warp takes per global atomic (fewer in small launches)
 #ifndef RT_MIN_BLOCKS
-#define RT_MIN_BLOCKS 3
+#define RT_MIN_BLOCKS 4
 #endif
 #ifndef RT_REGEN_BATCH
 #define RT_REGEN_BATCH 6
