@@ -45,7 +45,9 @@ extern "C" {
 #define RT_FATE_CAPPED 4
 #define RT_FATE_ROULETTE 5 /* weighted mode only */
 
-typedef struct rt_ctx rt_ctx; /* opaque; owned by the library; one CUDA device per context */
+typedef struct rt_ctx rt_ctx; /* opaque; owned by the library; one CUDA device per context.  The calls on one
+                                 context must be ordered (one stream, or streams synchronised by the caller):
+                                 its launches share a work counter.  Use one context per concurrent stream. */
 
 /* Always-on event counters, accumulated across rt_trace calls until rt_reset_tallies.
  * n_events = tentative collisions (null + real) = n_null + n_rayleigh + n_hg + n_atm_abs:
@@ -159,8 +161,7 @@ int rt_set_source(rt_ctx* ctx, float diffuse_fraction, int sampler);
  *   (full passes over the columns + remainder), i.e. exactly what rt_trace(..., counts[j], first_photon_id, seed,
  *   stream_id = j) on slot j's optics would trace; tallies accumulate.  records_out: NULL or 16 B per photon in
  *   the order of the points.  Reads the error mask and uploads the offsets before launching (waits for the
- *   stream once).  At most two rt_trace_batch launches of a context may be in flight (on different streams,
- *   e.g. the second half of the points packing while the first half traces).  Errors: RT_EINVAL, RT_ESTATE (a slot without optics), RT_EOPTICS, RT_ENOMEM, RT_ECUDA. */
+ *   stream once).  Errors: RT_EINVAL, RT_ESTATE (a slot without optics), RT_EOPTICS, RT_ENOMEM, RT_ECUDA. */
 int rt_set_slots(rt_ctx* ctx, int n_slots);
 int rt_set_optics_slot(rt_ctx* ctx, int slot, const float* k_ext, const float* k_ext_cloud, const float* ssa,
                        const float* g, const float* sfc_albedo, void* cuda_stream);

@@ -50,37 +50,14 @@ def spectral_sweep_overlapped(grids, streams, fields_of_point, counts, zenith_de
     return total
 
 
-def spectral_sweep_batched(grid, fields_of_point, counts, zenith_deg, azimuth_deg, seed=1, first_photon_id=0,
-                           streams=None):
+def spectral_sweep_batched(grid, fields_of_point, counts, zenith_deg, azimuth_deg, seed=1, first_photon_id=0):
     """The same sweep with every point's packed optics resident in its own HBM slot (`grid.set_slots(len(counts))`
-    beforehand; 16 B per voxel and point: 57 GB for config 4) and ONE launch per group of points
-    (rt_trace_batch): no launch drains between points and the host waits once per group, not once per point.
-    streams = two torch streams: the points are split in two halves, the second half's optics are packed
-    (HBM-bound) on the second stream while the first half traces (issue-bound) on the first.  Traces exactly
-    the photons of spectral_sweep (same ids, stream ids, column stratification): identical integer tallies."""
-    n = len(counts)
-    groups = [(0, n, None)] if not streams else [(0, n // 2, streams[0]), (n // 2, n, streams[1])]
-    if streams:
-        ready = torch.cuda.Event()
-        ready.record()
-    for lo, hi, st in groups:
-        if hi <= lo:
-            continue
-        if st is None:
-            for j in range(lo, hi):
-                grid.set_optics_slot(j, *fields_of_point(j))
-            grid.trace_batch(zenith_deg, azimuth_deg, counts[lo:hi], first_photon_id=first_photon_id, seed=seed,
-                             first_point=lo)
-        else:
-            st.wait_event(ready)
-            with torch.cuda.stream(st):
-                for j in range(lo, hi):
-                    grid.set_optics_slot(j, *fields_of_point(j))
-                grid.trace_batch(zenith_deg, azimuth_deg, counts[lo:hi], first_photon_id=first_photon_id, seed=seed,
-                                 first_point=lo)
-    if streams:
-        for st in streams:
-            torch.cuda.current_stream().wait_stream(st)
+    beforehand; 16 B per voxel and point: 57 GB for config 4) and ONE launch for all points (rt_trace_batch):
+    no launch drains between points and the host waits once, not once per point.  Traces exactly the photons of
+    spectral_sweep (same ids, stream ids, column stratification), so the integer tallies are identical."""
+    for j in range(len(counts)):
+        grid.set_optics_slot(j, *fields_of_point(j))
+    grid.trace_batch(zenith_deg, azimuth_deg, counts, first_photon_id=first_photon_id, seed=seed)
     return sum(int(x) for x in counts)
 
 

@@ -96,11 +96,10 @@ def test_config4_spectral_sweep():
     assert total3 == total and t3.counters.asdict() == c.asdict()
     for name in TALLIES:
         assert torch.equal(getattr(t3, name), getattr(t, name)), name
-    # ... in two halves on two streams (the second half packs while the first traces)
+    # ... and as two launches over the two halves of the points (first_point), one after the other
     g.reset_tallies()
-    spectral_sweep_batched(g, lambda j: [make_optics_torch(cfg, pts[j])[k] for k in NAMES], counts,
-                           cfg.zenith_deg, cfg.azimuth_deg, seed=cfg.seed, streams=streams)
-    torch.cuda.synchronize()
+    g.trace_batch(cfg.zenith_deg, cfg.azimuth_deg, counts[:50], seed=cfg.seed)
+    g.trace_batch(cfg.zenith_deg, cfg.azimuth_deg, counts[50:], seed=cfg.seed, first_point=50)
     t4 = g.read_tallies()
     assert t4.counters.asdict() == c.asdict()
     for name in TALLIES:
