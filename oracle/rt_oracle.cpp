@@ -13,9 +13,15 @@
 // optical properties fetched from the fine grid, Rayleigh / Henyey-
 // Greenstein scattering chosen with probability k_ext,cloud/k_ext,
 // Lambertian surface with local albedo, tallies of surface and
-// domain-top fluxes and 3D absorbed power.  Absorption is ANALOG
+// domain-top fluxes and 3D absorbed power.  By default absorption is ANALOG
 // (BASELINE.json north_star, reading D1): a photon ends in exactly one bin and
 // carries W0 = 2^32 integer quanta, so energy closes exactly in int64.
+// Options, each off by default and each with its own pins in tests/:
+//   merged acceleration cells (tests/test_oracle_merged_cells.py),
+//   the paper's absorption weights + Russian roulette (
+//     tests/test_oracle_weighted.py), with the direct part of the heating,
+//   the paper's top-of-domain source: scrambled Sobol entry points and a diffuse
+//     fraction (tests/test_oracle_source.py).
 //
 // Plain, slow, single-threaded by definition (n_threads > 1 only splits the
 // photon-id range for wall-clock timing; integer tallies make the result
