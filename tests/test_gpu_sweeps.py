@@ -161,21 +161,33 @@ def test_batched_points_equal_separate_traces():
     for k, opt in enumerate(opts):
         g.set_optics_slot(k, *[opt[n] for n in NAMES])
     first = (1 << 33) + 11
-    rec = g.trace_batch(cfg.zenith_deg, cfg.azimuth_deg, counts, first_photon_id=first, seed=cfg.seed,
-                        records=True).cpu().numpy().view(np.uint32)
-    t = g.read_tallies()
-    total = O.Tallies(cfg.nx, cfg.ny, cfg.nz)
-    off = 0
-    for k, (opt, n) in enumerate(zip(opts, counts)):
-        if n == 0:
-            continue
-        _, rec32, _ = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, first_photon_id=first, seed=cfg.seed,
-                              stream_id=k, precision=32, records=True, n_threads=8, tallies=total, **cfg.accel)
-        assert np.array_equal(rec[off:off + n], rec32), k
-        off += n
-    for name in TALLIES:
-        assert np.array_equal(getattr(t, name).numpy(), getattr(total, name)), name
-    assert t.counters.asdict() == total.counters.asdict() and t.closure() == sum(counts) * rt.W0
+    for weighted in (False, True):
+        g.reset_tallies()
+        g.set_mode(weighted)
+        rec = g.trace_batch(cfg.zenith_deg, cfg.azimuth_deg, counts, first_photon_id=first, seed=cfg.seed,
+                            records=True).cpu().numpy().view(np.uint32)
+        t = g.read_tallies()
+        total = O.Tallies(cfg.nx, cfg.ny, cfg.nz)
+        off = 0
+        for k, (opt, n) in enumerate(zip(opts, counts)):
+            if n == 0:
+                continue
+            _, rec32, _ = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, first_photon_id=first, seed=cfg.seed,
+                                  stream_id=k, precision=32, records=True, n_threads=8, tallies=total,
+                                  weighted=weighted, **cfg.accel)
+            assert np.array_equal(rec[off:off + n], rec32), (k, weighted)
+            off += n
+        for name in TALLIES:
+            assert np.array_equal(getattr(t, name).numpy(), getattr(total, name)), (name, weighted)
+        assert t.counters.asdict() == total.counters.asdict() and t.closure() == sum(counts) * rt.W0
+    # slot 0 is also what rt_set_optics / rt_trace use
+    g.set_mode(False)
+    g.reset_tallies()
+    g.set_optics(*[opts[2][n] for n in NAMES])
+    rec = g.trace(cfg.zenith_deg, cfg.azimuth_deg, 5000, seed=cfg.seed, stream_id=9, records=True).cpu().numpy().view(np.uint32)
+    _, rec32, _ = O.trace(cfg.grid, opts[2], cfg.zenith_deg, cfg.azimuth_deg, 5000, seed=cfg.seed, stream_id=9,
+                          precision=32, records=True, n_threads=8, **cfg.accel)
+    assert np.array_equal(rec, rec32)
     # errors: a slot without optics, a bad field reported at the batch trace
     g.set_slots(2)
     g.set_optics_slot(0, *[opts[0][n] for n in NAMES])
