@@ -270,6 +270,18 @@ def test_bad_inputs_fail_loudly():
     g.set_optics(opt["k_ext"], opt["k_ext_cloud"], opt["ssa"], opt["g"], opt["sfc_albedo"])
     with pytest.raises(rt.RtError):
         g.trace(95.0, 0.0, 16)
+    g.trace(30.0, 0.0, 16)
+    g.set_merge(2, 2, 2)                                # the majorant table must be rebuilt: optics again first
+    with pytest.raises(rt.RtError):
+        g.trace(30.0, 0.0, 16)
+    with pytest.raises(rt.RtError):
+        g.set_merge(3, 1, 1)                            # not a power of two
+    with pytest.raises(rt.RtError):
+        g.set_slots(0)
+    with pytest.raises(rt.RtError):
+        g.set_optics_slot(1, opt["k_ext"], opt["k_ext_cloud"], opt["ssa"], opt["g"], opt["sfc_albedo"])
+    with pytest.raises(rt.RtError):
+        g.trace_batch(30.0, 0.0, [4, 4])                # more points than slots
     g.close()
 
 
