@@ -252,17 +252,22 @@ int set_optics_impl(rt_ctx* c, int slot, const float* k_ext, const float* k_ext_
   float4* optics = c->optics + (size_t)slot * c->nvox;
   float* khat = c->khat + (size_t)slot * c->ncell;
   float* albedo = c->albedo + (size_t)slot * c->ncol;
+  const bool rows = (c->nx % 4 == 0) && !(((uintptr_t)k_ext | (uintptr_t)k_ext_cloud | (uintptr_t)ssa | (uintptr_t)g) & 15u);
+  const bool cellrows = rows && (c->bx == 1 || c->bx == 2 || c->bx == 4) && c->by * c->bz <= 64;   // no atomics, no zeroing
   if (sync) RT_CUDA(c, cudaMemsetAsync(c->bad, 0, sizeof(int), st));
-  RT_CUDA(c, cudaMemsetAsync(khat, 0, c->ncell * sizeof(float), st));
+  if (!cellrows) RT_CUDA(c, cudaMemsetAsync(khat, 0, c->ncell * sizeof(float), st));
   RT_CUDA(c, cudaMemcpyAsync(albedo, sfc_albedo, c->ncol * sizeof(float), cudaMemcpyDeviceToDevice, st));
   const int blocks = c->sm_count * 8;
   const bool merging = c->mx * c->my * c->mz > 1;
   if (merging) {
     if (!c->kmin) RT_CUDA(c, cudaMalloc(&c->kmin, c->ncell * sizeof(float)));
-    RT_CUDA(c, cudaMemsetAsync(c->kmin, 0x7f, c->ncell * sizeof(float), st));   // 0x7f7f7f7f: above any finite input's bits that matter (3.4e38)
+    if (!cellrows) RT_CUDA(c, cudaMemsetAsync(c->kmin, 0x7f, c->ncell * sizeof(float), st));   // 0x7f7f7f7f: above any finite input's bits that matter (3.4e38)
   }
-  const bool rows = (c->nx % 4 == 0) && !(((uintptr_t)k_ext | (uintptr_t)k_ext_cloud | (uintptr_t)ssa | (uintptr_t)g) & 15u);
-  if (rows)
+  if (cellrows)
+    rt::pack_optics_cellrows_kernel<<<c->sm_count * 16, 128, 0, st>>>(
+        (const float4*)k_ext, (const float4*)k_ext_cloud, (const float4*)ssa, (const float4*)g, optics,
+        khat, merging ? c->kmin : nullptr, c->nx, c->ny, c->nz, c->bx, c->by, c->bz, c->bad);
+  else if (rows)
     rt::pack_optics_rows_kernel<<<c->sm_count * 16, 128, 0, st>>>(
         (const float4*)k_ext, (const float4*)k_ext_cloud, (const float4*)ssa, (const float4*)g, optics,
         (int*)khat, merging ? (int*)c->kmin : nullptr, c->nx, c->ny, c->nz, c->bx, c->by, c->bz, c->bad);

@@ -123,6 +123,52 @@ __global__ void __launch_bounds__(128) pack_optics_rows_kernel(
   if (flags) atomicOr(bad, flags);
 }
 
+// The same step without atomics, for bx in {1, 2, 4} (and nx a multiple of 4): one block iteration handles a
+// whole ROW OF CELLS, i.e. the by x bz voxel rows that make up the cells (cy, cz) for all cx; a thread owns four
+// consecutive voxels in x (4 / bx cells) in every one of those rows, so it sees all voxels of its cells and
+// writes their maximum (and minimum) with plain stores: no atomics, no table to zero beforehand.
+__global__ void __launch_bounds__(128) pack_optics_cellrows_kernel(
+    const float4* __restrict__ k_ext, const float4* __restrict__ k_cloud, const float4* __restrict__ ssa,
+    const float4* __restrict__ g, float4* __restrict__ optics, float* __restrict__ khat, float* __restrict__ kmin,
+    int nx, int ny, int nz, int bx, int by, int bz, int* __restrict__ bad) {
+  const int ncx = nx / bx, ncy = ny / by, ncz = nz / bz, nx4 = nx >> 2;
+  const int cells_per_thread = 4 / bx;               // 4, 2 or 1
+  int flags = 0;
+  for (int cr = blockIdx.x; cr < ncy * ncz; cr += gridDim.x) {
+    const int cz = cr / ncy, cy = cr - cz * ncy;
+    for (int q = threadIdx.x; q < nx4; q += blockDim.x) {
+      float hi[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+      float lo[4] = {INFINITY, INFINITY, INFINITY, INFINITY};
+      for (int dz_ = 0; dz_ < bz; ++dz_)
+        for (int dy_ = 0; dy_ < by; ++dy_) {
+          const size_t base4 = ((size_t)(cz * bz + dz_) * ny + (size_t)(cy * by + dy_)) * nx4 + q;
+          const float4 K = __ldcs(k_ext + base4), KC = __ldcs(k_cloud + base4), W = __ldcs(ssa + base4),
+                       G = __ldcs(g + base4);
+          float4* out = optics + base4 * 4;
+          out[0] = pack_one(K.x, KC.x, W.x, G.x, flags);
+          out[1] = pack_one(K.y, KC.y, W.y, G.y, flags);
+          out[2] = pack_one(K.z, KC.z, W.z, G.z, flags);
+          out[3] = pack_one(K.w, KC.w, W.w, G.w, flags);
+          hi[0] = fmaxf(hi[0], K.x); hi[1] = fmaxf(hi[1], K.y); hi[2] = fmaxf(hi[2], K.z); hi[3] = fmaxf(hi[3], K.w);
+          lo[0] = fminf(lo[0], K.x); lo[1] = fminf(lo[1], K.y); lo[2] = fminf(lo[2], K.z); lo[3] = fminf(lo[3], K.w);
+        }
+      // per x position so far; now over the bx positions of each cell
+      const size_t cell0 = ((size_t)cz * ncy + cy) * ncx + (size_t)q * cells_per_thread;
+      if (bx == 1) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { khat[cell0 + j] = hi[j]; if (kmin) kmin[cell0 + j] = lo[j]; }
+      } else if (bx == 2) {
+        khat[cell0] = fmaxf(hi[0], hi[1]); khat[cell0 + 1] = fmaxf(hi[2], hi[3]);
+        if (kmin) { kmin[cell0] = fminf(lo[0], lo[1]); kmin[cell0 + 1] = fminf(lo[2], lo[3]); }
+      } else {
+        khat[cell0] = fmaxf(fmaxf(hi[0], hi[1]), fmaxf(hi[2], hi[3]));
+        if (kmin) kmin[cell0] = fminf(fminf(lo[0], lo[1]), fminf(lo[2], lo[3]));
+      }
+    }
+  }
+  if (flags) atomicOr(bad, flags);
+}
+
 // §3.5b merged cells.  One thread per block of mx x my x mz acceleration cells: if the block's highest
 // extinction is at most merge_ratio times its lowest (one fp32 multiply), every cell of the block stores
 // -(block maximum); the sign bit is what the trace kernel tests (set also for a maximum of 0).
