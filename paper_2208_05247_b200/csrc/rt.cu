@@ -279,7 +279,7 @@ int set_optics_impl(rt_ctx* c, int slot, const float* k_ext, const float* k_ext_
   c->launches += 2;
   if (merging) {
     const size_t nblk = c->ncell / ((size_t)c->mx * c->my * c->mz);
-    rt::merge_cells_kernel<<<(unsigned)((nblk + 127) / 128), 128, 0, st>>>(khat, c->kmin, c->ncx, c->ncy, c->ncz,
+    rt::merge_cells_kernel<<<(unsigned)((nblk * 32 + 127) / 128), 128, 0, st>>>(khat, c->kmin, c->ncx, c->ncy, c->ncz,
                                                                             c->mx, c->my, c->mz, c->merge_ratio);
     ++c->launches;
   }

@@ -169,29 +169,37 @@ __global__ void __launch_bounds__(128) pack_optics_cellrows_kernel(
   if (flags) atomicOr(bad, flags);
 }
 
-// §3.5b merged cells.  One thread per block of mx x my x mz acceleration cells: if the block's highest
-// extinction is at most merge_ratio times its lowest (one fp32 multiply), every cell of the block stores
-// -(block maximum); the sign bit is what the trace kernel tests (set also for a maximum of 0).
+// §3.5b merged cells.  One WARP per block of mx x my x mz acceleration cells (lanes stride over the block's
+// cells, x fastest): if the block's highest extinction is at most merge_ratio times its lowest (one fp32
+// multiply), every cell of the block stores -(block maximum); the sign bit is what the trace kernel tests
+// (set also for a maximum of 0).
 __global__ void merge_cells_kernel(float* __restrict__ khat, const float* __restrict__ kmin, int ncx, int ncy,
                                    int ncz, int mx, int my, int mz, float merge_ratio) {
   const int nbx = ncx / mx, nby = ncy / my, nbz = ncz / mz;
   const size_t nblk = (size_t)nbx * nby * nbz;
-  const size_t b = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (b >= nblk) return;
+  const size_t b = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (b >= nblk) return;                             // whole warps leave together
+  const unsigned lane = threadIdx.x & 31u;
   const int X = (int)(b % nbx), Y = (int)((b / nbx) % nby), Z = (int)(b / ((size_t)nbx * nby));
+  const int ncell = mx * my * mz;
   float hi = 0.0f, lo = INFINITY;
-  for (int z = Z * mz; z < (Z + 1) * mz; ++z)
-    for (int y = Y * my; y < (Y + 1) * my; ++y)
-      for (int x = X * mx; x < (X + 1) * mx; ++x) {
-        const size_t c = ((size_t)z * ncy + y) * ncx + x;
-        hi = fmaxf(hi, khat[c]);
-        lo = fminf(lo, kmin[c]);
-      }
+  for (int k = (int)lane; k < ncell; k += 32) {
+    const int x = X * mx + k % mx, y = Y * my + (k / mx) % my, z = Z * mz + k / (mx * my);
+    const size_t c = ((size_t)z * ncy + y) * ncx + x;
+    hi = fmaxf(hi, khat[c]);
+    lo = fminf(lo, kmin[c]);
+  }
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) {
+    hi = fmaxf(hi, __shfl_xor_sync(0xffffffffu, hi, off));
+    lo = fminf(lo, __shfl_xor_sync(0xffffffffu, lo, off));
+  }
   if (!(hi <= merge_ratio * lo)) return;
   const float v = -hi;
-  for (int z = Z * mz; z < (Z + 1) * mz; ++z)
-    for (int y = Y * my; y < (Y + 1) * my; ++y)
-      for (int x = X * mx; x < (X + 1) * mx; ++x) khat[((size_t)z * ncy + y) * ncx + x] = v;
+  for (int k = (int)lane; k < ncell; k += 32) {
+    const int x = X * mx + k % mx, y = Y * my + (k / mx) % my, z = Z * mz + k / (mx * my);
+    khat[((size_t)z * ncy + y) * ncx + x] = v;
+  }
 }
 
 __global__ void check_albedo_kernel(const float* __restrict__ albedo, size_t ncol, int* __restrict__ bad) {
