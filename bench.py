@@ -192,7 +192,17 @@ def run_ours(args):
         from paper_2208_05247_b200.sweeps import spectral_sweep_overlapped
         pts = spectral_points(112)
         counts = split_photons(n, [p["weight"] for p in pts])
-        resident = [[make_optics_torch(cfg, p, device=dev)[k] for k in names] for p in pts]
+        factored = not args.full_fields and args.contexts == 0
+        facs = None
+        if factored:
+            # FACTORED inputs (rt_set_optics_factored): one cloud field on the device + 2 nz numbers per point
+            from rt_inputs import factored_point
+            facs = [factored_point(cfg, p) for p in pts]
+            kc_dev = torch.from_numpy(facs[0]["k_cloud"]).to(dev)
+            al_dev = torch.from_numpy(facs[0]["sfc_albedo"]).to(dev)
+            resident = None
+        else:
+            resident = [[make_optics_torch(cfg, p, device=dev)[k] for k in names] for p in pts]
         pinned_all = None
         # two contexts on two streams, points alternating, so that one point's pack and trace fill the SMs the
         # previous point's draining persistent kernel frees; the integer tallies of the two are summed
@@ -221,7 +231,11 @@ def run_ours(args):
                 gx.reset_tallies()
             ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             ea.record()
-            if batched:
+            if batched and factored:
+                for j, f in enumerate(facs):                                        # 112 x (S0, S1) from the factors
+                    g.set_optics_factored(j, kc_dev, f["k_abs"], f["k_ray"], f["cloud_ssa"], f["cloud_g"], al_dev)
+                g.trace_batch(cfg.zenith_deg, cfg.azimuth_deg, counts, first_photon_id=first, seed=cfg.seed)
+            elif batched:
                 spectral_sweep_batched(g, lambda j: fields[j], counts, cfg.zenith_deg, cfg.azimuth_deg,
                                        seed=cfg.seed, first_photon_id=first)       # 112 x (S0, S1), one S2-S10 launch
             else:
@@ -294,6 +308,41 @@ def run_ours(args):
     # PCIe copies of every step are in the timed region but off the critical path.  Every step is checked after
     # the final synchronisation.  --e2e-serial keeps everything on one context and one stream.
     e2e = None
+    if spectral and factored and batched:
+        # spectral sweep end to end: the cloud field and the albedo come from pinned host memory every step, the
+        # gas profiles (2 nz numbers per point) from plain host arrays, all tallies go back to the host
+        import ctypes
+        kc_host = torch.from_numpy(facs[0]["k_cloud"]).pin_memory()
+        al_host = torch.from_numpy(facs[0]["sfc_albedo"]).pin_memory()
+        out_all = rt.Tallies(torch.empty((cfg.nz, cfg.ny, cfg.nx), dtype=torch.int64).pin_memory(),
+                             pinned_cols.sfc_dir, pinned_cols.sfc_dif, pinned_cols.sfc_abs, pinned_cols.toa_up,
+                             counters=None)
+
+        def e2e_sweep(i):
+            g.reset_tallies()
+            kc_dev.copy_(kc_host, non_blocking=True)
+            al_dev.copy_(al_host, non_blocking=True)
+            for j, f in enumerate(facs):
+                g.set_optics_factored(j, kc_dev, f["k_abs"], f["k_ray"], f["cloud_ssa"], f["cloud_g"], al_dev)
+            g.trace_batch(cfg.zenith_deg, cfg.azimuth_deg, counts, first_photon_id=weak_range(rank, world, i, n)[0],
+                          seed=cfg.seed)
+            t = g.read_tallies(out=out_all)
+            if t.counters.n_photons != n or t.counters.n_capped != 0:
+                raise SystemExit("bench.py: e2e photon count mismatch (%d of %d)" % (t.counters.n_photons, n))
+
+        e2e_sweep(0)
+        barrier()
+        t0 = time.perf_counter()
+        for i in range(args.steps):
+            e2e_sweep(args.warmup + args.steps + i)
+        barrier()
+        e2e_s = max_over_ranks(time.perf_counter() - t0)
+        h2d = kc_host.numel() * 4 + al_host.numel() * 4 + len(facs) * 2 * cfg.nz * 4
+        d2h = (cfg.nvox + 4 * cfg.ncol) * 8 + ctypes.sizeof(rt.rt_counters)
+        e2e = {"value": total_photons / e2e_s, "unit": UNIT, "ms_per_step": 1e3 * e2e_s / args.steps,
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+               "how": "factored inputs: cloud field + albedo from pinned host memory, 112 x 2 nz profile values; "
+                      "all tallies to pinned host memory; one context, synchronous read"}
     if not spectral:
         import ctypes
         h2d = sum(x.numel() * x.element_size() for x in host)
@@ -408,14 +457,14 @@ def run_ours(args):
         "trace_kernel": {"ms": ms_avg, "paths_per_s": n / (ms_avg * 1e-3), "events_per_s": trace_events_per_s},
         "config": {"workload": cfg.name, "grid": [cfg.nx, cfg.ny, cfg.nz], "photons_per_gpu_per_step": n,
                    "block": list(cfg.block), "merge": list(cfg.merge), "merge_ratio": cfg.merge_ratio,
-                   "mode": args.mode,
+                   "mode": args.mode, "factored_inputs": bool(spectral and not args.full_fields and args.contexts == 0),
                    "zenith_deg": cfg.zenith_deg, "azimuth_deg": cfg.azimuth_deg,
                    "parallelism": "photon-id ranges per GPU, no collective" if world > 1 else "1 GPU",
                    "l2": ("inputs exceed L2 (%d MiB packed optics + %d MiB tallies vs 126 MB)" % (
                        cfg.nvox * 16 >> 20, cfg.nvox * 8 >> 20)) if cfg.nvox * 24 > (126 << 20) else
                          "inputs fit L2; every step traces new photon ids",
-                   "step": ("reset_tallies + 112 x set_optics_slot + one trace_batch launch (stream_id = point) + "
-                            "read_tallies" if spectral and args.contexts == 0 else
+                   "step": ("reset_tallies + 112 x set_optics_factored (or set_optics_slot with --full-fields) + one "
+                            "trace_batch launch (stream_id = point) + read_tallies" if spectral and args.contexts == 0 else
                             "reset_tallies + 112 x (set_optics + trace, stream_id = point; points alternating over "
                             "--contexts contexts and streams) + read_tallies of all"
                             if spectral else
@@ -462,6 +511,9 @@ def main():
                     help="workload 4: 0 (default) = all points' optics in HBM slots and one launch (rt_trace_batch); "
                          "N >= 1 = one rt_trace per point, points alternating over N contexts on N streams")
     ap.add_argument("--merge", default=None, help="merged-cell factors mx,my,mz (default: the config's; 1,1,1 = off)")
+    ap.add_argument("--full-fields", action="store_true",
+                    help="workload 4: give every point's optics as four full 3-D fields (rt_set_optics_slot) instead of "
+                         "as factors (one cloud field + per-level gas profiles per point, rt_set_optics_factored)")
     ap.add_argument("--e2e-serial", action="store_true", help="e2e leg on one context with synchronous copies")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing (used under ncu)")
     args = ap.parse_args()

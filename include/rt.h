@@ -165,6 +165,17 @@ int rt_set_source(rt_ctx* ctx, float diffuse_fraction, int sampler);
 int rt_set_slots(rt_ctx* ctx, int n_slots);
 int rt_set_optics_slot(rt_ctx* ctx, int slot, const float* k_ext, const float* k_ext_cloud, const float* ssa,
                        const float* g, const float* sfc_albedo, void* cuda_stream);
+/* rt_set_optics_slot from FACTORED inputs (per spectral point the gas part of the optics depends on height
+ * only; NEXT-3 of SURVEY.md §8(f)).  Per voxel at level z, in fp32 and in this order:
+ *   k_ext = (k_abs[z] + k_ray[z]) + k_cloud;  ssa = (k_ray[z] + cloud_ssa * k_cloud) / k_ext (0 if k_ext = 0);
+ *   k_ext_cloud = k_cloud;  g = cloud_g;  then packing and majorant exactly as rt_set_optics.
+ * k_cloud ([z][y][x], nvox) and sfc_albedo (ncol) are DEVICE pointers (the cloud field is shared by all points
+ * and uploaded once); k_abs, k_ray (nz each) may be HOST or DEVICE.  Reads 4 B per voxel instead of 16 and
+ * needs 2 nz numbers per point from the host.  Asynchronous like rt_set_optics_slot (errors of the field values
+ * at the next rt_trace_batch).  Requires nx % 4 == 0, bx in {1, 2, 4}, by * bz <= 64.  Errors: RT_EINVAL,
+ * RT_EOPTICS (cloud_ssa, cloud_g out of range), RT_ENOMEM, RT_ECUDA. */
+int rt_set_optics_factored(rt_ctx* ctx, int slot, const float* k_cloud, const float* k_abs, const float* k_ray,
+                           float cloud_ssa, float cloud_g, const float* sfc_albedo, void* cuda_stream);
 int rt_trace_batch(rt_ctx* ctx, double zenith_deg, double azimuth_deg, int first_point, int n_points,
                    const uint64_t* counts, uint64_t first_photon_id, uint64_t seed, void* cuda_stream,
                    uint32_t* records_out);

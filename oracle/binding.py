@@ -186,5 +186,20 @@ def sobol2(k):
     return x1, x2
 
 
+def assemble_factored(k_cloud, k_abs, k_ray, cloud_ssa, cloud_g):
+    """the four optical fields of a spectral point from its factors, in fp32 and in this
+    order: k_ext = (k_abs[z] + k_ray[z]) + k_cloud; ssa = (k_ray[z] + cloud_ssa * k_cloud) / k_ext (0 where
+    k_ext = 0); k_ext_cloud = k_cloud; g = cloud_g.  Every numpy operation below is one IEEE fp32 operation."""
+    kc = np.ascontiguousarray(k_cloud, dtype=np.float32)
+    ka = np.asarray(k_abs, dtype=np.float32).reshape(-1, 1, 1)
+    kr = np.asarray(k_ray, dtype=np.float32).reshape(-1, 1, 1)
+    k_ext = (ka + kr) + kc
+    num = kr + np.float32(cloud_ssa) * kc
+    with np.errstate(divide="ignore", invalid="ignore"):
+        ssa = np.where(k_ext > 0, num / k_ext, np.float32(0)).astype(np.float32)
+    assert k_ext.dtype == np.float32 and num.dtype == np.float32
+    return {"k_ext": k_ext, "k_ext_cloud": kc, "ssa": ssa, "g": np.full(kc.shape, np.float32(cloud_g), dtype=np.float32)}
+
+
 def hardware_threads():
     return int(lib().orc_hardware_threads())

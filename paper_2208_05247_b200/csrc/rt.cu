@@ -21,6 +21,7 @@ struct rt_ctx {
   int n_slots = 1;                        // rt_set_slots: optics / majorant / albedo slots (spectral points)
   std::vector<char> slot_ok = std::vector<char>(1, 0);
   rt_counters* d_counters = nullptr;      // rt_read_tallies_async: counters assembled on the device
+  float* gas_tab = nullptr;               // rt_set_optics_factored: per slot k_abs[nz] then k_ray[nz] (device)
   unsigned batch_calls = 0;
   unsigned long long* batch_tab = nullptr; // device: offsets (n_slots + 1) then nfull (n_slots), for rt_trace_batch
   int weighted = 0;                       // rt_set_mode: 0 analog absorption, 1 weights + roulette
@@ -317,8 +318,8 @@ int rt_set_slots(rt_ctx* c, int n_slots) {
     return fail(c, RT_EINVAL, "rt_set_slots: need 1 <= n_slots and n_slots * nvox < 2^32");
   DeviceGuard guard(c->device);
   RT_CUDA(c, cudaDeviceSynchronize());
-  cudaFree(c->optics); cudaFree(c->khat); cudaFree(c->albedo); cudaFree(c->batch_tab);
-  c->optics = nullptr; c->khat = nullptr; c->albedo = nullptr; c->batch_tab = nullptr;
+  cudaFree(c->optics); cudaFree(c->khat); cudaFree(c->albedo); cudaFree(c->batch_tab); cudaFree(c->gas_tab);
+  c->optics = nullptr; c->khat = nullptr; c->albedo = nullptr; c->batch_tab = nullptr; c->gas_tab = nullptr;
   c->have_optics = false;
   c->n_slots = n_slots;
   c->slot_ok.assign((size_t)n_slots, 0);
@@ -336,6 +337,52 @@ int rt_set_optics_slot(rt_ctx* c, int slot, const float* k_ext, const float* k_e
   if (slot < 0 || slot >= c->n_slots) return fail(c, RT_EINVAL, "rt_set_optics_slot: slot out of range (rt_set_slots)");
   return set_optics_impl(c, slot, k_ext, k_ext_cloud, ssa, g, sfc_albedo, (cudaStream_t)cuda_stream, false,
                          "rt_set_optics_slot");
+}
+
+int rt_set_optics_factored(rt_ctx* c, int slot, const float* k_cloud, const float* k_abs, const float* k_ray,
+                           float cloud_ssa, float cloud_g, const float* sfc_albedo, void* cuda_stream) {
+  if (!c) return RT_EINVAL;
+  if (slot < 0 || slot >= c->n_slots) return fail(c, RT_EINVAL, "rt_set_optics_factored: slot out of range (rt_set_slots)");
+  if (!k_cloud || !k_abs || !k_ray || !sfc_albedo) return fail(c, RT_EINVAL, "rt_set_optics_factored: NULL argument");
+  if (c->nx % 4 || !(c->bx == 1 || c->bx == 2 || c->bx == 4) || c->by * c->bz > 64 || ((uintptr_t)k_cloud & 15u))
+    return fail(c, RT_EINVAL, "rt_set_optics_factored: needs nx % 4 == 0, bx in {1, 2, 4}, by * bz <= 64, 16-byte aligned k_cloud");
+  if (!(cloud_ssa >= 0.0f && cloud_ssa <= 1.0f) || !(std::fabs(cloud_g) < 1.0f))
+    return fail(c, RT_EOPTICS, "rt_set_optics_factored: cloud_ssa must be in [0, 1] and |cloud_g| < 1");
+  DeviceGuard guard(c->device);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  for (const void* p : {(const void*)k_cloud, (const void*)sfc_albedo}) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess || !(at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged)) {
+      cudaGetLastError();
+      return fail(c, RT_EINVAL, "rt_set_optics_factored: k_cloud and sfc_albedo must be device pointers");
+    }
+  }
+  c->slot_ok[slot] = 0;
+  if (slot == 0) c->have_optics = false;
+  if (!c->gas_tab) RT_CUDA(c, cudaMalloc(&c->gas_tab, (size_t)c->n_slots * 2 * c->nz * sizeof(float)));
+  float* tab = c->gas_tab + (size_t)slot * 2 * c->nz;
+  RT_CUDA(c, cudaMemcpyAsync(tab, k_abs, c->nz * sizeof(float), cudaMemcpyDefault, st));
+  RT_CUDA(c, cudaMemcpyAsync(tab + c->nz, k_ray, c->nz * sizeof(float), cudaMemcpyDefault, st));
+  float4* optics = c->optics + (size_t)slot * c->nvox;
+  float* khat = c->khat + (size_t)slot * c->ncell;
+  float* albedo = c->albedo + (size_t)slot * c->ncol;
+  RT_CUDA(c, cudaMemcpyAsync(albedo, sfc_albedo, c->ncol * sizeof(float), cudaMemcpyDeviceToDevice, st));
+  const bool merging = c->mx * c->my * c->mz > 1;
+  if (merging && !c->kmin) RT_CUDA(c, cudaMalloc(&c->kmin, c->ncell * sizeof(float)));
+  rt::pack_factored_cellrows_kernel<<<c->sm_count * 16, 128, 0, st>>>(
+      (const float4*)k_cloud, tab, tab + c->nz, cloud_ssa, cloud_g, optics, khat, merging ? c->kmin : nullptr,
+      c->nx, c->ny, c->nz, c->bx, c->by, c->bz, c->bad);
+  rt::check_albedo_kernel<<<c->sm_count, 256, 0, st>>>(albedo, c->ncol, c->bad);
+  c->launches += 2;
+  if (merging) {
+    const size_t nblk = c->ncell / ((size_t)c->mx * c->my * c->mz);
+    rt::merge_cells_kernel<<<(unsigned)((nblk * 32 + 127) / 128), 128, 0, st>>>(khat, c->kmin, c->ncx, c->ncy, c->ncz,
+                                                                                 c->mx, c->my, c->mz, c->merge_ratio);
+    ++c->launches;
+  }
+  RT_CUDA(c, cudaGetLastError());
+  c->slot_ok[slot] = 1;
+  return RT_OK;
 }
 
 int rt_trace_batch(rt_ctx* c, double zenith_deg, double azimuth_deg, int first_point, int n_points,
@@ -582,7 +629,7 @@ void rt_destroy(rt_ctx* c) {
     DeviceGuard guard(c->device);
     cudaDeviceSynchronize();
     cudaFree(c->optics); cudaFree(c->khat); cudaFree(c->kmin); cudaFree(c->atm_dir); cudaFree(c->albedo); cudaFree(c->tallies);
-    cudaFree(c->counters); cudaFree(c->d_counters); cudaFree(c->bad); cudaFree(c->batch_tab); cudaFree(c->sink); cudaFree(c->stage);
+    cudaFree(c->counters); cudaFree(c->d_counters); cudaFree(c->bad); cudaFree(c->gas_tab); cudaFree(c->batch_tab); cudaFree(c->sink); cudaFree(c->stage);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
   }

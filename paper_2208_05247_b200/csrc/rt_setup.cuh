@@ -169,6 +169,59 @@ __global__ void __launch_bounds__(128) pack_optics_cellrows_kernel(
   if (flags) atomicOr(bad, flags);
 }
 
+// Factored inputs (the optical properties of a spectral point are a gas part that
+// depends on height only plus the cloud part): per voxel, in fp32 and in this order,
+//   k_ext = (k_abs[z] + k_ray[z]) + k_cloud;  ssa = (k_ray[z] + cloud_ssa * k_cloud) / k_ext (0 if k_ext = 0);
+//   g = cloud_g;  then the packing of §3.4.  Same cell-row scheme as above, reading 4 B per voxel instead of 16.
+__global__ void __launch_bounds__(128) pack_factored_cellrows_kernel(
+    const float4* __restrict__ k_cloud, const float* __restrict__ k_abs, const float* __restrict__ k_ray,
+    float cloud_ssa, float cloud_g, float4* __restrict__ optics, float* __restrict__ khat, float* __restrict__ kmin,
+    int nx, int ny, int nz, int bx, int by, int bz, int* __restrict__ bad) {
+  const int ncx = nx / bx, ncy = ny / by, ncz = nz / bz, nx4 = nx >> 2;
+  const int cells_per_thread = 4 / bx;
+  int flags = 0;
+  for (int cr = blockIdx.x; cr < ncy * ncz; cr += gridDim.x) {
+    const int cz = cr / ncy, cy = cr - cz * ncy;
+    for (int q = threadIdx.x; q < nx4; q += blockDim.x) {
+      float hi[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+      float lo[4] = {INFINITY, INFINITY, INFINITY, INFINITY};
+      for (int dz_ = 0; dz_ < bz; ++dz_) {
+        const int z = cz * bz + dz_;
+        const float ka = __ldg(k_abs + z), kr = __ldg(k_ray + z);
+        const float kg = ka + kr;
+        if (!(ka >= 0.0f) || !(kr >= 0.0f) || isinf(kg)) flags |= 1;
+        for (int dy_ = 0; dy_ < by; ++dy_) {
+          const size_t base4 = ((size_t)z * ny + (size_t)(cy * by + dy_)) * nx4 + q;
+          const float4 KC = __ldcs(k_cloud + base4);
+          const float kc[4] = {KC.x, KC.y, KC.z, KC.w};
+          float4* out = optics + base4 * 4;
+          float k[4];
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            k[j] = kg + kc[j];
+            const float w = (k[j] > 0.0f) ? (kr + cloud_ssa * kc[j]) / k[j] : 0.0f;
+            out[j] = pack_one(k[j], kc[j], w, cloud_g, flags);
+          }
+          hi[0] = fmaxf(hi[0], k[0]); hi[1] = fmaxf(hi[1], k[1]); hi[2] = fmaxf(hi[2], k[2]); hi[3] = fmaxf(hi[3], k[3]);
+          lo[0] = fminf(lo[0], k[0]); lo[1] = fminf(lo[1], k[1]); lo[2] = fminf(lo[2], k[2]); lo[3] = fminf(lo[3], k[3]);
+        }
+      }
+      const size_t cell0 = ((size_t)cz * ncy + cy) * ncx + (size_t)q * cells_per_thread;
+      if (bx == 1) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { khat[cell0 + j] = hi[j]; if (kmin) kmin[cell0 + j] = lo[j]; }
+      } else if (bx == 2) {
+        khat[cell0] = fmaxf(hi[0], hi[1]); khat[cell0 + 1] = fmaxf(hi[2], hi[3]);
+        if (kmin) { kmin[cell0] = fminf(lo[0], lo[1]); kmin[cell0 + 1] = fminf(lo[2], lo[3]); }
+      } else {
+        khat[cell0] = fmaxf(fmaxf(hi[0], hi[1]), fmaxf(hi[2], hi[3]));
+        if (kmin) kmin[cell0] = fminf(fminf(lo[0], lo[1]), fminf(lo[2], lo[3]));
+      }
+    }
+  }
+  if (flags) atomicOr(bad, flags);
+}
+
 // §3.5b merged cells.  One WARP per block of mx x my x mz acceleration cells (lanes stride over the block's
 // cells, x fastest): if the block's highest extinction is at most merge_ratio times its lowest (one fp32
 // multiply), every cell of the block stores -(block maximum); the sign bit is what the trace kernel tests

@@ -5,5 +5,5 @@ no packing, no majorant): it only produces the optical-property fields, surface 
 and run parameters that stand in for the paper's LES cumulus fields (PAPER.md P:40-44,
 P:60), which are not available.  Recipe: DESIGN.md §4; configurations: BASELINE.json.
 """
-from .fields import (CONFIGS, Config, make_optics, make_optics_torch, spectral_points, split_photons,  # noqa: F401
+from .fields import (CONFIGS, Config, make_optics, make_optics_torch, factored_point, spectral_points, split_photons,  # noqa: F401
                      plane_parallel)

@@ -150,6 +150,21 @@ def make_optics(cfg: Config, spectral=None):
                      spectral["cloud_g"])
 
 
+def factored_point(cfg: Config, spectral=None):
+    """The same spectral point as make_optics(cfg, spectral), as FACTORS: cloud extinction field (fp32, shared by
+    all points) and per-level gas absorption / Rayleigh profiles (fp32), cloud single-scattering albedo and g."""
+    key = (cfg.nx, cfg.ny, cfg.nz, cfg.dx, cfg.dy, cfg.dz, cfg.n_blobs, cfg.name.startswith("tiny_box"))
+    if key not in _cloud_cache:
+        make_optics(cfg)
+    p = spectral or {"k_abs0": cfg.k_abs0, "k_ray0": cfg.k_ray0, "cloud_ssa": cfg.cloud_ssa, "cloud_g": cfg.cloud_g}
+    zc = (np.arange(cfg.nz) + 0.5) * cfg.dz
+    prof = np.ones(cfg.nz) if cfg.name.startswith("tiny_box") else np.exp(-zc / SCALE_HEIGHT)
+    return {"k_cloud": _cloud_cache[key].astype(np.float32), "k_abs": (p["k_abs0"] * prof).astype(np.float32),
+            "k_ray": (p["k_ray0"] * prof).astype(np.float32), "cloud_ssa": float(np.float32(p["cloud_ssa"])),
+            "cloud_g": float(np.float32(p["cloud_g"])),
+            "sfc_albedo": np.full((cfg.ny, cfg.nx), cfg.sfc_albedo, dtype=np.float32)}
+
+
 def spectral_points(n=112):
     """Config 4: n spectral points, 0.2-4 um log-spaced; gas absorption log-uniform 1e-7..1e-3 1/m,
     Rayleigh ~ lambda^-4, cloud ssa 0.9999 -> 0.9 and g 0.86 -> 0.80; weight = Planck(5772 K) * dlambda

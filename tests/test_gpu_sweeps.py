@@ -199,3 +199,50 @@ def test_batched_points_equal_separate_traces():
     with pytest.raises(rt.RtError):
         g.trace_batch(cfg.zenith_deg, cfg.azimuth_deg, [10, 10])
     g.close()
+
+
+def test_factored_optics_slots():
+    """rt_set_optics_factored: packed optics and majorant table bit-identical to the oracle's
+    packing of the fields assembled from the factors; a batched trace over factored slots identical to the oracle
+    on those fields; bad factors are refused."""
+    rt = _rt()
+    from dataclasses import replace
+    from rt_inputs import factored_point
+    cfg = replace(CONFIGS[2], block=(2, 2, 2), merge=(8, 8, 4))
+    pts = spectral_points(112)
+    sel = (0, 58, 111)
+    g = rt.Grid(*cfg.grid, device=0, **cfg.accel)
+    g.set_slots(len(sel))
+    facs = [factored_point(cfg, pts[j]) for j in sel]
+    kc_dev = torch.from_numpy(facs[0]["k_cloud"]).cuda()
+    al_dev = torch.from_numpy(facs[0]["sfc_albedo"]).cuda()
+    fields = []
+    for k, f in enumerate(facs):
+        g.set_optics_factored(k, kc_dev, f["k_abs"], f["k_ray"], f["cloud_ssa"], f["cloud_g"], al_dev)
+        asm = O.assemble_factored(f["k_cloud"], f["k_abs"], f["k_ray"], f["cloud_ssa"], f["cloud_g"])
+        asm["sfc_albedo"] = f["sfc_albedo"]
+        fields.append(asm)
+    packed = g.read_packed_optics().numpy().reshape(-1, 4)           # slot 0
+    want = O.pack_optics_f32(fields[0]["k_ext"], fields[0]["k_ext_cloud"], fields[0]["ssa"], fields[0]["g"])
+    assert np.array_equal(packed.view(np.uint32), want.view(np.uint32))
+    kh = g.read_majorant().numpy()
+    assert np.array_equal(kh.view(np.uint32), O.majorant(cfg.nx, cfg.ny, cfg.nz, *cfg.block, fields[0]["k_ext"],
+                                                         **cfg.accel).view(np.uint32))
+    counts = [cfg.ncol + 99, 4000, cfg.ncol * 2]
+    rec = g.trace_batch(cfg.zenith_deg, cfg.azimuth_deg, counts, seed=cfg.seed, records=True).cpu().numpy().view(np.uint32)
+    t = g.read_tallies()
+    total = O.Tallies(cfg.nx, cfg.ny, cfg.nz)
+    off = 0
+    for k, (opt, n) in enumerate(zip(fields, counts)):
+        _, rec32, _ = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed, stream_id=k,
+                              precision=32, records=True, n_threads=8, tallies=total, **cfg.accel)
+        assert np.array_equal(rec[off:off + n], rec32), k
+        off += n
+    for name in TALLIES:
+        assert np.array_equal(getattr(t, name).numpy(), getattr(total, name)), name
+    assert t.counters.asdict() == total.counters.asdict()
+    with pytest.raises(rt.RtError):
+        g.set_optics_factored(0, kc_dev, facs[0]["k_abs"], facs[0]["k_ray"], 1.5, 0.8, al_dev)
+    with pytest.raises(rt.RtError):
+        g.set_optics_factored(0, facs[0]["k_cloud"], facs[0]["k_abs"], facs[0]["k_ray"], 0.9, 0.8, al_dev)   # host field
+    g.close()

@@ -52,3 +52,21 @@ def test_spectral_points_and_photon_split():
     counts = split_photons(n, w)
     assert sum(counts) == n and all(abs(c - n * x) < 1 for c, x in zip(counts, w))
     assert split_photons(7, [1, 1, 1]) == [3, 2, 2] and split_photons(0, [1, 2]) == [0, 0]
+
+
+def test_factored_point_is_the_same_point():
+    """The factored form of a spectral point (cloud field + gas profiles, assembled in fp32 by DESIGN.md §3.4b)
+    describes the same optics as the full fields of make_optics (assembled in fp64, rounded once): equal to
+    fp32 rounding."""
+    import oracle as O
+    from rt_inputs import factored_point
+    cfg = CONFIGS[2]
+    p = spectral_points(112)[60]
+    full = make_optics(cfg, p)
+    f = factored_point(cfg, p)
+    asm = O.assemble_factored(f["k_cloud"], f["k_abs"], f["k_ray"], f["cloud_ssa"], f["cloud_g"])
+    assert np.array_equal(asm["k_ext_cloud"], full["k_ext_cloud"]) and np.array_equal(asm["g"], full["g"])
+    for k in ("k_ext", "ssa"):
+        rel = np.abs(asm[k].astype(np.float64) - full[k]) / np.maximum(np.abs(full[k]), 1e-30)
+        assert rel.max() < 4e-7, (k, rel.max())
+    assert np.array_equal(f["sfc_albedo"], full["sfc_albedo"])
