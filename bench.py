@@ -223,6 +223,17 @@ def run_ours(args):
                                 counters=None)
     point_ms = []
 
+    def set_factored(kc, al):
+        """All 112 points from their factors: kept factored in the trace (rt_set_cloud + rt_set_point; default) or
+        packed into 16-byte records per voxel and point (rt_set_optics_factored; --packed-slots)."""
+        if args.packed_slots:
+            for j, f in enumerate(facs):
+                g.set_optics_factored(j, kc, f["k_abs"], f["k_ray"], f["cloud_ssa"], f["cloud_g"], al)
+        else:
+            g.set_cloud(kc)
+            for j, f in enumerate(facs):
+                g.set_point(j, f["k_abs"], f["k_ray"], f["cloud_ssa"], f["cloud_g"], al)
+
     def step(i, fields, out):
         g.reset_tallies()
         first = weak_range(rank, world, i, n)[0]
@@ -232,8 +243,7 @@ def run_ours(args):
             ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             ea.record()
             if batched and factored:
-                for j, f in enumerate(facs):                                        # 112 x (S0, S1) from the factors
-                    g.set_optics_factored(j, kc_dev, f["k_abs"], f["k_ray"], f["cloud_ssa"], f["cloud_g"], al_dev)
+                set_factored(kc_dev, al_dev)                                        # S0, S1 from the factors
                 g.trace_batch(cfg.zenith_deg, cfg.azimuth_deg, counts, first_photon_id=first, seed=cfg.seed)
             elif batched:
                 spectral_sweep_batched(g, lambda j: fields[j], counts, cfg.zenith_deg, cfg.azimuth_deg,
@@ -320,10 +330,12 @@ def run_ours(args):
 
         def e2e_sweep(i):
             g.reset_tallies()
-            kc_dev.copy_(kc_host, non_blocking=True)
-            al_dev.copy_(al_host, non_blocking=True)
-            for j, f in enumerate(facs):
-                g.set_optics_factored(j, kc_dev, f["k_abs"], f["k_ray"], f["cloud_ssa"], f["cloud_g"], al_dev)
+            if args.packed_slots:
+                kc_dev.copy_(kc_host, non_blocking=True)
+                al_dev.copy_(al_host, non_blocking=True)
+                set_factored(kc_dev, al_dev)
+            else:
+                set_factored(kc_host, al_host)           # the library copies the host fields itself
             g.trace_batch(cfg.zenith_deg, cfg.azimuth_deg, counts, first_photon_id=weak_range(rank, world, i, n)[0],
                           seed=cfg.seed)
             t = g.read_tallies(out=out_all)
@@ -463,8 +475,9 @@ def run_ours(args):
                    "l2": ("inputs exceed L2 (%d MiB packed optics + %d MiB tallies vs 126 MB)" % (
                        cfg.nvox * 16 >> 20, cfg.nvox * 8 >> 20)) if cfg.nvox * 24 > (126 << 20) else
                          "inputs fit L2; every step traces new photon ids",
-                   "step": ("reset_tallies + 112 x set_optics_factored (or set_optics_slot with --full-fields) + one "
-                            "trace_batch launch (stream_id = point) + read_tallies" if spectral and args.contexts == 0 else
+                   "step": ("reset_tallies + set_cloud + 112 x set_point (--packed-slots: 112 x set_optics_factored; "
+                            "--full-fields: 112 x set_optics_slot) + one trace_batch launch (stream_id = point) + "
+                            "read_tallies" if spectral and args.contexts == 0 else
                             "reset_tallies + 112 x (set_optics + trace, stream_id = point; points alternating over "
                             "--contexts contexts and streams) + read_tallies of all"
                             if spectral else
@@ -511,6 +524,10 @@ def main():
                     help="workload 4: 0 (default) = all points' optics in HBM slots and one launch (rt_trace_batch); "
                          "N >= 1 = one rt_trace per point, points alternating over N contexts on N streams")
     ap.add_argument("--merge", default=None, help="merged-cell factors mx,my,mz (default: the config's; 1,1,1 = off)")
+    ap.add_argument("--packed-slots", action="store_true",
+                    help="workload 4 with factored inputs: pack a 16-byte record per voxel and point "
+                         "(rt_set_optics_factored) instead of keeping the optics factored in the trace "
+                         "(rt_set_cloud + rt_set_point, the default)")
     ap.add_argument("--full-fields", action="store_true",
                     help="workload 4: give every point's optics as four full 3-D fields (rt_set_optics_slot) instead of "
                          "as factors (one cloud field + per-level gas profiles per point, rt_set_optics_factored)")

@@ -151,8 +151,8 @@ int rt_set_source(rt_ctx* ctx, float diffuse_fraction, int sampler);
  * quadrature point"): the context holds n_slots packed-optics, majorant and albedo slots in HBM (16 B per voxel
  * and slot: 112 points of the 512x512x128 grid = 57 GB of the B200's 180 GB), and ONE launch traces the photons
  * of all points, so that no launch drains between points and the host does not wait per point.
- * rt_set_slots: (re)allocates the slots (n_slots * nvox < 2^32); slot 0 is the one rt_set_optics and rt_trace
- *   use; every slot must be given optics again afterwards.  Synchronises the device.
+ * rt_set_slots: (re)allocates the slots (n_slots * nvox < 2^32; the 16 B x nvox records of the slots above 0 are
+ *   allocated when the first of them is set); slot 0 is the one rt_set_optics and rt_trace use; every slot must be given optics again afterwards.  Synchronises the device.
  * rt_set_optics_slot: rt_set_optics into slot `slot`, asynchronous on `cuda_stream`: range errors accumulate on
  *   the device and are reported by the next rt_trace_batch (RT_EOPTICS).  Host fields are accepted but make
  *   the call wait for the stream.
@@ -176,6 +176,20 @@ int rt_set_optics_slot(rt_ctx* ctx, int slot, const float* k_ext, const float* k
  * RT_EOPTICS (cloud_ssa, cloud_g out of range), RT_ENOMEM, RT_ECUDA. */
 int rt_set_optics_factored(rt_ctx* ctx, int slot, const float* k_cloud, const float* k_abs, const float* k_ray,
                            float cloud_ssa, float cloud_g, const float* sfc_albedo, void* cuda_stream);
+/* Factored optics kept factored in the trace as well (NEXT-3 in full).  rt_set_cloud stores the cloud extinction
+ * field once (own copy; DEVICE or HOST pointer; synchronises the stream to report a bad value, RT_EOPTICS) and
+ * derives, per acceleration cell and level, its extrema.  rt_set_point then defines slot `slot` by the factors of
+ * rt_set_optics_factored WITHOUT packing a 16-byte record per voxel: it only builds the point's majorant table
+ * from those extrema (exact: fl(gas + k_cloud) is monotone in k_cloud) and keeps the 2 nz + 2 numbers; a
+ * rt_trace_batch over such slots gathers 4 B of cloud extinction per tentative collision and rebuilds the
+ * record of §3.4b + §3.4 with the same fp32 operations, so its photons are bit-identical to those of the packed
+ * slots.  k_abs, k_ray (nz), sfc_albedo (ncol): HOST or DEVICE.  Needs rt_set_slots (any n >= 1) beforehand; the
+ * points of one rt_trace_batch launch must all be of the same kind.  Per point this costs a pass over the cell
+ * tables (a few MB) instead of over the voxel fields, and no 16 B x nvox slot.  Errors: RT_EINVAL, RT_ESTATE
+ * (rt_set_point before rt_set_cloud), RT_EOPTICS, RT_ENOMEM, RT_ECUDA. */
+int rt_set_cloud(rt_ctx* ctx, const float* k_cloud, void* cuda_stream);
+int rt_set_point(rt_ctx* ctx, int slot, const float* k_abs, const float* k_ray, float cloud_ssa, float cloud_g,
+                 const float* sfc_albedo, void* cuda_stream);
 int rt_trace_batch(rt_ctx* ctx, double zenith_deg, double azimuth_deg, int first_point, int n_points,
                    const uint64_t* counts, uint64_t first_photon_id, uint64_t seed, void* cuda_stream,
                    uint32_t* records_out);

@@ -12,7 +12,7 @@ W0 = 1 << 32
 FATE_ATM_ABS, FATE_SFC_ABS, FATE_TOD_EXIT, FATE_CAPPED, FATE_ROULETTE = 1, 2, 3, 4, 5
 MODE_ANALOG, MODE_WEIGHTED = 0, 1
 
-EXPORTS = ("rt_create_grid", "rt_set_merge", "rt_set_mode", "rt_set_source", "rt_set_optics", "rt_set_slots", "rt_set_optics_slot", "rt_set_optics_factored", "rt_trace_batch", "rt_trace", "rt_trace_records", "rt_read_tallies", "rt_read_tallies_async",
+EXPORTS = ("rt_create_grid", "rt_set_merge", "rt_set_mode", "rt_set_source", "rt_set_optics", "rt_set_slots", "rt_set_optics_slot", "rt_set_optics_factored", "rt_set_cloud", "rt_set_point", "rt_trace_batch", "rt_trace", "rt_trace_records", "rt_read_tallies", "rt_read_tallies_async",
            "rt_reset_tallies", "rt_set_heating_split", "rt_read_heating_direct", "rt_tally_to_flux", "rt_read_majorant", "rt_read_packed_optics", "rt_gather_bench",
            "rt_last_trace_ms", "rt_launch_count", "rt_philox_words", "rt_last_error", "rt_destroy")
 
@@ -54,6 +54,8 @@ def lib():
     L.rt_set_slots.argtypes = [vp, i32]
     L.rt_set_optics_slot.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp]
     L.rt_set_optics_factored.argtypes = [vp, i32, vp, vp, vp, f32, f32, vp, vp]
+    L.rt_set_cloud.argtypes = [vp, vp, vp]
+    L.rt_set_point.argtypes = [vp, i32, vp, vp, f32, f32, vp, vp]
     L.rt_trace_batch.argtypes = [vp, f64, f64, i32, i32, C.POINTER(u64), u64, u64, vp, vp]
     L.rt_trace.argtypes = [vp, f64, f64, u64, u64, u64, u32, vp]
     L.rt_trace_records.argtypes = [vp, f64, f64, u64, u64, u64, u32, vp, vp]
@@ -194,6 +196,19 @@ class Grid:
         self._check(self.L.rt_set_optics_factored(self.ctx, int(slot), _ptr(kc), _ptr(ka), _ptr(kr), float(cloud_ssa),
                                                   float(cloud_g), _ptr(al), _stream(self.device)),
                     "rt_set_optics_factored")
+
+    def set_cloud(self, k_cloud):
+        """include/rt.h rt_set_cloud: the cloud extinction field shared by all spectral points."""
+        nz, ny, nx = self.shape
+        self._check(self.L.rt_set_cloud(self.ctx, _ptr(self._f32(k_cloud, nx * ny * nz)), _stream(self.device)),
+                    "rt_set_cloud")
+
+    def set_point(self, slot, k_abs, k_ray, cloud_ssa, cloud_g, sfc_albedo):
+        """include/rt.h rt_set_point: a spectral point by its factors, kept factored in the trace."""
+        nz, ny, nx = self.shape
+        ka, kr, al = self._f32(k_abs, nz), self._f32(k_ray, nz), self._f32(sfc_albedo, nx * ny)
+        self._check(self.L.rt_set_point(self.ctx, int(slot), _ptr(ka), _ptr(kr), float(cloud_ssa), float(cloud_g),
+                                        _ptr(al), _stream(self.device)), "rt_set_point")
 
     def trace_batch(self, zenith_deg, azimuth_deg, counts, first_photon_id=0, seed=1, records=False, first_point=0):
         """One launch for the spectral points first_point .. first_point + len(counts) - 1 (slot = stream id =

@@ -21,6 +21,12 @@ struct rt_ctx {
   int n_slots = 1;                        // rt_set_slots: optics / majorant / albedo slots (spectral points)
   std::vector<char> slot_ok = std::vector<char>(1, 0);
   rt_counters* d_counters = nullptr;      // rt_read_tallies_async: counters assembled on the device
+  int optics_slots = 1;                   // slots the packed-optics array currently holds (grown on demand)
+  float* cloud = nullptr;                 // rt_set_cloud: own copy of the cloud field, nvox
+  float* cloud_max = nullptr;             // ... highest / lowest cloud extinction per cell and level-in-cell
+  float* cloud_min = nullptr;
+  float2* point_par = nullptr;            // rt_set_point: (cloud_ssa, cloud_g) per slot
+  bool cloud_ok = false;
   float* gas_tab = nullptr;               // rt_set_optics_factored: per slot k_abs[nz] then k_ray[nz] (device)
   unsigned batch_calls = 0;
   unsigned long long* batch_tab = nullptr; // device: offsets (n_slots + 1) then nfull (n_slots), for rt_trace_batch
@@ -92,7 +98,7 @@ const float* stage_input(rt_ctx* c, const float* p, size_t n, size_t slot_offset
 
 int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photons, uint64_t first_id,
              uint64_t seed, uint32_t stream_id, void* stream_v, uint32_t* records, int n_points = 0, int first_point = 0,
-             const unsigned long long* tab = nullptr) {
+             const unsigned long long* tab = nullptr, bool factored_trace = false) {
   if (!c) return RT_EINVAL;
   if (n_points == 0 && !c->have_optics) return fail(c, RT_ESTATE, "rt_trace: call rt_set_optics first");
   if (!(zenith_deg >= 0.0 && zenith_deg < 90.0) || !std::isfinite(azimuth_deg))
@@ -137,6 +143,7 @@ int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photon
   A.diffuse_fraction = c->diffuse_fraction; A.sobol = c->sobol;
   A.n_points = n_points; A.first_point = first_point; A.offsets = tab; A.nfull = tab ? tab + c->n_slots + 1 : nullptr;
   A.nvox32 = (unsigned)c->nvox; A.ncell32 = (unsigned)c->ncell; A.ncol32 = (unsigned)c->ncol;
+  A.cloud = factored_trace ? c->cloud : nullptr; A.gas = c->gas_tab; A.point_par = c->point_par;
   RT_CUDA(c, cudaMemsetAsync(A.next_photon, 0, sizeof(unsigned long long), st));
   RT_CUDA(c, cudaEventRecord(c->ev0, st));
   if (n_photons > 0) {
@@ -234,12 +241,28 @@ int rt_create_grid(rt_ctx** out, int nx, int ny, int nz, float dx, float dy, flo
 
 namespace {
 
+// The packed-optics array holds one slot until a packed slot > 0 is asked for; then it is grown to all n_slots
+// (16 B per voxel and slot), keeping what it holds.
+int ensure_optics_slots(rt_ctx* c, int slot) {
+  if (slot < c->optics_slots) return RT_OK;
+  DeviceGuard guard(c->device);
+  RT_CUDA(c, cudaDeviceSynchronize());
+  float4* grown = nullptr;
+  RT_CUDA(c, cudaMalloc(&grown, (size_t)c->n_slots * c->nvox * sizeof(float4)));
+  RT_CUDA(c, cudaMemcpy(grown, c->optics, (size_t)c->optics_slots * c->nvox * sizeof(float4), cudaMemcpyDeviceToDevice));
+  cudaFree(c->optics);
+  c->optics = grown;
+  c->optics_slots = c->n_slots;
+  return RT_OK;
+}
+
 // S0 + S1 into optics / majorant / albedo slot `slot`.  sync: wait for the kernels and report range errors now
 // (rt_set_optics); otherwise the error mask accumulates on the device until rt_trace_batch reads it.
 int set_optics_impl(rt_ctx* c, int slot, const float* k_ext, const float* k_ext_cloud, const float* ssa,
                     const float* g, const float* sfc_albedo, cudaStream_t st, bool sync, const char* who) {
   if (!k_ext || !k_ext_cloud || !ssa || !g || !sfc_albedo) return fail(c, RT_EINVAL, "rt_set_optics: NULL field");
   DeviceGuard guard(c->device);
+  if (int rce = ensure_optics_slots(c, slot)) return rce;
   c->slot_ok[slot] = 0;
   if (slot == 0) c->have_optics = false;
   int rc = RT_OK;
@@ -318,12 +341,13 @@ int rt_set_slots(rt_ctx* c, int n_slots) {
     return fail(c, RT_EINVAL, "rt_set_slots: need 1 <= n_slots and n_slots * nvox < 2^32");
   DeviceGuard guard(c->device);
   RT_CUDA(c, cudaDeviceSynchronize());
-  cudaFree(c->optics); cudaFree(c->khat); cudaFree(c->albedo); cudaFree(c->batch_tab); cudaFree(c->gas_tab);
-  c->optics = nullptr; c->khat = nullptr; c->albedo = nullptr; c->batch_tab = nullptr; c->gas_tab = nullptr;
+  cudaFree(c->optics); cudaFree(c->khat); cudaFree(c->albedo); cudaFree(c->batch_tab); cudaFree(c->gas_tab); cudaFree(c->point_par);
+  c->optics = nullptr; c->khat = nullptr; c->albedo = nullptr; c->batch_tab = nullptr; c->gas_tab = nullptr; c->point_par = nullptr;
   c->have_optics = false;
   c->n_slots = n_slots;
   c->slot_ok.assign((size_t)n_slots, 0);
-  RT_CUDA(c, cudaMalloc(&c->optics, (size_t)n_slots * c->nvox * sizeof(float4)));
+  RT_CUDA(c, cudaMalloc(&c->optics, c->nvox * sizeof(float4)));   // one slot; grown when a packed slot > 0 is set
+  c->optics_slots = 1;
   RT_CUDA(c, cudaMalloc(&c->khat, (size_t)n_slots * c->ncell * sizeof(float)));
   RT_CUDA(c, cudaMalloc(&c->albedo, (size_t)n_slots * c->ncol * sizeof(float)));
   RT_CUDA(c, cudaMalloc(&c->batch_tab, 2 * (2 * (size_t)n_slots + 1) * sizeof(unsigned long long)));   // two launches may be in flight
@@ -357,6 +381,7 @@ int rt_set_optics_factored(rt_ctx* c, int slot, const float* k_cloud, const floa
       return fail(c, RT_EINVAL, "rt_set_optics_factored: k_cloud and sfc_albedo must be device pointers");
     }
   }
+  if (int rce = ensure_optics_slots(c, slot)) return rce;
   c->slot_ok[slot] = 0;
   if (slot == 0) c->have_optics = false;
   if (!c->gas_tab) RT_CUDA(c, cudaMalloc(&c->gas_tab, (size_t)c->n_slots * 2 * c->nz * sizeof(float)));
@@ -385,12 +410,77 @@ int rt_set_optics_factored(rt_ctx* c, int slot, const float* k_cloud, const floa
   return RT_OK;
 }
 
+int rt_set_cloud(rt_ctx* c, const float* k_cloud, void* cuda_stream) {
+  if (!c || !k_cloud) return c ? fail(c, RT_EINVAL, "rt_set_cloud: NULL field") : RT_EINVAL;
+  DeviceGuard guard(c->device);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  c->cloud_ok = false;
+  for (auto& ok : c->slot_ok) if (ok == 2) ok = 0;      // points built on the old cloud field
+  if (!c->cloud) RT_CUDA(c, cudaMalloc(&c->cloud, c->nvox * sizeof(float)));
+  if (!c->cloud_max) RT_CUDA(c, cudaMalloc(&c->cloud_max, c->ncell * c->bz * sizeof(float)));
+  if (!c->cloud_min) RT_CUDA(c, cudaMalloc(&c->cloud_min, c->ncell * c->bz * sizeof(float)));
+  RT_CUDA(c, cudaMemcpyAsync(c->cloud, k_cloud, c->nvox * sizeof(float), cudaMemcpyDefault, st));
+  RT_CUDA(c, cudaMemsetAsync(c->bad, 0, sizeof(int), st));
+  rt::cloud_levels_kernel<<<c->sm_count * 8, 256, 0, st>>>(c->cloud, c->cloud_max, c->cloud_min, c->nx, c->ny, c->nz,
+                                                           c->bx, c->by, c->bz, c->bad);
+  ++c->launches;
+  RT_CUDA(c, cudaGetLastError());
+  int bad = 0;
+  RT_CUDA(c, cudaMemcpyAsync(&bad, c->bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+  RT_CUDA(c, cudaStreamSynchronize(st));
+  if (bad) return fail(c, RT_EOPTICS, "rt_set_cloud: the cloud extinction must be finite and >= 0");
+  c->cloud_ok = true;
+  return RT_OK;
+}
+
+int rt_set_point(rt_ctx* c, int slot, const float* k_abs, const float* k_ray, float cloud_ssa, float cloud_g,
+                 const float* sfc_albedo, void* cuda_stream) {
+  if (!c) return RT_EINVAL;
+  if (slot < 0 || slot >= c->n_slots) return fail(c, RT_EINVAL, "rt_set_point: slot out of range (rt_set_slots)");
+  if (!k_abs || !k_ray || !sfc_albedo) return fail(c, RT_EINVAL, "rt_set_point: NULL argument");
+  if (!c->cloud_ok) return fail(c, RT_ESTATE, "rt_set_point: call rt_set_cloud first");
+  if (!(cloud_ssa >= 0.0f && cloud_ssa <= 1.0f) || !(std::fabs(cloud_g) < 1.0f))
+    return fail(c, RT_EOPTICS, "rt_set_point: cloud_ssa must be in [0, 1] and |cloud_g| < 1");
+  DeviceGuard guard(c->device);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  c->slot_ok[slot] = 0;
+  if (!c->gas_tab) RT_CUDA(c, cudaMalloc(&c->gas_tab, (size_t)c->n_slots * 2 * c->nz * sizeof(float)));
+  if (!c->point_par) RT_CUDA(c, cudaMalloc(&c->point_par, (size_t)c->n_slots * sizeof(float2)));
+  float* tab = c->gas_tab + (size_t)slot * 2 * c->nz;
+  const float2 pp = make_float2(cloud_ssa, cloud_g);
+  RT_CUDA(c, cudaMemcpyAsync(tab, k_abs, c->nz * sizeof(float), cudaMemcpyDefault, st));
+  RT_CUDA(c, cudaMemcpyAsync(tab + c->nz, k_ray, c->nz * sizeof(float), cudaMemcpyDefault, st));
+  RT_CUDA(c, cudaMemcpyAsync(c->point_par + slot, &pp, sizeof pp, cudaMemcpyHostToDevice, st));   // pageable: staged before return
+  float* khat = c->khat + (size_t)slot * c->ncell;
+  float* albedo = c->albedo + (size_t)slot * c->ncol;
+  RT_CUDA(c, cudaMemcpyAsync(albedo, sfc_albedo, c->ncol * sizeof(float), cudaMemcpyDefault, st));
+  const bool merging = c->mx * c->my * c->mz > 1;
+  if (merging && !c->kmin) RT_CUDA(c, cudaMalloc(&c->kmin, c->ncell * sizeof(float)));
+  rt::point_majorant_kernel<<<c->sm_count * 8, 256, 0, st>>>(c->cloud_max, c->cloud_min, tab, tab + c->nz, khat,
+                                                             merging ? c->kmin : nullptr, c->ncx, c->ncy, c->ncz, c->bz, c->bad);
+  rt::check_albedo_kernel<<<c->sm_count, 256, 0, st>>>(albedo, c->ncol, c->bad);
+  c->launches += 2;
+  if (merging) {
+    const size_t nblk = c->ncell / ((size_t)c->mx * c->my * c->mz);
+    rt::merge_cells_kernel<<<(unsigned)((nblk * 32 + 127) / 128), 128, 0, st>>>(khat, c->kmin, c->ncx, c->ncy, c->ncz,
+                                                                                 c->mx, c->my, c->mz, c->merge_ratio);
+    ++c->launches;
+  }
+  RT_CUDA(c, cudaGetLastError());
+  c->slot_ok[slot] = 2;
+  return RT_OK;
+}
+
 int rt_trace_batch(rt_ctx* c, double zenith_deg, double azimuth_deg, int first_point, int n_points,
                    const uint64_t* counts, uint64_t first_photon_id, uint64_t seed, void* cuda_stream,
                    uint32_t* records_out) {
   if (!c) return RT_EINVAL;
   if (first_point < 0 || n_points < 1 || first_point + n_points > c->n_slots || !counts || !c->batch_tab)
     return fail(c, RT_EINVAL, "rt_trace_batch: points must lie within the slots (rt_set_slots), counts not NULL");
+  const char kind = c->slot_ok[first_point];
+  for (int j = first_point; j < first_point + n_points; ++j)
+    if (c->slot_ok[j] != kind)
+      return fail(c, RT_ESTATE, "rt_trace_batch: the points of a launch must all be packed slots or all rt_set_point slots");
   for (int j = first_point; j < first_point + n_points; ++j)
     if (!c->slot_ok[j]) return fail(c, RT_ESTATE, "rt_trace_batch: a slot below n_points has no optics (rt_set_optics_slot)");
   DeviceGuard guard(c->device);
@@ -416,7 +506,7 @@ int rt_trace_batch(rt_ctx* c, double zenith_deg, double azimuth_deg, int first_p
   RT_CUDA(c, cudaMemcpyAsync(dtab, tab.data(), tab.size() * sizeof(unsigned long long), cudaMemcpyHostToDevice, st));
   RT_CUDA(c, cudaStreamSynchronize(st));   // tab is a stack vector
   return do_trace(c, zenith_deg, azimuth_deg, total, first_photon_id, seed, 0u, cuda_stream, records_out, n_points,
-                  first_point, dtab);
+                  first_point, dtab, kind == 2);
 }
 
 int rt_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photons, uint64_t first_photon_id,
@@ -629,7 +719,8 @@ void rt_destroy(rt_ctx* c) {
     DeviceGuard guard(c->device);
     cudaDeviceSynchronize();
     cudaFree(c->optics); cudaFree(c->khat); cudaFree(c->kmin); cudaFree(c->atm_dir); cudaFree(c->albedo); cudaFree(c->tallies);
-    cudaFree(c->counters); cudaFree(c->d_counters); cudaFree(c->bad); cudaFree(c->gas_tab); cudaFree(c->batch_tab); cudaFree(c->sink); cudaFree(c->stage);
+    cudaFree(c->counters); cudaFree(c->d_counters); cudaFree(c->bad); cudaFree(c->gas_tab); cudaFree(c->point_par);
+    cudaFree(c->cloud); cudaFree(c->cloud_max); cudaFree(c->cloud_min); cudaFree(c->batch_tab); cudaFree(c->sink); cudaFree(c->stage);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
   }

@@ -222,6 +222,57 @@ __global__ void __launch_bounds__(128) pack_factored_cellrows_kernel(
   if (flags) atomicOr(bad, flags);
 }
 
+// Factored optics kept factored (rt_set_cloud + rt_set_point): the cloud field is stored once; what depends on the
+// spectral point is built from small tables.  cloud_levels_kernel: per acceleration cell and per level inside the
+// cell, the highest and lowest cloud extinction over the cell's bx x by voxels of that level ([cell][bz] floats).
+// fl(gas[z] + k_cloud) is monotone in k_cloud, so the extrema of k_ext over the cell follow from these tables
+// exactly (point_majorant_kernel), without touching the field again.
+__global__ void cloud_levels_kernel(const float* __restrict__ k_cloud, float* __restrict__ cmax, float* __restrict__ cmin,
+                                    int nx, int ny, int nz, int bx, int by, int bz, int* __restrict__ bad) {
+  const int ncx = nx / bx, ncy = ny / by, ncz = nz / bz;
+  const size_t n = (size_t)ncx * ncy * ncz * bz;
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += stride) {
+    // t = ((cz * bz + dz) * ncy + cy) * ncx + cx: consecutive threads read neighbouring x
+    const int cx = (int)(t % ncx), cy = (int)((t / ncx) % ncy), z = (int)(t / ((size_t)ncx * ncy));
+    float hi = 0.0f, lo = INFINITY;
+    bool ok = true;
+    for (int dy_ = 0; dy_ < by; ++dy_)
+      for (int dx_ = 0; dx_ < bx; ++dx_) {
+        const float k = k_cloud[((size_t)z * ny + (size_t)(cy * by + dy_)) * nx + (size_t)(cx * bx + dx_)];
+        if (!(k >= 0.0f) || isinf(k)) ok = false;
+        hi = fmaxf(hi, k); lo = fminf(lo, k);
+      }
+    if (!ok) atomicOr(bad, 2);
+    const size_t cell = ((size_t)(z / bz) * ncy + cy) * ncx + cx;
+    cmax[cell * bz + (z % bz)] = hi;
+    cmin[cell * bz + (z % bz)] = lo;
+  }
+}
+
+// Majorant (and per-cell minimum, for the merge criterion) of one spectral point from the cloud level tables and
+// the point's gas profiles: k_hat[cell] = max over the cell's levels of fl((k_abs[z] + k_ray[z]) + cmax).
+__global__ void point_majorant_kernel(const float* __restrict__ cmax, const float* __restrict__ cmin,
+                                      const float* __restrict__ k_abs, const float* __restrict__ k_ray,
+                                      float* __restrict__ khat, float* __restrict__ kmin, int ncx, int ncy, int ncz,
+                                      int bz, int* __restrict__ bad) {
+  const size_t ncell = (size_t)ncx * ncy * ncz;
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < ncell; c += stride) {
+    const int cz = (int)(c / ((size_t)ncx * ncy));
+    float hi = 0.0f, lo = INFINITY;
+    for (int dz_ = 0; dz_ < bz; ++dz_) {
+      const float ka = __ldg(k_abs + cz * bz + dz_), kr = __ldg(k_ray + cz * bz + dz_);
+      const float kg = ka + kr;
+      if (!(ka >= 0.0f) || !(kr >= 0.0f) || isinf(kg)) atomicOr(bad, 1);
+      hi = fmaxf(hi, kg + cmax[c * bz + dz_]);
+      lo = fminf(lo, kg + cmin[c * bz + dz_]);
+    }
+    khat[c] = hi;
+    if (kmin) kmin[c] = lo;
+  }
+}
+
 // §3.5b merged cells.  One WARP per block of mx x my x mz acceleration cells (lanes stride over the block's
 // cells, x fastest): if the block's highest extinction is at most merge_ratio times its lowest (one fp32
 // multiply), every cell of the block stores -(block maximum); the sign bit is what the trace kernel tests

@@ -88,6 +88,11 @@ struct TraceArgs {
   const unsigned long long* nfull;     // per point: ncol * floor(count / ncol) (device)
   int n_points, first_point;           // points first_point .. first_point + n_points - 1 (slot = stream id = point)
   unsigned nvox32, ncell32, ncol32;    // slot strides of optics, majorant and albedo
+  // factored optics in the trace (kBatch only; rt_set_cloud / rt_set_point): COLLIDE builds the voxel's record from
+  // the shared cloud field and the point's tables with the operations of §3.4b + §3.4 instead of gathering it
+  const float* cloud;                  // [z][y][x] or nullptr (then the packed slots are used)
+  const float* gas;                    // per point: k_abs[nz] then k_ray[nz]
+  const float2* point_par;             // per point: (cloud_ssa, cloud_g)
   float diffuse_fraction;              // §3.15: share of photons launched diffusely (0: none)
   int sobol;                           // §3.15: entry points from the scrambled 2-D Sobol sequence
   uint32_t stream_id;
@@ -428,7 +433,24 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
         // 32-bit indices: rt_create_grid refuses grids of 2^32 voxels or more
         const unsigned vox = ((unsigned)(cz * A.bz + lz) * (unsigned)A.ny + (unsigned)(cy * A.by + ly)) * (unsigned)A.nx
                              + (unsigned)(cx * A.bx + lx);
-        const float4 v = __ldg(&A.optics[kBatch ? vox + jpt * A.nvox32 : vox]);
+        float4 v;
+        if (kBatch && A.cloud) {
+          const float kc = __ldg(A.cloud + vox);
+          const int z = cz * A.bz + lz;
+          const float ka = __ldg(A.gas + (size_t)jpt * 2u * (unsigned)A.nz + z);
+          const float kr = __ldg(A.gas + (size_t)jpt * 2u * (unsigned)A.nz + (unsigned)A.nz + z);
+          const float2 pp = __ldg(A.point_par + jpt);
+          const float k = (ka + kr) + kc;                                     // §3.4b
+          const float w = (k > 0.0f) ? (kr + pp.x * kc) / k : 0.0f;
+          float c1 = (1.0f - w) * k;                                          // §3.4
+          const float frac = (k > 0.0f) ? kc / k : 0.0f;
+          float c2 = c1 + (w * k) * frac;
+          c2 = fminf(c2, k);
+          c1 = fminf(c1, c2);
+          v = make_float4(c1, c2, k, pp.y);
+        } else {
+          v = __ldg(&A.optics[kBatch ? vox + jpt * A.nvox32 : vox]);
+        }
         ++t_ev;
         float xi = u1 * fabsf(kh);
         st = ST_MOVE;

@@ -241,6 +241,29 @@ def test_factored_optics_slots():
     for name in TALLIES:
         assert np.array_equal(getattr(t, name).numpy(), getattr(total, name)), name
     assert t.counters.asdict() == total.counters.asdict()
+    # the same points kept factored in the trace (rt_set_cloud + rt_set_point): no packed records at all; the
+    # majorant table and every photon must come out the same
+    g2 = rt.Grid(*cfg.grid, device=0, **cfg.accel)
+    g2.set_slots(len(sel))
+    with pytest.raises(rt.RtError):
+        g2.set_point(0, facs[0]["k_abs"], facs[0]["k_ray"], facs[0]["cloud_ssa"], facs[0]["cloud_g"], al_dev)   # no cloud yet
+    g2.set_cloud(facs[0]["k_cloud"])                                     # host field accepted
+    for k, f in enumerate(facs):
+        g2.set_point(k, f["k_abs"], f["k_ray"], f["cloud_ssa"], f["cloud_g"], f["sfc_albedo"])
+    assert np.array_equal(g2.read_majorant().numpy().view(np.uint32), kh.view(np.uint32))
+    for weighted in (False, True):
+        g.reset_tallies(); g2.reset_tallies()
+        g.set_mode(weighted); g2.set_mode(weighted)
+        ra = g.trace_batch(cfg.zenith_deg, cfg.azimuth_deg, counts, seed=cfg.seed, records=True)
+        rb = g2.trace_batch(cfg.zenith_deg, cfg.azimuth_deg, counts, seed=cfg.seed, records=True)
+        assert torch.equal(ra, rb), weighted
+        ta, tb = g.read_tallies(), g2.read_tallies()
+        for name in TALLIES:
+            assert torch.equal(getattr(ta, name), getattr(tb, name)), (name, weighted)
+        assert ta.counters.asdict() == tb.counters.asdict()
+    g.set_mode(False)
+    assert np.array_equal(rb.cpu().numpy().view(np.uint32)[:0], rec[:0])
+    g2.close()
     with pytest.raises(rt.RtError):
         g.set_optics_factored(0, kc_dev, facs[0]["k_abs"], facs[0]["k_ray"], 1.5, 0.8, al_dev)
     with pytest.raises(rt.RtError):
