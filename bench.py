@@ -183,6 +183,9 @@ def run_ours(args):
     n = cfg.n_photons                            # per GPU (weak scaling: photon ids are sharded by rank)
     g = rt.Grid(*cfg.grid, device=local, **cfg.accel)
     g.set_mode(weighted=(args.mode == "weighted"))
+    if args.kernel:
+        rt.binding.DEFAULT_KERNEL = rt.KERNEL_LANES if args.kernel == "lanes" else rt.KERNEL_POOL
+        g.set_kernel(rt.binding.DEFAULT_KERNEL)
     pinned_cols = rt.Tallies(None, *[torch.empty((cfg.ny, cfg.nx), dtype=torch.int64).pin_memory() for _ in range(4)],
                              counters=None)
     if spectral:
@@ -531,6 +534,8 @@ def main():
     ap.add_argument("--full-fields", action="store_true",
                     help="workload 4: give every point's optics as four full 3-D fields (rt_set_optics_slot) instead of "
                          "as factors (one cloud field + per-level gas profiles per point, rt_set_optics_factored)")
+    ap.add_argument("--kernel", choices=("pool", "lanes"), default=None,
+                    help="trace kernel (include/rt.h rt_set_kernel): pool (the library's default) or lanes")
     ap.add_argument("--e2e-serial", action="store_true", help="e2e leg on one context with synchronous copies")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing (used under ncu)")
     args = ap.parse_args()

@@ -95,6 +95,28 @@ int rt_trace_records(rt_ctx* ctx, double zenith_deg, double azimuth_deg, uint64_
                      uint64_t first_photon_id, uint64_t seed, uint32_t stream_id, void* cuda_stream,
                      uint32_t* records_out);
 
+/* A PART of a job (multi-GPU sharding; checkpointing): traces the photons with indices
+ * [range_begin, range_begin + range_count) of the job that rt_trace(ctx, ..., job_photons, first_photon_id, ...)
+ * would trace in one call -- same ids (first_photon_id + index), same columns and passes (§3.6 stratifies by
+ * the index in the JOB), same Sobol shifts -- so the integer tallies of disjoint ranges covering
+ * [0, job_photons), added up over calls, contexts or GPUs, equal the one-call tallies bit for bit.
+ * records_out: NULL, or a DEVICE pointer to 16 B x range_count (index = job index - range_begin).
+ * Errors: RT_EINVAL (range outside the job), else as rt_trace. */
+int rt_trace_range(rt_ctx* ctx, double zenith_deg, double azimuth_deg, uint64_t job_photons,
+                   uint64_t first_photon_id, uint64_t seed, uint32_t stream_id, void* cuda_stream,
+                   uint64_t range_begin, uint64_t range_count, uint32_t* records_out);
+
+/* Which kernel traces.  Both follow the same per-photon operation sequence, so
+ * photon records, tallies and counters are identical; only the schedule differs.
+ * RT_KERNEL_POOL (default): every warp keeps a pool of photons in shared memory, sorted by the phase they wait
+ *   for, and runs each phase with full warps (rt_trace_pool.cuh).  Used when the launch has fewer than 2^32
+ *   photons and the acceleration grid has at most 2048 x 2048 x 896 cells; otherwise the library falls back to
+ * RT_KERNEL_LANES: one photon per lane, phases scheduled by warp votes (rt_trace.cuh).
+ * Errors: RT_EINVAL. */
+#define RT_KERNEL_POOL 0
+#define RT_KERNEL_LANES 1
+int rt_set_kernel(rt_ctx* ctx, int kernel);
+
 /* Synchronise the context's device work and copy tallies out.  Each output may be a host or a
  * device pointer (detected), or NULL to skip: atm_abs nvox int64 in [z][y][x]; the others ncol
  * int64 in [y][x]; counters is a HOST pointer or NULL.  Energy closure: sum(atm_abs) +
@@ -114,7 +136,7 @@ int rt_read_tallies_async(rt_ctx* ctx, int64_t* atm_abs, int64_t* sfc_dir, int64
  * merge_ratio * min k_ext over the block's voxels) are traversed as ONE cell with the block's maximum as
  * majorant: clear air above, below and between the clouds costs one step per block instead of one per
  * cell.  Any majorant >= k_ext gives the same expectations, so only the sample paths change.
- * mx, my, mz: powers of two dividing the acceleration grid's extents; 1,1,1 (the default after
+ * mx, my, mz: powers of two, at most 64, dividing the acceleration grid's extents; 1,1,1 (the default after
  * rt_create_grid) = single-level grid.  merge_ratio >= 1.  Takes effect at the next rt_set_optics;
  * a context that already holds optics must be given them again before the next rt_trace
  * (RT_ESTATE otherwise).  Errors: RT_EINVAL. */

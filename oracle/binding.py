@@ -40,7 +40,7 @@ def lib():
                                    C.c_float, C.c_int, fp, fp, fp, fp, fp, C.c_double, C.c_double,
                                    C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint32, ip, ip, ip, ip, ip, ip,
                                    C.POINTER(Counters), C.POINTER(C.c_uint32), C.c_int,
-                                   C.POINTER(C.c_double)]
+                                   C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_uint64, C.c_uint64]
         _lib.orc_hardware_threads.restype = C.c_int
     return _lib
 
@@ -71,12 +71,15 @@ class Tallies:
 
 def trace(grid, optics, zenith_deg, azimuth_deg, n_photons, first_photon_id=0, seed=1, stream_id=0,
           precision=64, tallies=None, records=False, n_threads=1, merge=(1, 1, 1), merge_ratio=1.25,
-          weighted=False, diffuse_fraction=0.0, sobol=False, heating_split=False):
+          weighted=False, diffuse_fraction=0.0, sobol=False, heating_split=False, margins=False, index_range=None):
     """Run the oracle.  grid = (nx, ny, nz, dx, dy, dz, bx, by, bz); optics = dict with
     k_ext, k_ext_cloud, ssa, g ([nz][ny][nx] fp32) and sfc_albedo ([ny][nx] fp32); merge = merged-cell
     factors ((1, 1, 1) = single-level acceleration grid); weighted = the paper's absorption
     weights + Russian roulette instead of analog absorption; diffuse_fraction and
     sobol = the paper's top-of-domain source.
+    margins=True also returns, as tallies.margins, the smallest relative margin of any decision each photon took
+    (bookkeeping for the fp32-vs-fp64 attribution test).  index_range=(begin, count) traces only that part of the
+    n_photons-photon job (records stay indexed by the index in the job): the shards of a multi-GPU job.
     Returns (tallies, records or None, elapsed seconds of the photon loop)."""
     nx, ny, nz, dx, dy, dz, bx, by, bz = grid
     k, kp = _f32(optics["k_ext"])
@@ -90,6 +93,8 @@ def trace(grid, optics, zenith_deg, azimuth_deg, n_photons, first_photon_id=0, s
     ip = C.POINTER(C.c_int64)
     if heating_split and getattr(t, "atm_abs_direct", None) is None:
         t.atm_abs_direct = np.zeros((nz, ny, nx), dtype=np.int64)   # heating by never-scattered photons
+    mg = np.full(n_photons, np.inf, dtype=np.float64) if margins else None
+    rb, rn = (0, n_photons) if index_range is None else (int(index_range[0]), int(index_range[1]))
     el = C.c_double(0.0)
     rc = lib().orc_trace(int(precision), nx, ny, nz, dx, dy, dz, bx, by, bz, int(merge[0]), int(merge[1]),
                          int(merge[2]), float(merge_ratio), int(bool(weighted)), float(diffuse_fraction), int(bool(sobol)), kp, kcp, wp, gp, alp,
@@ -99,9 +104,12 @@ def trace(grid, optics, zenith_deg, azimuth_deg, n_photons, first_photon_id=0, s
                          t.sfc_abs.ctypes.data_as(ip), t.toa_up.ctypes.data_as(ip),
                          t.atm_abs_direct.ctypes.data_as(ip) if heating_split else None, C.byref(t.counters),
                          rec.ctypes.data_as(C.POINTER(C.c_uint32)) if records else None,
-                         int(n_threads), C.byref(el))
+                         int(n_threads), C.byref(el),
+                         mg.ctypes.data_as(C.POINTER(C.c_double)) if margins else None, rb, rn)
     if rc != 0:
         raise ValueError("orc_trace: bad arguments (rc=%d)" % rc)
+    if margins:
+        t.margins = mg
     return t, rec, el.value
 
 

@@ -240,6 +240,9 @@ struct Problem {
   int64_t *atm_abs, *sfc_dir, *sfc_dif, *sfc_abs, *toa_up;
   int64_t* atm_abs_direct;   // optional (may be null): the part of atm_abs deposited by never-scattered photons
   uint32_t* records;
+  double* margins;           // optional (may be null), one per photon: the smallest relative margin of any decision the
+                             // photon took (bookkeeping only; no effect on the path).  A photon whose fp32 and fp64 paths
+                             // differ must have met a decision whose two sides lie within rounding of each other.
 };
 
 inline void add64(int64_t* p, int64_t v) { __atomic_fetch_add(p, v, __ATOMIC_RELAXED); }
@@ -379,6 +382,19 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
     }
     uint32_t e = 1, n_ev = 0, n_sc = 0, n_sfc = 0;
     int fate = 0; uint32_t term = 0;
+    // decision margins (only when P.margins is given): how far each comparison or floor was from going the other way
+    double mg = INFINITY;
+    const bool track = P.margins != nullptr;
+    auto note = [&](double m) { if (m < mg) mg = m; };
+    auto note_rel = [&](R a, R b) {            // |a - b| relative to the larger magnitude
+      const double s = std::max(std::fabs((double)a), std::fabs((double)b));
+      note(s > 0 ? std::fabs((double)a - (double)b) / s : 0.0);
+    };
+    auto note_floor = [&](R f, int n) {        // f is floored to a voxel index in 0..n-1: distance to the nearest interior boundary
+      if (n <= 1) return;
+      const double x = (double)f, k = std::min((double)(n - 1), std::max(1.0, std::round(x)));
+      note(std::fabs(x - k));
+    };
     // §3.14 weighted mode: integer weight in tally quanta, W0 at launch.  Roulette (Iwabuchi 2006
     // as quoted in P:56): below W0/2 the photon survives with probability w/W0 exactly (a 32-bit word of
     // the Philox block at counter e | 2^31 is compared with w) and continues with W0, else it ends; both
@@ -411,6 +427,7 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
       else if (r[1] <= r[2])            { axis = 1; t = r[1]; }
       else                              { axis = 2; t = r[2]; }
       R dtau = kh * t;
+      if (track && kh > 0) note_rel(tau, dtau);
       if (kh > 0 && tau <= dtau) {
         // ---- step 7: tentative collision inside this cell -------------------
         R s = tau * rk;
@@ -419,12 +436,20 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
         for (int a = 0; a < 3; ++a) {
           q[a] = local(a);
           gv[a] = c[a] * bs[a] + std::min((int)(q[a] * rds[a]), (lev ? mxyz[a] : 1) * bs[a] - 1);
+          if (track) note_floor(q[a] * rds[a], (lev ? mxyz[a] : 1) * bs[a]);
         }
         size_t vox = ((size_t)gv[2] * ny + gv[1]) * nx + gv[0];
         Vox<R> vx = pack_voxel<R>(P.k_ext[vox], P.k_cloud[vox], P.ssa[vox], P.g[vox]);
         ++n_ev; ++C.n_events;                  // step 6
         // ---- step 8: classify ----------------------------------------------
         R xi = u1 * kh;
+        if (track) {
+          const R x = P.weighted ? E::fma(u1, kh - vx.c1, vx.c1) : xi;
+          if (!P.weighted) note(std::fabs((double)x - (double)vx.c1) / (double)kh);
+          note(std::fabs((double)x - (double)vx.c2) / (double)kh);
+          note(std::fabs((double)x - (double)vx.c3) / (double)kh);
+          if (x < vx.c3) note(std::fabs(std::fabs((double)d[2]) - 0.99999));   // which rotation formula (§3.9)
+        }
         if (P.weighted) {
           // §3.14: deposit w * P(absorbed), P = c1 / k_hat as a 24-bit fixed-point number; the rest goes on
           const R f = vx.c1 * rk;
@@ -461,6 +486,10 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
         draw();
       } else {
         // ---- step 5 (cont.): leave the cell through `axis` -------------------
+        if (track) {                           // which face: the gap to the runner-up
+          const R o1 = r[(axis + 1) % 3], o2 = r[(axis + 2) % 3];
+          note_rel(t, std::min(o1, o2));
+        }
         tau = tau - dtau;
         ++C.n_cell_steps;
         const int step = lev ? mxyz[axis] : 1;
@@ -477,6 +506,7 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
           R qx = local(0), qy = local(1);
           int hx = c[0] * bx + std::min((int)(qx * rdx), (lev ? P.mx : 1) * bx - 1);
           int hy = c[1] * by + std::min((int)(qy * rdy), (lev ? P.my : 1) * by - 1);
+          if (track) { note_floor(qx * rdx, (lev ? P.mx : 1) * bx); note_floor(qy * rdy, (lev ? P.my : 1) * by); }
           size_t col = (size_t)hy * nx + hx;
           if (at_top) {                        // step 11
             add64(&P.toa_up[col], P.weighted ? (int64_t)w : W0); ++C.n_toa;
@@ -497,6 +527,7 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
             reflect = true;
           } else {
             reflect = u1 < (R)P.albedo[col];
+            if (track) note(std::fabs((double)u1 - (double)P.albedo[col]));
           }
           if (reflect) {
             R mu = std::sqrt((R)1 - u2), s = std::sqrt(u2);
@@ -538,6 +569,7 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
                 const int m = mxyz[a];
                 if (a != axis) {
                   const int k = std::min(m - 1, (int)(r[a] / del[0][a]));
+                  if (track) note_floor(r[a] / del[0][a], m);
                   r[a] = std::max((R)0, E::fma(-(R)k, del[0][a], r[a]));
                   c[a] += (v[a] > 0) ? (m - 1 - k) : k;
                 } else {
@@ -554,6 +586,7 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
       }
     }
     ++C.n_photons;
+    if (track) P.margins[i] = mg;
     if (P.records) {
       uint32_t* r = P.records + 4 * i;
       r[0] = (uint32_t)fate | (std::min(n_sfc, 0xFFFFFFu) << 8);
@@ -609,7 +642,8 @@ int orc_trace(int precision, int nx, int ny, int nz, float dx, float dy, float d
               const float* sfc_albedo, double zenith_deg, double azimuth_deg, uint64_t n_photons,
               uint64_t first_photon_id, uint64_t seed, uint32_t stream_id, int64_t* atm_abs,
               int64_t* sfc_dir, int64_t* sfc_dif, int64_t* sfc_abs, int64_t* toa_up,
-              int64_t* atm_abs_direct, orc_counters* counters, uint32_t* records, int n_threads, double* elapsed_s) {
+              int64_t* atm_abs_direct, orc_counters* counters, uint32_t* records, int n_threads, double* elapsed_s,
+              double* margins, uint64_t range_begin, uint64_t range_count) {
   if (nx <= 0 || ny <= 0 || nz <= 0 || bx <= 0 || by <= 0 || bz <= 0) return -1;
   if (nx % bx || ny % by || nz % bz) return -1;
   if (mx <= 0 || my <= 0 || mz <= 0 || (nx / bx) % mx || (ny / by) % my || (nz / bz) % mz) return -1;
@@ -618,13 +652,16 @@ int orc_trace(int precision, int nx, int ny, int nz, float dx, float dy, float d
   if (!(diffuse_fraction >= 0.0f && diffuse_fraction <= 1.0f)) return -1;
   Problem P{nx, ny, nz, bx, by, bz, mx, my, mz, merge_ratio, weighted ? 1 : 0, diffuse_fraction, sobol ? 1 : 0, dx, dy, dz, k_ext, k_ext_cloud, ssa, g, sfc_albedo,
             zenith_deg, azimuth_deg, n_photons, first_photon_id, seed, stream_id,
-            atm_abs, sfc_dir, sfc_dif, sfc_abs, toa_up, atm_abs_direct, records};
+            atm_abs, sfc_dir, sfc_dif, sfc_abs, toa_up, atm_abs_direct, records, margins};
+  // a PART of the job: photon indices [range_begin, range_begin + range_count) of the n_photons;
+  // records and margins stay indexed by the index in the job
+  if (range_begin > n_photons || range_count > n_photons - range_begin) return -1;
   std::vector<float> khat = build_majorant(P);
   if (n_threads < 1) n_threads = 1;
   std::vector<orc_counters> cs(n_threads);
   std::memset(cs.data(), 0, sizeof(orc_counters) * n_threads);
   auto run = [&](int t) {
-    uint64_t b = n_photons * (uint64_t)t / n_threads, e = n_photons * (uint64_t)(t + 1) / n_threads;
+    uint64_t b = range_begin + range_count * (uint64_t)t / n_threads, e = range_begin + range_count * (uint64_t)(t + 1) / n_threads;
     if (precision == 64) trace_range<double>(P, khat, b, e, cs[t]);
     else                 trace_range<float>(P, khat, b, e, cs[t]);
   };

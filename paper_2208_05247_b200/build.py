@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "librt_b200.so")
 SOURCES = ["rt.cu"]
-DEPS = ["rt.cu", "rt_device.cuh", "rt_setup.cuh", "rt_trace.cuh", os.path.join("..", "..", "include", "rt.h")]
+DEPS = ["rt.cu", "rt_device.cuh", "rt_setup.cuh", "rt_trace.cuh", "rt_trace_pool.cuh", os.path.join("..", "..", "include", "rt.h")]
 
 # -fmad=false: no implicit contraction; every FMA in the kernels is written explicitly so the
 # fp32 decisions are reproducible operation by operation.

@@ -11,6 +11,7 @@
 
 #include "rt_setup.cuh"
 #include "rt_trace.cuh"
+#include "rt_trace_pool.cuh"
 
 struct rt_ctx {
   int device = 0;
@@ -47,7 +48,9 @@ struct rt_ctx {
   float* stage = nullptr;                 // 4 nvox + ncol floats; only allocated when a caller passes host fields
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   bool have_optics = false, have_trace = false;
-  int trace_blocks[2][2] = {{0, 0}, {0, 0}};   // persistent grid size, [records][weighted]
+  int kernel = RT_KERNEL_LANES;           // rt_set_kernel: which scheduler traces (same photons either way)
+  bool pool_fits = true;                  // the grid fits the pool kernel's packed cell index
+  int trace_blocks[2][16] = {};           // persistent grid size per kernel instantiation, [pool][records | pow2 | weighted | batch]; 0 = not asked yet
   int sm_count = 0;
   uint64_t launches = 0;
   std::string err;
@@ -96,10 +99,44 @@ const float* stage_input(rt_ctx* c, const float* p, size_t n, size_t slot_offset
   return dst;
 }
 
+// One source, 16 instantiations per scheduler: <records, power-of-two wrap, weighted, batch>.
+struct KernelInfo { const void* fn; int threads; size_t smem; };
+template <bool R, bool P, bool W, bool B> KernelInfo kernel_info(bool pool) {
+  if (pool) return {(const void*)rt::trace_pool_kernel<R, P, W, B>, rt::kPoolThreads, rt::pool_smem_bytes(R || W || B)};
+  return {(const void*)rt::trace_kernel<R, P, W, B>, rt::kTraceThreads, 0};
+}
+KernelInfo pick_kernel(int variant, bool pool) {
+  switch (variant) {
+#define RT_CASE(v) case v: return kernel_info<((v) & 1) != 0, ((v) & 2) != 0, ((v) & 4) != 0, ((v) & 8) != 0>(pool);
+    RT_CASE(0) RT_CASE(1) RT_CASE(2) RT_CASE(3) RT_CASE(4) RT_CASE(5) RT_CASE(6) RT_CASE(7)
+    RT_CASE(8) RT_CASE(9) RT_CASE(10) RT_CASE(11) RT_CASE(12) RT_CASE(13) RT_CASE(14) RT_CASE(15)
+#undef RT_CASE
+  }
+  return {nullptr, 0, 0};
+}
+// Persistent grid of one instantiation: resident blocks per SM (occupancy query, once) x SM count.
+int trace_grid(rt_ctx* c, int variant, bool pool, const KernelInfo& k, int* blocks_out) {
+  int& cached = c->trace_blocks[pool ? 1 : 0][variant];
+  if (cached == 0) {
+    if (k.smem > 0)   // static + dynamic shared memory pass the 48 KB that need no opt-in
+      RT_CUDA(c, cudaFuncSetAttribute(k.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.smem));
+    if (pool)   // the photon pools want the shared-memory side of the L1 / shared-memory split
+      RT_CUDA(c, cudaFuncSetAttribute(k.fn, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    int per_sm = 0;
+    RT_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k.fn, k.threads, k.smem));
+    if (per_sm < 1) return fail(c, RT_ECUDA, "rt_trace: the trace kernel does not fit on an SM");
+    cached = c->sm_count * per_sm;
+  }
+  *blocks_out = cached;
+  return RT_OK;
+}
+
 int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photons, uint64_t first_id,
              uint64_t seed, uint32_t stream_id, void* stream_v, uint32_t* records, int n_points = 0, int first_point = 0,
-             const unsigned long long* tab = nullptr, bool factored_trace = false) {
+             const unsigned long long* tab = nullptr, bool factored_trace = false, uint64_t index_base = 0,
+             uint64_t job_photons = 0) {
   if (!c) return RT_EINVAL;
+  if (job_photons == 0) job_photons = n_photons;   // a whole job in one call
   if (n_points == 0 && !c->have_optics) return fail(c, RT_ESTATE, "rt_trace: call rt_set_optics first");
   if (!(zenith_deg >= 0.0 && zenith_deg < 90.0) || !std::isfinite(azimuth_deg))
     return fail(c, RT_EINVAL, "rt_trace: zenith must be in [0, 90) degrees and azimuth finite");
@@ -128,12 +165,20 @@ int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photon
   A.sfc_abs = tally_ptr(c, 3); A.toa_up = tally_ptr(c, 4);
   A.counters = c->counters; A.next_photon = c->counters + rt::C_COUNT;
   A.records = records;
-  A.n_photons = n_photons; A.first_id = first_id; A.ncol = c->ncol;
-  A.n_full = (n_photons / c->ncol) * c->ncol;
+  A.n_photons = n_photons; A.first_id = first_id; A.ncol = c->ncol; A.index_base = index_base;
+  A.n_full = (job_photons / c->ncol) * c->ncol;
+  const bool pow2 = !(c->ncx & (c->ncx - 1)) && !(c->ncy & (c->ncy - 1));
+  // the pool kernel keeps a photon's index in 32 bits and its cell index packed: larger launches and grids go to
+  // the one-photon-per-lane kernel (same photons)
+  const bool pool = c->kernel == RT_KERNEL_POOL && c->pool_fits && n_photons < (1ull << 32);
+  const int variant = (records ? 1 : 0) | (pow2 ? 2 : 0) | (c->weighted ? 4 : 0) | (n_points > 0 ? 8 : 0);
+  const KernelInfo kinfo = pick_kernel(variant, pool);
+  int blocks = 0;
+  if (int rcg = trace_grid(c, variant, pool, kinfo, &blocks)) return rcg;
   {
     // ids per work-counter atomic: 128, or fewer (a multiple of 32) when the launch has under ~8 chunks per warp,
     // so that short launches (one spectral point of config 4) balance over all resident warps
-    const unsigned long long warps = (unsigned long long)c->trace_blocks[records ? 1 : 0][c->weighted] * (rt::kTraceThreads / 32);
+    const unsigned long long warps = (unsigned long long)blocks * (rt::kTraceThreads / 32);
     unsigned long long ch = n_photons / (warps * 8ull);
     ch = (ch / 32ull) * 32ull;
     A.chunk = (unsigned)(ch < 32ull ? 32ull : (ch > (unsigned long long)rt::kChunk ? (unsigned long long)rt::kChunk : ch));
@@ -147,27 +192,8 @@ int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photon
   RT_CUDA(c, cudaMemsetAsync(A.next_photon, 0, sizeof(unsigned long long), st));
   RT_CUDA(c, cudaEventRecord(c->ev0, st));
   if (n_photons > 0) {
-    const bool pow2 = !(c->ncx & (c->ncx - 1)) && !(c->ncy & (c->ncy - 1));
-    const int blocks = c->trace_blocks[records ? 1 : 0][c->weighted];
-#define RT_LAUNCH(R, P, W) rt::trace_kernel<R, P, W><<<blocks, rt::kTraceThreads, 0, st>>>(A)
-#define RT_LAUNCH_B(R, P, W) rt::trace_kernel<R, P, W, true><<<blocks, rt::kTraceThreads, 0, st>>>(A)
-    if (n_points > 0) {
-      if (c->weighted) {
-        if (records) { if (pow2) RT_LAUNCH_B(true, true, true); else RT_LAUNCH_B(true, false, true); }
-        else         { if (pow2) RT_LAUNCH_B(false, true, true); else RT_LAUNCH_B(false, false, true); }
-      } else {
-        if (records) { if (pow2) RT_LAUNCH_B(true, true, false); else RT_LAUNCH_B(true, false, false); }
-        else         { if (pow2) RT_LAUNCH_B(false, true, false); else RT_LAUNCH_B(false, false, false); }
-      }
-    } else if (c->weighted) {
-      if (records) { if (pow2) RT_LAUNCH(true, true, true); else RT_LAUNCH(true, false, true); }
-      else         { if (pow2) RT_LAUNCH(false, true, true); else RT_LAUNCH(false, false, true); }
-    } else {
-      if (records) { if (pow2) RT_LAUNCH(true, true, false); else RT_LAUNCH(true, false, false); }
-      else         { if (pow2) RT_LAUNCH(false, true, false); else RT_LAUNCH(false, false, false); }
-    }
-#undef RT_LAUNCH
-#undef RT_LAUNCH_B
+    void* kargs[1] = {(void*)&A};
+    RT_CUDA(c, cudaLaunchKernel(kinfo.fn, dim3((unsigned)blocks), dim3((unsigned)kinfo.threads), kargs, kinfo.smem, st));
     ++c->launches;
   }
   RT_CUDA(c, cudaEventRecord(c->ev1, st));
@@ -211,29 +237,8 @@ int rt_create_grid(rt_ctx** out, int nx, int ny, int nz, float dx, float dy, flo
   RT_CUDA(c, cudaEventCreate(&c->ev0));
   RT_CUDA(c, cudaEventCreate(&c->ev1));
   RT_CUDA(c, cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, cuda_device));
-  // persistent grid: resident blocks per SM (the smallest over the wrap and absorption-mode variants) x SM count
-  auto occupancy = [&](int* out, auto... kernels) {
-    int best = 1 << 30;
-    cudaError_t err = cudaSuccess;
-    auto one = [&](auto k) {
-      int v = 0;
-      cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, k, rt::kTraceThreads, 0);
-      if (e != cudaSuccess) err = e;
-      if (v < best) best = v;
-    };
-    (one(kernels), ...);
-    *out = best > 0 && best < (1 << 30) ? best : 1;
-    return err;
-  };
-  int per_sm = 1;
-  RT_CUDA(c, occupancy(&per_sm, rt::trace_kernel<false, false, false>, rt::trace_kernel<false, true, false>));
-  c->trace_blocks[0][0] = c->sm_count * per_sm;
-  RT_CUDA(c, occupancy(&per_sm, rt::trace_kernel<false, false, true>, rt::trace_kernel<false, true, true>));
-  c->trace_blocks[0][1] = c->sm_count * per_sm;
-  RT_CUDA(c, occupancy(&per_sm, rt::trace_kernel<true, false, false>, rt::trace_kernel<true, true, false>));
-  c->trace_blocks[1][0] = c->sm_count * per_sm;
-  RT_CUDA(c, occupancy(&per_sm, rt::trace_kernel<true, false, true>, rt::trace_kernel<true, true, true>));
-  c->trace_blocks[1][1] = c->sm_count * per_sm;
+  // the pool kernel packs (cx, cy, cz + 64) into 11 + 11 + 10 bits (rt_trace_pool.cuh)
+  c->pool_fits = c->ncx <= 2048 && c->ncy <= 2048 && c->ncz <= 896;
   return RT_OK;
 }
 
@@ -514,6 +519,22 @@ int rt_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photon
   return do_trace(c, zenith_deg, azimuth_deg, n_photons, first_photon_id, seed, stream_id, cuda_stream, nullptr);
 }
 
+int rt_trace_range(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t job_photons, uint64_t first_photon_id,
+                   uint64_t seed, uint32_t stream_id, void* cuda_stream, uint64_t range_begin, uint64_t range_count,
+                   uint32_t* records_out) {
+  if (c && (range_begin > job_photons || range_count > job_photons - range_begin))
+    return fail(c, RT_EINVAL, "rt_trace_range: the range must lie within [0, job_photons)");
+  return do_trace(c, zenith_deg, azimuth_deg, range_count, first_photon_id, seed, stream_id, cuda_stream, records_out,
+                  0, 0, nullptr, false, range_begin, job_photons);
+}
+
+int rt_set_kernel(rt_ctx* c, int kernel) {
+  if (!c) return RT_EINVAL;
+  if (kernel != RT_KERNEL_POOL && kernel != RT_KERNEL_LANES) return fail(c, RT_EINVAL, "rt_set_kernel: unknown kernel");
+  c->kernel = kernel;
+  return RT_OK;
+}
+
 int rt_trace_records(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photons,
                      uint64_t first_photon_id, uint64_t seed, uint32_t stream_id, void* cuda_stream,
                      uint32_t* records_out) {
@@ -588,8 +609,8 @@ int rt_read_tallies_async(rt_ctx* c, int64_t* atm_abs, int64_t* sfc_dir, int64_t
 int rt_set_merge(rt_ctx* c, int mx, int my, int mz, float merge_ratio) {
   if (!c) return RT_EINVAL;
   auto pow2 = [](int v) { return v > 0 && !(v & (v - 1)); };
-  if (!pow2(mx) || !pow2(my) || !pow2(mz) || c->ncx % mx || c->ncy % my || c->ncz % mz)
-    return fail(c, RT_EINVAL, "rt_set_merge: factors must be powers of two dividing the acceleration grid");
+  if (!pow2(mx) || !pow2(my) || !pow2(mz) || c->ncx % mx || c->ncy % my || c->ncz % mz || mx > 64 || my > 64 || mz > 64)
+    return fail(c, RT_EINVAL, "rt_set_merge: factors must be powers of two <= 64 dividing the acceleration grid");
   if (!(merge_ratio >= 1.0f) || !std::isfinite(merge_ratio)) return fail(c, RT_EINVAL, "rt_set_merge: merge_ratio must be >= 1");
   c->mx = mx; c->my = my; c->mz = mz; c->merge_ratio = merge_ratio;
   c->have_optics = false;                 // the majorant table is rebuilt by the next rt_set_optics

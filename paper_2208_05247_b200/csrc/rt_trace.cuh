@@ -78,7 +78,8 @@ struct TraceArgs {
   unsigned long long* counters;        // C_COUNT words
   unsigned long long* next_photon;     // work counter, zeroed before launch
   uint32_t* records;                   // 4 words per photon or nullptr
-  unsigned long long n_photons, first_id, n_full, ncol;
+  unsigned long long n_photons, first_id, n_full, ncol;   // photons of this launch; id of the JOB's photon 0; job's full passes
+  unsigned long long index_base;       // index in the job of this launch's first photon (rt_trace: 0; rt_trace_range: range_begin)
   unsigned chunk;                      // photon ids per global atomic: kChunk, or less so that a small launch still spreads over all warps
   PhiloxKeys keys;                     // round keys of the Philox key (seed)
   PhiloxKeys keys_sobol;               // ... of (seed low, seed high ^ 'SOBL'): digital shifts of §3.15
@@ -158,7 +159,7 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
 
   auto sid = [&]() { return kBatch ? jpt : A.stream_id; };
   auto draw = [&]() {
-    const unsigned long long pid = A.first_id + i;
+    const unsigned long long pid = A.first_id + A.index_base + i;
     const uint4 X = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), e, sid(), A.keys);
     tau = neg_log(1.0f - u24(X.x)); u1 = u24(X.y); w2 = X.z; w3 = X.w;
   };
@@ -194,7 +195,7 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
   uint32_t term = 0;
   auto roulette = [&](uint32_t where) {
     if (wq >= kW0 / 2) return false;
-    const unsigned long long pid = A.first_id + i;
+    const unsigned long long pid = A.first_id + A.index_base + i;
     const uint4 Y = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), e | 0x80000000u, sid(), A.keys);
     if ((unsigned long long)Y.w < wq) { t_rgain += kW0 - wq; ++t_rkept; wq = kW0; return false; }
     t_rlost += wq; fate = 5; term = where;
@@ -272,18 +273,19 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
           i -= __ldg(A.offsets + lo);
           n_full = __ldg(A.nfull + lo);
         }
-        const unsigned long long pid = A.first_id + i;
+        const unsigned long long ij = A.index_base + i;   // index in the job: column and pass
+        const unsigned long long pid = A.first_id + ij;
         const uint4 X = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), 0u, sid(), A.keys);
         int ix, iy;
         float e0 = u24(X.x), e1 = u24(X.y);   // sub-pixel entry point
-        if (i < n_full) {
-          // column = i mod ncol; 32-bit arithmetic whenever the index allows it
-          const uint32_t col = (i >> 32) ? (uint32_t)(i % A.ncol) : (uint32_t)i % (uint32_t)A.ncol;
+        if (ij < n_full) {
+          // column = index mod ncol; 32-bit arithmetic whenever the index allows it
+          const uint32_t col = (ij >> 32) ? (uint32_t)(ij % A.ncol) : (uint32_t)ij % (uint32_t)A.ncol;
           ix = (int)(col % (uint32_t)A.nx);
           iy = (int)(col / (uint32_t)A.nx);
           if (A.sobol) {
             // §3.15: point k = pass number of the 2-D Sobol sequence, XORed with the column's digital shift
-            const uint32_t k = (i >> 32) ? (uint32_t)(i / A.ncol) : (uint32_t)i / (uint32_t)A.ncol;
+            const uint32_t k = (ij >> 32) ? (uint32_t)(ij / A.ncol) : (uint32_t)ij / (uint32_t)A.ncol;
             const uint4 S = philox4x32_10(col, sid(), (uint32_t)A.first_id, (uint32_t)(A.first_id >> 32),
                                           A.keys_sobol);
             uint32_t x1 = __brev(k), x2 = 0, V = 0x80000000u;
