@@ -11,6 +11,8 @@ from . import build as _build
 
 W0 = 1 << 32  # tally quanta per photon
 FATE_ATM_ABS, FATE_SFC_ABS, FATE_TOD_EXIT, FATE_CAPPED, FATE_ROULETTE = 1, 2, 3, 4, 5
+# decision kinds of the optional decision log (rt_oracle.cpp, enum DK_*)
+DK_COLLIDE, DK_FACE, DK_VOXEL, DK_CLASS, DK_POLE, DK_COLUMN, DK_ALBEDO, DK_RELEVEL = 1, 2, 3, 4, 5, 6, 7, 8
 
 COUNTER_FIELDS = ("n_photons", "n_events", "n_null", "n_rayleigh", "n_hg", "n_atm_abs",
                   "n_sfc_hits", "n_sfc_abs", "n_toa", "n_capped", "n_cell_steps", "n_relevel",
@@ -40,7 +42,8 @@ def lib():
                                    C.c_float, C.c_int, fp, fp, fp, fp, fp, C.c_double, C.c_double,
                                    C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint32, ip, ip, ip, ip, ip, ip,
                                    C.POINTER(Counters), C.POINTER(C.c_uint32), C.c_int,
-                                   C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_uint64, C.c_uint64]
+                                   C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_uint64, C.c_uint64,
+                                   C.POINTER(C.c_uint8), C.POINTER(C.c_float), C.POINTER(C.c_uint32), C.c_uint32]
         _lib.orc_hardware_threads.restype = C.c_int
     return _lib
 
@@ -71,14 +74,17 @@ class Tallies:
 
 def trace(grid, optics, zenith_deg, azimuth_deg, n_photons, first_photon_id=0, seed=1, stream_id=0,
           precision=64, tallies=None, records=False, n_threads=1, merge=(1, 1, 1), merge_ratio=1.25,
-          weighted=False, diffuse_fraction=0.0, sobol=False, heating_split=False, margins=False, index_range=None):
+          weighted=False, diffuse_fraction=0.0, sobol=False, heating_split=False, margins=False, index_range=None,
+          decision_log=0):
     """Run the oracle.  grid = (nx, ny, nz, dx, dy, dz, bx, by, bz); optics = dict with
     k_ext, k_ext_cloud, ssa, g ([nz][ny][nx] fp32) and sfc_albedo ([ny][nx] fp32); merge = merged-cell
     factors ((1, 1, 1) = single-level acceleration grid); weighted = the paper's absorption
     weights + Russian roulette instead of analog absorption; diffuse_fraction and
     sobol = the paper's top-of-domain source.
     margins=True also returns, as tallies.margins, the smallest relative margin of any decision each photon took
-    (bookkeeping for the fp32-vs-fp64 attribution test).  index_range=(begin, count) traces only that part of the
+    (bookkeeping for the fp32-vs-fp64 attribution test); decision_log=K also returns tallies.decisions = (codes
+    uint8 [n][K], margins float32 [n][K], counts uint32 [n]): each photon's first K decisions as kind << 4 | outcome
+    (kinds: oracle.DK_*) with the margin each was taken by.  index_range=(begin, count) traces only that part of the
     n_photons-photon job (records stay indexed by the index in the job): the shards of a multi-GPU job.
     Returns (tallies, records or None, elapsed seconds of the photon loop)."""
     nx, ny, nz, dx, dy, dz, bx, by, bz = grid
@@ -95,6 +101,10 @@ def trace(grid, optics, zenith_deg, azimuth_deg, n_photons, first_photon_id=0, s
         t.atm_abs_direct = np.zeros((nz, ny, nx), dtype=np.int64)   # heating by never-scattered photons
     mg = np.full(n_photons, np.inf, dtype=np.float64) if margins else None
     rb, rn = (0, n_photons) if index_range is None else (int(index_range[0]), int(index_range[1]))
+    K = int(decision_log)
+    dcode = np.zeros((n_photons, K), dtype=np.uint8) if K else None
+    dmarg = np.zeros((n_photons, K), dtype=np.float32) if K else None
+    dcnt = np.zeros(n_photons, dtype=np.uint32) if K else None
     el = C.c_double(0.0)
     rc = lib().orc_trace(int(precision), nx, ny, nz, dx, dy, dz, bx, by, bz, int(merge[0]), int(merge[1]),
                          int(merge[2]), float(merge_ratio), int(bool(weighted)), float(diffuse_fraction), int(bool(sobol)), kp, kcp, wp, gp, alp,
@@ -105,11 +115,16 @@ def trace(grid, optics, zenith_deg, azimuth_deg, n_photons, first_photon_id=0, s
                          t.atm_abs_direct.ctypes.data_as(ip) if heating_split else None, C.byref(t.counters),
                          rec.ctypes.data_as(C.POINTER(C.c_uint32)) if records else None,
                          int(n_threads), C.byref(el),
-                         mg.ctypes.data_as(C.POINTER(C.c_double)) if margins else None, rb, rn)
+                         mg.ctypes.data_as(C.POINTER(C.c_double)) if margins else None, rb, rn,
+                         dcode.ctypes.data_as(C.POINTER(C.c_uint8)) if K else None,
+                         dmarg.ctypes.data_as(C.POINTER(C.c_float)) if K else None,
+                         dcnt.ctypes.data_as(C.POINTER(C.c_uint32)) if K else None, K)
     if rc != 0:
         raise ValueError("orc_trace: bad arguments (rc=%d)" % rc)
     if margins:
         t.margins = mg
+    if K:
+        t.decisions = (dcode, dmarg, dcnt)
     return t, rec, el.value
 
 
@@ -142,25 +157,32 @@ def _f64(a):
     return a, a.ctypes.data_as(C.POINTER(C.c_double))
 
 
-def sample_hg(g, u, precision=64):
+def sample_hg(g, u, precision=64, with_sine=False):
+    """Polar cosine mu(u) of the Henyey-Greenstein sampler; with_sine: also sin(theta)."""
     u, up = _f64(u)
     mu = np.empty_like(u)
-    lib().orc_sample_hg(int(precision), C.c_double(g), up, mu.ctypes.data_as(C.POINTER(C.c_double)),
+    sn = np.empty_like(u)
+    dp = C.POINTER(C.c_double)
+    lib().orc_sample_hg(int(precision), C.c_double(g), up, mu.ctypes.data_as(dp), sn.ctypes.data_as(dp),
                         C.c_uint64(u.size))
-    return mu
+    return (mu, sn) if with_sine else mu
 
 
-def sample_rayleigh(u, precision=64):
+def sample_rayleigh(u, precision=64, with_sine=False):
     u, up = _f64(u)
     mu = np.empty_like(u)
-    lib().orc_sample_rayleigh(int(precision), up, mu.ctypes.data_as(C.POINTER(C.c_double)),
-                              C.c_uint64(u.size))
-    return mu
+    sn = np.empty_like(u)
+    dp = C.POINTER(C.c_double)
+    lib().orc_sample_rayleigh(int(precision), up, mu.ctypes.data_as(dp), sn.ctypes.data_as(dp), C.c_uint64(u.size))
+    return (mu, sn) if with_sine else mu
 
 
-def rotate(d, mu, u_phi, precision=64):
+def rotate(d, mu, u_phi, precision=64, sn=None):
+    """Rotate the unit vector d by the polar angle (cosine mu, sine sn; default sqrt(1 - mu^2)) and azimuth 2 pi u_phi."""
     v = (C.c_double * 3)(*d)
-    lib().orc_rotate(int(precision), v, C.c_double(mu), C.c_double(u_phi))
+    if sn is None:
+        sn = float(np.sqrt(max(0.0, 1.0 - float(mu) ** 2)))
+    lib().orc_rotate(int(precision), v, C.c_double(mu), C.c_double(sn), C.c_double(u_phi))
     return np.array(list(v))
 
 

@@ -150,25 +150,26 @@ template <> struct Elem<double> {
 // §3.9 samplers
 // ---------------------------------------------------------------------------
 // Henyey-Greenstein ("Henyey-Greenstein phase function without delta-scaling"):
-// inverse CDF of p(mu) = (1-g^2) / (2 (1 + g^2 - 2 g mu)^(3/2)).
-template <class R> inline R sample_hg(R g, R u) {
-  R mu;
-  if (std::fabs(g) < (R)1e-3) {
-    mu = Elem<R>::fma((R)2, u, (R)-1);
-  } else {
-    R gg = g * g;
-    R den = Elem<R>::fma((R)2 * g, u, (R)1 - g);
-    R q = ((R)1 - gg) / den;
-    R num = Elem<R>::fma(-q, q, (R)1 + gg);
-    mu = num / ((R)2 * g);
-  }
-  return std::min((R)1, std::max((R)-1, mu));
+// inverse CDF of p(mu) = (1-g^2) / (2 (1 + g^2 - 2 g mu)^(3/2)), i.e. mu = (1 + g^2 - q^2) / (2 g) with
+// q = (1 - g^2) / (1 - g + 2 g u).  Written in the cancellation-free form of DESIGN.md 3.9: with den = 1 - g + 2 g u,
+//   1 - mu = (1 - g)(1 - u)(q + 1 - g) / den,     1 + mu = (1 + g) u (q + 1 + g) / den
+// (their sum is 2 identically), mu = half their difference and sin(theta) = sqrt of their product, so the sine of
+// a forward-peak angle keeps its relative accuracy in fp32 (1 - u is exact for a 24-bit u).  Regular at g = 0.
+template <class R> inline void sample_hg(R g, R u, R& mu, R& s) {
+  const R a = (R)1 - g, b = (R)1 + g;
+  const R den = Elem<R>::fma((R)2 * g, u, a);
+  const R rden = (R)1 / den;
+  const R q = (a * b) * rden;
+  const R omm = ((a * ((R)1 - u)) * rden) * (q + a);
+  const R opm = ((b * u) * rden) * (q + b);
+  mu = (R)0.5 * (opm - omm);
+  s = std::sqrt(omm * opm);
 }
 
 // Rayleigh ("Rayleigh phase function for scattering of gases"):
 // p(mu) = 3/8 (1 + mu^2); CDF(mu) = (mu^3 + 3 mu + 4)/8 = u.  Solve the cubic
-// mu^3 + 3 mu - y = 0, y = 8u - 4, by 4 Newton steps from mu0 = y/4.
-template <class R> inline R sample_rayleigh(R u) {
+// mu^3 + 3 mu - y = 0, y = 8u - 4, by 4 Newton steps from mu0 = y/4; sin(theta) = sqrt(1 - mu^2).
+template <class R> inline void sample_rayleigh(R u, R& mu_out, R& s) {
   R y = Elem<R>::fma((R)8, u, (R)-4);
   R mu = (R)0.25 * y;
   for (int it = 0; it < 4; ++it) {
@@ -177,28 +178,34 @@ template <class R> inline R sample_rayleigh(R u) {
     R dv = Elem<R>::fma((R)3, m2, (R)3);
     mu = mu - fv / dv;
   }
-  return std::min((R)1, std::max((R)-1, mu));
+  mu = std::min((R)1, std::max((R)-1, mu));
+  mu_out = mu;
+  s = std::sqrt(std::max((R)0, Elem<R>::fma(-mu, mu, (R)1)));
 }
 
-// Rotate direction (a,b,c) by polar cosine mu and azimuth (cphi,sphi); §3.9.
+// Rotate the unit direction (a,b,c) by the polar angle (cosine mu, sine s) and the azimuth (cphi,sphi); §3.9.
+// r^2 = a^2 + b^2 is the squared sine of the direction's own polar angle (not 1 - c^2: no cancellation near the
+// poles); below POLE_R2 the direction is taken as exactly +-z (an error below 1e-6 rad).  The result has norm
+// 1 + O(rounding), so it is renormalised by the first-order reciprocal square root 3/2 - n2/2.
+constexpr double POLE_R2 = 1e-12;
 template <class R>
-inline void rotate_dir(R& a, R& b, R& c, R mu, R cphi, R sphi) {
-  R s = std::sqrt(std::max((R)0, Elem<R>::fma(-mu, mu, (R)1)));
+inline void rotate_dir(R& a, R& b, R& c, R mu, R s, R cphi, R sphi) {
+  const R r2 = Elem<R>::fma(a, a, b * b);
   R nx, ny, nz;
-  if (std::fabs(c) < (R)0.99999) {
-    R r = std::sqrt(Elem<R>::fma(-c, c, (R)1));
-    R h = s / r;
-    R ac = a * c, bc = b * c;
-    R t1 = Elem<R>::fma(ac, cphi, -(b * sphi));
-    R t2 = Elem<R>::fma(bc, cphi, a * sphi);
-    nx = Elem<R>::fma(h, t1, a * mu);
-    ny = Elem<R>::fma(h, t2, b * mu);
+  if (r2 > (R)POLE_R2) {
+    const R r = std::sqrt(r2);
+    const R ir = (R)1 / r;
+    const R ah = a * ir, bh = b * ir;
+    const R t1 = Elem<R>::fma(ah * c, cphi, -(bh * sphi));
+    const R t2 = Elem<R>::fma(bh * c, cphi, ah * sphi);
+    nx = Elem<R>::fma(s, t1, a * mu);
+    ny = Elem<R>::fma(s, t2, b * mu);
     nz = Elem<R>::fma(-(s * r), cphi, c * mu);
   } else {
     nx = s * cphi; ny = s * sphi; nz = (c > 0 ? mu : -mu);
   }
-  R n2 = Elem<R>::fma(nz, nz, Elem<R>::fma(ny, ny, nx * nx));
-  R inv = (R)1 / std::sqrt(n2);
+  const R n2 = Elem<R>::fma(nz, nz, Elem<R>::fma(ny, ny, nx * nx));
+  const R inv = Elem<R>::fma((R)-0.5, n2, (R)1.5);
   a = nx * inv; b = ny * inv; c = nz * inv;
 }
 
@@ -243,7 +250,20 @@ struct Problem {
   double* margins;           // optional (may be null), one per photon: the smallest relative margin of any decision the
                              // photon took (bookkeeping only; no effect on the path).  A photon whose fp32 and fp64 paths
                              // differ must have met a decision whose two sides lie within rounding of each other.
+  // optional decision log (may be null; bookkeeping only): the photon's first dlog_cap decisions, one byte each
+  // (kind << 4 | outcome, kinds below) with the margin by which it was taken, and the number of decisions taken
+  uint8_t* dlog_code; float* dlog_margin; uint32_t* dlog_count; uint32_t dlog_cap;
 };
+
+// decision kinds of the log: what was compared, and in which unit its margin is
+enum { DK_COLLIDE = 1,   // tau <= k_hat t ?            distance between collision point and face, in face spacings of that axis
+       DK_FACE = 2,      // which axis' face is next    distance to the runner-up face, in face spacings of the chosen axis
+       DK_VOXEL = 3,     // floor to a voxel index      distance to the nearest voxel boundary, in voxels
+       DK_CLASS = 4,     // absorb / HG / Rayleigh / null   distance to the nearest threshold, in units of k_hat
+       DK_POLE = 5,      // which rotation formula      | |d_z| - threshold |
+       DK_COLUMN = 6,    // floor to a surface column   as DK_VOXEL
+       DK_ALBEDO = 7,    // u1 < albedo ?               |u1 - albedo|
+       DK_RELEVEL = 8 }; // floor to a cell of the entered block (3.7b)   in cells
 
 inline void add64(int64_t* p, int64_t v) { __atomic_fetch_add(p, v, __ATOMIC_RELAXED); }
 
@@ -384,16 +404,24 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
     int fate = 0; uint32_t term = 0;
     // decision margins (only when P.margins is given): how far each comparison or floor was from going the other way
     double mg = INFINITY;
-    const bool track = P.margins != nullptr;
-    auto note = [&](double m) { if (m < mg) mg = m; };
-    auto note_rel = [&](R a, R b) {            // |a - b| relative to the larger magnitude
-      const double s = std::max(std::fabs((double)a), std::fabs((double)b));
-      note(s > 0 ? std::fabs((double)a - (double)b) / s : 0.0);
+    const bool track = P.margins != nullptr || P.dlog_code != nullptr;
+    uint32_t n_dec = 0;
+    auto note = [&](int kind, int outcome, double m) {
+      if (m < mg) mg = m;
+      if (P.dlog_code && n_dec < P.dlog_cap) {
+        P.dlog_code[(size_t)i * P.dlog_cap + n_dec] = (uint8_t)((kind << 4) | (outcome & 15));
+        P.dlog_margin[(size_t)i * P.dlog_cap + n_dec] = (float)m;
+      }
+      ++n_dec;
     };
-    auto note_floor = [&](R f, int n) {        // f is floored to a voxel index in 0..n-1: distance to the nearest interior boundary
+    auto note_rel = [&](int kind, int outcome, R a, R b) {   // |a - b| relative to the larger magnitude
+      const double s = std::max(std::fabs((double)a), std::fabs((double)b));
+      note(kind, outcome, s > 0 ? std::fabs((double)a - (double)b) / s : 0.0);
+    };
+    auto note_floor = [&](int kind, int outcome, R f, int n) {   // f is floored to an index in 0..n-1: distance to the nearest interior boundary
       if (n <= 1) return;
       const double x = (double)f, k = std::min((double)(n - 1), std::max(1.0, std::round(x)));
-      note(std::fabs(x - k));
+      note(kind, outcome, std::fabs(x - k));
     };
     // §3.14 weighted mode: integer weight in tally quanta, W0 at launch.  Roulette (Iwabuchi 2006
     // as quoted in P:56): below W0/2 the photon survives with probability w/W0 exactly (a 32-bit word of
@@ -427,7 +455,8 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
       else if (r[1] <= r[2])            { axis = 1; t = r[1]; }
       else                              { axis = 2; t = r[2]; }
       R dtau = kh * t;
-      if (track && kh > 0) note_rel(tau, dtau);
+      if (track && kh > 0)                     // distance along the flight between the collision point and the face
+        note(DK_COLLIDE, tau <= dtau ? 1 : 0, std::fabs((double)tau / (double)kh - (double)t) / (double)del[lev][axis]);
       if (kh > 0 && tau <= dtau) {
         // ---- step 7: tentative collision inside this cell -------------------
         R s = tau * rk;
@@ -436,7 +465,7 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
         for (int a = 0; a < 3; ++a) {
           q[a] = local(a);
           gv[a] = c[a] * bs[a] + std::min((int)(q[a] * rds[a]), (lev ? mxyz[a] : 1) * bs[a] - 1);
-          if (track) note_floor(q[a] * rds[a], (lev ? mxyz[a] : 1) * bs[a]);
+          if (track) note_floor(DK_VOXEL, gv[a], q[a] * rds[a], (lev ? mxyz[a] : 1) * bs[a]);
         }
         size_t vox = ((size_t)gv[2] * ny + gv[1]) * nx + gv[0];
         Vox<R> vx = pack_voxel<R>(P.k_ext[vox], P.k_cloud[vox], P.ssa[vox], P.g[vox]);
@@ -445,10 +474,14 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
         R xi = u1 * kh;
         if (track) {
           const R x = P.weighted ? E::fma(u1, kh - vx.c1, vx.c1) : xi;
-          if (!P.weighted) note(std::fabs((double)x - (double)vx.c1) / (double)kh);
-          note(std::fabs((double)x - (double)vx.c2) / (double)kh);
-          note(std::fabs((double)x - (double)vx.c3) / (double)kh);
-          if (x < vx.c3) note(std::fabs(std::fabs((double)d[2]) - 0.99999));   // which rotation formula (§3.9)
+          const int cls = (!P.weighted && x < vx.c1) ? 0 : (x < vx.c2 ? 1 : (x < vx.c3 ? 2 : 3));
+          double m = std::min(std::fabs((double)x - (double)vx.c2), std::fabs((double)x - (double)vx.c3));
+          if (!P.weighted) m = std::min(m, std::fabs((double)x - (double)vx.c1));
+          note(DK_CLASS, cls, m / (double)kh);
+          if (cls == 1 || cls == 2) {            // which rotation formula (§3.9)
+            const double r2 = (double)E::fma(d[0], d[0], d[1] * d[1]);
+            note(DK_POLE, r2 > POLE_R2 ? 0 : 1, std::fabs(r2 - POLE_R2) / std::max(r2, POLE_R2));
+          }
         }
         if (P.weighted) {
           // §3.14: deposit w * P(absorbed), P = c1 / k_hat as a 24-bit fixed-point number; the rest goes on
@@ -466,14 +499,14 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
           if (direct && P.atm_abs_direct) add64(&P.atm_abs_direct[vox], W0);
           fate = ORC_ATM_ABS; term = (uint32_t)vox; break;
         } else if (xi < vx.c2) {               // cloud droplet: Henyey-Greenstein
-          R mu = sample_hg<R>(vx.g, u2);
+          R mu, sn; sample_hg<R>(vx.g, u2, mu, sn);
           R sp, cp; E::sincos_2pi(u3, sp, cp);
-          rotate_dir<R>(d[0], d[1], d[2], mu, cp, sp); set_dir(); place(q);
+          rotate_dir<R>(d[0], d[1], d[2], mu, sn, cp, sp); set_dir(); place(q);
           direct = false; ++n_sc; ++C.n_hg;
         } else if (xi < vx.c3) {               // gas: Rayleigh
-          R mu = sample_rayleigh<R>(u2);
+          R mu, sn; sample_rayleigh<R>(u2, mu, sn);
           R sp, cp; E::sincos_2pi(u3, sp, cp);
-          rotate_dir<R>(d[0], d[1], d[2], mu, cp, sp); set_dir(); place(q);
+          rotate_dir<R>(d[0], d[1], d[2], mu, sn, cp, sp); set_dir(); place(q);
           direct = false; ++n_sc; ++C.n_rayleigh;
         } else {
           ++C.n_null;                          // null collision: direction unchanged
@@ -488,7 +521,7 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
         // ---- step 5 (cont.): leave the cell through `axis` -------------------
         if (track) {                           // which face: the gap to the runner-up
           const R o1 = r[(axis + 1) % 3], o2 = r[(axis + 2) % 3];
-          note_rel(t, std::min(o1, o2));
+          note(DK_FACE, axis, std::fabs((double)std::min(o1, o2) - (double)t) / (double)del[lev][axis]);
         }
         tau = tau - dtau;
         ++C.n_cell_steps;
@@ -506,7 +539,7 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
           R qx = local(0), qy = local(1);
           int hx = c[0] * bx + std::min((int)(qx * rdx), (lev ? P.mx : 1) * bx - 1);
           int hy = c[1] * by + std::min((int)(qy * rdy), (lev ? P.my : 1) * by - 1);
-          if (track) { note_floor(qx * rdx, (lev ? P.mx : 1) * bx); note_floor(qy * rdy, (lev ? P.my : 1) * by); }
+          if (track) { note_floor(DK_COLUMN, hx, qx * rdx, (lev ? P.mx : 1) * bx); note_floor(DK_COLUMN, hy, qy * rdy, (lev ? P.my : 1) * by); }
           size_t col = (size_t)hy * nx + hx;
           if (at_top) {                        // step 11
             add64(&P.toa_up[col], P.weighted ? (int64_t)w : W0); ++C.n_toa;
@@ -527,7 +560,7 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
             reflect = true;
           } else {
             reflect = u1 < (R)P.albedo[col];
-            if (track) note(std::fabs((double)u1 - (double)P.albedo[col]));
+            if (track) note(DK_ALBEDO, reflect ? 1 : 0, std::fabs((double)u1 - (double)P.albedo[col]));
           }
           if (reflect) {
             R mu = std::sqrt((R)1 - u2), s = std::sqrt(u2);
@@ -569,7 +602,7 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
                 const int m = mxyz[a];
                 if (a != axis) {
                   const int k = std::min(m - 1, (int)(r[a] / del[0][a]));
-                  if (track) note_floor(r[a] / del[0][a], m);
+                  if (track) note_floor(DK_RELEVEL, k, r[a] / del[0][a], m);
                   r[a] = std::max((R)0, E::fma(-(R)k, del[0][a], r[a]));
                   c[a] += (v[a] > 0) ? (m - 1 - k) : k;
                 } else {
@@ -586,7 +619,8 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
       }
     }
     ++C.n_photons;
-    if (track) P.margins[i] = mg;
+    if (P.margins) P.margins[i] = mg;
+    if (P.dlog_count) P.dlog_count[i] = n_dec;
     if (P.records) {
       uint32_t* r = P.records + 4 * i;
       r[0] = (uint32_t)fate | (std::min(n_sfc, 0xFFFFFFu) << 8);
@@ -643,7 +677,8 @@ int orc_trace(int precision, int nx, int ny, int nz, float dx, float dy, float d
               uint64_t first_photon_id, uint64_t seed, uint32_t stream_id, int64_t* atm_abs,
               int64_t* sfc_dir, int64_t* sfc_dif, int64_t* sfc_abs, int64_t* toa_up,
               int64_t* atm_abs_direct, orc_counters* counters, uint32_t* records, int n_threads, double* elapsed_s,
-              double* margins, uint64_t range_begin, uint64_t range_count) {
+              double* margins, uint64_t range_begin, uint64_t range_count,
+              uint8_t* dlog_code, float* dlog_margin, uint32_t* dlog_count, uint32_t dlog_cap) {
   if (nx <= 0 || ny <= 0 || nz <= 0 || bx <= 0 || by <= 0 || bz <= 0) return -1;
   if (nx % bx || ny % by || nz % bz) return -1;
   if (mx <= 0 || my <= 0 || mz <= 0 || (nx / bx) % mx || (ny / by) % my || (nz / bz) % mz) return -1;
@@ -652,7 +687,8 @@ int orc_trace(int precision, int nx, int ny, int nz, float dx, float dy, float d
   if (!(diffuse_fraction >= 0.0f && diffuse_fraction <= 1.0f)) return -1;
   Problem P{nx, ny, nz, bx, by, bz, mx, my, mz, merge_ratio, weighted ? 1 : 0, diffuse_fraction, sobol ? 1 : 0, dx, dy, dz, k_ext, k_ext_cloud, ssa, g, sfc_albedo,
             zenith_deg, azimuth_deg, n_photons, first_photon_id, seed, stream_id,
-            atm_abs, sfc_dir, sfc_dif, sfc_abs, toa_up, atm_abs_direct, records, margins};
+            atm_abs, sfc_dir, sfc_dif, sfc_abs, toa_up, atm_abs_direct, records, margins,
+            dlog_code, dlog_margin, dlog_count, dlog_cap};
   // a PART of the job: photon indices [range_begin, range_begin + range_count) of the n_photons;
   // records and margins stay indexed by the index in the job
   if (range_begin > n_photons || range_count > n_photons - range_begin) return -1;
@@ -695,23 +731,28 @@ void orc_neg_log_f32(const float* w, float* out, uint64_t n) {
 void orc_sincos_2pi_f32(const float* u, float* sn, float* cs, uint64_t n) {
   for (uint64_t i = 0; i < n; ++i) spec_sincos_2pi(u[i], sn[i], cs[i]);
 }
-void orc_sample_hg(int precision, double g, const double* u, double* mu, uint64_t n) {
-  for (uint64_t i = 0; i < n; ++i)
-    mu[i] = precision == 64 ? sample_hg<double>(g, u[i]) : (double)sample_hg<float>((float)g, (float)u[i]);
+// mu and sin(theta) for each u (sn may be NULL)
+void orc_sample_hg(int precision, double g, const double* u, double* mu, double* sn, uint64_t n) {
+  for (uint64_t i = 0; i < n; ++i) {
+    if (precision == 64) { double m, s; sample_hg<double>(g, u[i], m, s); mu[i] = m; if (sn) sn[i] = s; }
+    else { float m, s; sample_hg<float>((float)g, (float)u[i], m, s); mu[i] = m; if (sn) sn[i] = s; }
+  }
 }
-void orc_sample_rayleigh(int precision, const double* u, double* mu, uint64_t n) {
-  for (uint64_t i = 0; i < n; ++i)
-    mu[i] = precision == 64 ? sample_rayleigh<double>(u[i]) : (double)sample_rayleigh<float>((float)u[i]);
+void orc_sample_rayleigh(int precision, const double* u, double* mu, double* sn, uint64_t n) {
+  for (uint64_t i = 0; i < n; ++i) {
+    if (precision == 64) { double m, s; sample_rayleigh<double>(u[i], m, s); mu[i] = m; if (sn) sn[i] = s; }
+    else { float m, s; sample_rayleigh<float>((float)u[i], m, s); mu[i] = m; if (sn) sn[i] = s; }
+  }
 }
-// d is 3 doubles in/out; rotation by polar cosine mu and azimuth 2*pi*u_phi.
-void orc_rotate(int precision, double* d, double mu, double u_phi) {
+// d is 3 doubles in/out; rotation by the polar angle (cosine mu, sine sn) and azimuth 2*pi*u_phi.
+void orc_rotate(int precision, double* d, double mu, double sn, double u_phi) {
   if (precision == 64) {
     double s, c; Elem<double>::sincos_2pi(u_phi, s, c);
-    rotate_dir<double>(d[0], d[1], d[2], mu, c, s);
+    rotate_dir<double>(d[0], d[1], d[2], mu, sn, c, s);
   } else {
     float a = (float)d[0], b = (float)d[1], cc = (float)d[2], s, c;
     Elem<float>::sincos_2pi((float)u_phi, s, c);
-    rotate_dir<float>(a, b, cc, (float)mu, c, s);
+    rotate_dir<float>(a, b, cc, (float)mu, (float)sn, c, s);
     d[0] = a; d[1] = b; d[2] = cc;
   }
 }

@@ -53,27 +53,66 @@ def test_rayleigh_inverse_cdf():
     assert abs(O.sample_rayleigh(np.array([1 - 2.0 ** -24]))[0] - 1.0) < 1e-6
 
 
+def test_hg_sine_keeps_relative_accuracy_at_the_forward_peak():
+    """DESIGN.md §3.9 computes 1 - mu and 1 + mu without cancellation and sin(theta) as the root of their product.
+    Pin: against the textbook inverse CDF evaluated with 60-digit arithmetic, the fp64 AND the fp32 sampler give
+    sin(theta) to a few ulp RELATIVE even where mu is within 1e-7 of 1 (sqrt(1 - mu^2) from a rounded fp32 mu
+    would be off by 100 % there), and mu^2 + sin^2 = 1."""
+    from mpmath import mp, mpf, sqrt as msqrt
+    mp.dps = 60
+    for g in (0.86, 0.85, 0.3, -0.4, 1e-4, 0.0):
+        us = [k / 2.0 ** 24 for k in (0, 1, 5, 1 << 12, 1 << 23, (1 << 24) - (1 << 10), (1 << 24) - 37, (1 << 24) - 1)]
+        mu64, s64 = O.sample_hg(g, np.array(us), with_sine=True)
+        mu32, s32 = O.sample_hg(float(np.float32(g)), np.array(us), precision=32, with_sine=True)
+        for j, u in enumerate(us):
+            for gg, mus, ss, eps in ((g, mu64, s64, 1e-14), (float(np.float32(g)), mu32, s32, 1e-6)):
+                G, U = mpf(gg), mpf(u)
+                if gg == 0.0:
+                    mu_x = 2 * U - 1
+                else:
+                    q = (1 - G * G) / (1 - G + 2 * G * U)
+                    mu_x = (1 + G * G - q * q) / (2 * G)
+                s_x = msqrt(max(mpf(0), 1 - mu_x * mu_x))
+                assert abs(mpf(float(mus[j])) - mu_x) <= eps, (gg, u)
+                assert abs(mpf(float(ss[j])) - s_x) <= eps * s_x * 4 + mpf(10) ** -30, (gg, u, float(ss[j]), float(s_x))
+        assert np.abs(mu64 ** 2 + s64 ** 2 - 1).max() < 1e-14
+
+
 def test_rotation_geometry():
     """New direction d' is a unit vector with d . d' = mu; azimuth 2 pi u turns d' around d through a
-    full circle (the perpendicular parts at u and u + 1/2 are opposite, at u + 1/4 orthogonal).  Within
-    |c| >= 0.99999 of the pole the algorithm treats d as exactly +-z, an error of at most
-    sqrt(1 - c^2) <= 4.5e-3 in d . d' that the test allows there and nowhere else."""
+    full circle (the perpendicular parts at u and u + 1/2 are opposite, at u + 1/4 orthogonal).  The frame is built
+    from a^2 + b^2, so the same tolerance holds 1e-4 rad from the pole as anywhere else; only
+    within 1e-6 rad (a^2 + b^2 <= 1e-12) is the direction taken as exactly +-z."""
     rng = np.random.default_rng(11)
-    for _ in range(300):
+    for it in range(400):
         d = rng.normal(size=3)
         d /= np.linalg.norm(d)
-        if rng.uniform() < 0.15:
-            d = np.array([1e-4 * rng.normal(), 1e-4 * rng.normal(), rng.choice([-1.0, 1.0])])
-            d /= np.linalg.norm(d)          # the |c| >= 0.99999 branch
+        if it % 6 == 0:
+            sc = 10.0 ** rng.uniform(-5.5, -2)
+            d = np.array([sc * rng.normal(), sc * rng.normal(), rng.choice([-1.0, 1.0])])
+            d /= np.linalg.norm(d)          # near a pole, still on the regular branch
         mu, u = rng.uniform(-1, 1), rng.uniform(0, 0.5)
         a = O.rotate(d, mu, u)
         b = O.rotate(d, mu, u + 0.5)
         c = O.rotate(d, mu, u + 0.25)
-        tol = 1e-9 if abs(d[2]) < 0.99999 else 1.01 * np.sqrt(1 - d[2] ** 2)
+        assert d[0] ** 2 + d[1] ** 2 > 1e-12
         for v in (a, b, c):
-            assert abs(np.linalg.norm(v) - 1) < 1e-12 and abs(v @ d - mu) <= tol
+            assert abs(np.linalg.norm(v) - 1) < 1e-12 and abs(v @ d - mu) <= 1e-9
         pa, pb, pc = a - mu * d, b - mu * d, c - mu * d
-        assert np.abs(pa + pb).max() < 1e-7 + 2 * tol and abs(pa @ pc) < 1e-7 + 2 * tol
+        assert np.abs(pa + pb).max() < 1e-7 and abs(pa @ pc) < 1e-7
+    # the pole branch: d = +-z exactly (and within 1e-6 rad of it): d' = (s cos, s sin, +-mu)
+    for sign in (1.0, -1.0):
+        for eps in (0.0, 3e-7):
+            v = O.rotate([eps, -eps, sign], 0.3, 0.125)
+            s = np.sqrt(1 - 0.09)
+            assert np.abs(v - np.array([s * np.cos(np.pi / 4), s * np.sin(np.pi / 4), sign * 0.3])).max() < 2e-6
+    # the first-order renormalisation 3/2 - n2/2 keeps the norm at 1 over a long chain of scatters, in fp32 too
+    for prec, tol in ((64, 1e-13), (32, 4e-7)):
+        d = np.array([0.6, 0.0, -0.8])
+        for j in range(2000):
+            d = O.rotate(d, float(np.cos(0.3 + 0.001 * j)), (0.61803398875 * j) % 1.0, precision=prec,
+                         sn=float(np.sin(0.3 + 0.001 * j)))
+        assert abs(np.linalg.norm(d) - 1) < tol
 
 
 # ------------------------------------------------------------------------------------------------
