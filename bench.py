@@ -29,11 +29,34 @@ UNIT = "paths/s"
 REF_SAMPLE_PHOTONS = 1 << 23      # per --impl reference step: 32 photons per column (~2 s on 16 cores)
 CPU_BASELINE_PHOTONS = 1 << 25    # cpu_baseline leg: 128 photons per column (~10 s on 16 cores)
 SECTOR = 32                       # bytes moved per random 16-byte gather (one DRAM/L2 sector)
-# thread instructions per unit of the method's work, counted in the shipped kernel's SASS
-# (profiles/r1b_trace_kernel.md E): one MOVE step (find the nearest face; cross or park),
-# one tentative collision (gather, classify, Philox draw, logarithm), one real scatter, one surface
-# or top arrival, one photon launch, one change of level at a merged cell's face.
-INST_PER_UNIT = {"move": 52, "collide": 190, "scatter": 250, "boundary": 150, "launch": 265, "relevel": 45}
+COUNTERS_FILE = os.path.join(ROOT, "profiles", "trace_kernel_counters.json")   # ncu counters per workload (text)
+KERNEL_SOURCES = ("rt_trace.cuh", "rt_device.cuh")   # what the trace kernel is compiled from: hashed into that file
+
+
+def _kernel_sha16():
+    """sha256 of the trace kernel's sources: an ncu entry only counts for the kernel it was captured from."""
+    import hashlib
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, "paper_2208_05247_b200", "csrc", name), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
+def _ncu_counters(cfg, mode, n):
+    """The committed ncu counters of the trace kernel for this workload, or None if there are none for the
+    kernel as it stands (profiles/trace_kernel_counters.md says how they were captured)."""
+    if not os.path.exists(COUNTERS_FILE):
+        return None
+    with open(COUNTERS_FILE) as f:
+        entries = json.load(f).get("entries", [])
+    sha = _kernel_sha16()
+    for e in entries:
+        if (e.get("workload") == cfg.name and e.get("mode") == mode and e.get("n_photons") == n
+                and e.get("block") == list(cfg.block) and e.get("merge") == list(cfg.merge)
+                and e.get("kernel_sha16") == sha):
+            return e
+    return None
 
 
 def _peaks():
@@ -183,9 +206,6 @@ def run_ours(args):
     n = cfg.n_photons                            # per GPU (weak scaling: photon ids are sharded by rank)
     g = rt.Grid(*cfg.grid, device=local, **cfg.accel)
     g.set_mode(weighted=(args.mode == "weighted"))
-    if args.kernel:
-        rt.binding.DEFAULT_KERNEL = rt.KERNEL_LANES if args.kernel == "lanes" else rt.KERNEL_POOL
-        g.set_kernel(rt.binding.DEFAULT_KERNEL)
     pinned_cols = rt.Tallies(None, *[torch.empty((cfg.ny, cfg.nx), dtype=torch.int64).pin_memory() for _ in range(4)],
                              counters=None)
     if spectral:
@@ -315,6 +335,35 @@ def run_ours(args):
     total_events = sum_over_ranks(events)
     value = total_photons / (elapsed_ms * 1e-3)
 
+    # ---- the path's one exchange step, outside the timed region ---------------------------
+    # One JOB of world x 2^22 photons split over the ranks by job index (rt_trace_range), then ONE exact int64
+    # all-reduce of the device tallies over NCCL: the merged tallies must close to the job's energy and every
+    # rank must hold the same sums.  (At world = 1 the same calls run without a collective.)
+    exchange = None
+    if not spectral:
+        from paper_2208_05247_b200.shard import job_range, allreduce_tallies
+        job = world * min(n, 1 << 22)
+        begin, count = job_range(rank, world, job)
+        g.reset_tallies()
+        g.trace_range(cfg.zenith_deg, cfg.azimuth_deg, job, begin, count, first_photon_id=1 << 40, seed=cfg.seed)
+        td = g.read_tallies(host=False)
+        parts = [td.atm_abs, td.sfc_dir, td.sfc_dif, td.sfc_abs, td.toa_up]
+        led = torch.tensor([td.counters.capped_energy + td.counters.roulette_lost - td.counters.roulette_gained,
+                            td.counters.n_photons], dtype=torch.int64, device=dev)
+        torch.cuda.synchronize(dev)
+        x0 = time.perf_counter()
+        allreduce_tallies(parts + [led])
+        torch.cuda.synchronize(dev)
+        x_ms = 1e3 * (time.perf_counter() - x0)
+        merged = int(td.atm_abs.sum()) + int(td.sfc_abs.sum()) + int(td.toa_up.sum()) + int(led[0])
+        ok = merged == job * rt.W0 and int(led[1]) == job
+        if not ok:
+            raise SystemExit("bench.py: all-reduced tallies do not close (%d of %d quanta)" % (merged, job * rt.W0))
+        exchange = {"tallies_allreduced": world > 1, "ranks": world, "job_photons": job, "closure_exact": bool(ok),
+                    "allreduce_bytes": sum(p.numel() * 8 for p in parts), "allreduce_ms": max_over_ranks(x_ms),
+                    "how": "rt_trace_range per rank + one int64 sum all-reduce (NCCL) of atm_abs and the four column tallies"}
+        del td, parts
+
     # ---- end-to-end leg: host fields in, all tallies out to the host, every step --------------------------
     # Two contexts on two streams, steps alternating: while one context traces, the other uploads its next fields
     # (pinned host memory, inside rt_set_optics) and downloads its last tallies (rt_read_tallies_async), so the
@@ -415,37 +464,50 @@ def run_ours(args):
                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "how": how}
 
     # ---- roofline of the dominant kernel (trace_kernel), this rank ---------------------------------------
-    # The kernel is bound by instruction issue, not by memory (0.5 % of the HBM copy rate, 80 %
-    # of issue slots busy), so the bound is "alu".  Algorithmic work = thread instructions the method's steps
-    # need, per unit, as counted in the shipped kernel's SASS (profiles/r1b_trace_kernel.md) x the units the
-    # launch processed; peak = every lane of every SM sub-partition issuing each cycle at the SM clock.
+    # the path's bound is the memory GATHER rate.  Two ceilings are measured in this run by
+    # rt_gather_bench (8 independent random 16 B loads in flight per thread = one 32 B sector each): over the whole
+    # packed-optics array (HBM) and over its first 16 MiB (L2).  The time a perfect kernel would need for THIS
+    # launch's memory work is max(L2 read sectors / L2 gather rate, DRAM read sectors / HBM gather rate), with the
+    # sector counts of the shipped kernel from the committed ncu capture (profiles/trace_kernel_counters.json,
+    # keyed by the kernel sources' hash); frac = that time / the kernel's measured time = achieved events/s over
+    # the events/s the ceiling allows.  Without a capture of the kernel as it stands, the algorithmic model of
+    # §8(d) is used: one 32 B sector from HBM per tentative collision.
     hbm_peak, peak_src = _peaks()
     ms_avg = sum(trace_ms) / len(trace_ms)
     per = {k: v / args.steps for k, v in csum.items()}
-    units = {"move": per["n_cell_steps"] + per["n_events"], "collide": per["n_events"],
-             "scatter": per["n_hg"] + per["n_rayleigh"], "boundary": per["n_sfc_hits"] + per["n_toa"],
-             "launch": per["n_photons"], "relevel": per["n_relevel"]}
-    alg_inst = sum(INST_PER_UNIT[k] * units[k] for k in units)
-    sm_mhz = _sm_max_mhz()
-    alu_peak = 148 * 4 * 32 * sm_mhz * 1e6 / 1e12            # T thread-instructions / s
-    achieved = alg_inst / (ms_avg * 1e-3) / 1e12
     ev_per_launch = per["n_events"]
     atomics_per_launch = n + per["n_sfc_hits"]
     alg_bytes = SECTOR * ev_per_launch + 2 * SECTOR * atomics_per_launch
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "trace_kernel_traffic.txt")
-    if os.path.exists(tpath):
-        with open(tpath) as f:
-            tj = json.load(f)
-        if (tj.get("n_photons") == n and tj.get("workload") == cfg.name and tj.get("block") == list(cfg.block)
-                and tj.get("merge", [1, 1, 1]) == list(cfg.merge)):
-            traffic = tj.get("dram_bytes_per_launch")
     trace_events_per_s = ev_per_launch / (ms_avg * 1e-3)
-    trace_gathers_per_s = (units["move"] + units["collide"]) / (ms_avg * 1e-3)   # majorant + voxel loads
+    trace_gathers_per_s = (per["n_cell_steps"] + 2 * per["n_events"]) / (ms_avg * 1e-3)   # majorant + voxel loads
     gather = {}
-    for label, foot in (("hbm_512MiB", 0), ("l2_16MiB", min(1 << 20, cfg.nvox))):   # labels name config 3's sizes
+    for label, foot in (("hbm_whole_array", 0), ("l2_16MiB", min(1 << 20, cfg.nvox))):
         gb_ms, gb_loads = g.gather_bench(64, foot)
         gather[label] = gb_loads / (gb_ms * 1e-3)
+    ncu = _ncu_counters(cfg, args.mode, n) if not spectral else None
+    if ncu:
+        t_l2 = ncu["lts_t_sectors_op_read"] / gather["l2_16MiB"]
+        t_hbm = ncu["dram_bytes_read"] / SECTOR / gather["hbm_whole_array"]
+        t_roof = max(t_l2, t_hbm)
+        traffic = ncu["dram_bytes_read"] + ncu["dram_bytes_write"]
+        model = ("max(L2 read sectors / L2 gather rate, DRAM read sectors / HBM gather rate); sector counts from "
+                 "profiles/trace_kernel_counters.json (kernel_sha16 %s), gather rates measured in this run" % ncu["kernel_sha16"])
+        sm_mhz = _sm_max_mhz()
+        lane_peak = 148 * 4 * 32 * sm_mhz * 1e6
+        alu = {"thread_inst_per_launch": ncu["thread_inst_executed"], "warp_inst_per_launch": ncu["inst_executed"],
+               "active_lanes_per_inst": ncu["thread_inst_executed"] / ncu["inst_executed"],
+               "issue_active_pct_ncu": ncu["issue_active_pct"],
+               "lane_slots_used": ncu["thread_inst_executed"] / (ms_avg * 1e-3) / lane_peak,
+               "issue_slots_used": ncu["inst_executed"] / (ms_avg * 1e-3) / (148 * 4 * sm_mhz * 1e6),
+               "peak": "148 SMs x 4 sub-partitions x 32 lanes x %.0f MHz; instruction counts measured by ncu" % sm_mhz}
+    else:
+        t_l2, t_hbm = None, ev_per_launch / gather["hbm_whole_array"]
+        t_roof = t_hbm
+        traffic = None
+        alu = None
+        model = ("no ncu capture of the kernel as it stands: SURVEY.md 8(d)'s algorithmic model, one 32 B sector from "
+                 "HBM per tentative collision")
+    roof_events_per_s = ev_per_launch / t_roof
 
     if rank != 0:
         if world > 1:
@@ -489,23 +551,21 @@ def run_ours(args):
         "gpu_launches": launches,
         "closure_exact": bool(closure_ok),
         "clocks": clocks,
-        "roofline": {"bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "T thread-inst/s",
-                     "frac": achieved / alu_peak, "traffic": traffic, "kernel": "trace_kernel",
-                     "peak_source": "148 SMs x 4 sub-partitions x 32 lanes x %.0f MHz (DESIGN.md §6)" % sm_mhz,
-                     "algorithmic_inst_per_launch": alg_inst, "inst_per_unit": INST_PER_UNIT,
-                     "units_per_launch": units},
+        "roofline": {"bound": "gather", "achieved": trace_events_per_s, "peak": roof_events_per_s,
+                     "unit": "tentative collisions/s", "frac": trace_events_per_s / roof_events_per_s,
+                     "traffic": traffic, "kernel": "trace_kernel", "model": model,
+                     "events_per_launch": ev_per_launch, "kernel_ms": ms_avg,
+                     "roof_ms": 1e3 * t_roof, "roof_ms_l2": None if t_l2 is None else 1e3 * t_l2, "roof_ms_hbm": 1e3 * t_hbm,
+                     "gather_sectors_per_s": gather,
+                     "frac_events_vs_hbm_gather": trace_events_per_s / gather["hbm_whole_array"],
+                     "frac_all_gathers_vs_l2_gather": trace_gathers_per_s / gather["l2_16MiB"],
+                     "ncu": ncu},
+        "alu": alu,
         "hbm": {"algorithmic_GBps": alg_bytes / (ms_avg * 1e-3) / 1e9, "peak_GBps": hbm_peak, "peak_source": peak_src,
                 "frac": alg_bytes / (ms_avg * 1e-3) / 1e9 / hbm_peak,
-                "bytes_model": "32 B sector per tentative collision + 2 x 32 B per tally atomic; ncu shows the "
-                               "real DRAM traffic (roofline.traffic) is ~100x smaller: the working set sits in L2"},
-        "gather_roofline": {"random_16B_loads_per_s": gather, "trace_events_per_s": trace_events_per_s,
-                            "trace_gathers_per_s": trace_gathers_per_s,
-                            "frac_events_vs_hbm": trace_events_per_s / gather["hbm_512MiB"],
-                            "frac_gathers_vs_hbm": trace_gathers_per_s / gather["hbm_512MiB"],
-                            "frac_gathers_vs_l2": trace_gathers_per_s / gather["l2_16MiB"],
-                            "how": "rt_gather_bench: 8 independent random 16 B loads in flight per thread over the "
-                                   "whole 512 MiB packed-optics array (HBM) and over its first 16 MiB (L2); "
-                                   "trace gathers = voxel records + 4 B majorant loads"},
+                "bytes_model": "32 B sector per tentative collision + 2 x 32 B per tally atomic (SURVEY.md 8(d)), "
+                               "against the streaming copy rate: context only, a random gather cannot reach it"},
+        "exchange": exchange,
         "cpu_baseline": cpu,
     }))
     if world > 1:
@@ -534,8 +594,6 @@ def main():
     ap.add_argument("--full-fields", action="store_true",
                     help="workload 4: give every point's optics as four full 3-D fields (rt_set_optics_slot) instead of "
                          "as factors (one cloud field + per-level gas profiles per point, rt_set_optics_factored)")
-    ap.add_argument("--kernel", choices=("pool", "lanes"), default=None,
-                    help="trace kernel (include/rt.h rt_set_kernel): pool (the library's default) or lanes")
     ap.add_argument("--e2e-serial", action="store_true", help="e2e leg on one context with synchronous copies")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing (used under ncu)")
     args = ap.parse_args()

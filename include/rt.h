@@ -34,7 +34,7 @@ extern "C" {
 #define RT_ENOMEM (-2)   /* device allocation failed */
 #define RT_ECUDA (-3)    /* a CUDA call or kernel failed; see rt_last_error */
 #define RT_EOPTICS (-4)  /* rt_set_optics: a field value is outside its physical range */
-#define RT_ESTATE (-5)   /* rt_trace before rt_set_optics */
+#define RT_ESTATE (-5)   /* a call before the call it needs: rt_trace before rt_set_optics, slots before rt_set_slots, ... */
 
 #define RT_W0 (1ll << 32) /* tally quanta per photon */
 
@@ -106,18 +106,8 @@ int rt_trace_range(rt_ctx* ctx, double zenith_deg, double azimuth_deg, uint64_t 
                    uint64_t first_photon_id, uint64_t seed, uint32_t stream_id, void* cuda_stream,
                    uint64_t range_begin, uint64_t range_count, uint32_t* records_out);
 
-/* Which kernel traces.  Both follow the same per-photon operation sequence, so
- * photon records, tallies and counters are identical; only the schedule differs.
- * RT_KERNEL_POOL (default): every warp keeps a pool of photons in shared memory, sorted by the phase they wait
- *   for, and runs each phase with full warps (rt_trace_pool.cuh).  Used when the launch has fewer than 2^32
- *   photons and the acceleration grid has at most 2048 x 2048 x 896 cells; otherwise the library falls back to
- * RT_KERNEL_LANES: one photon per lane, phases scheduled by warp votes (rt_trace.cuh).
- * Errors: RT_EINVAL. */
-#define RT_KERNEL_POOL 0
-#define RT_KERNEL_LANES 1
-int rt_set_kernel(rt_ctx* ctx, int kernel);
-
-/* Synchronise the context's device work and copy tallies out.  Each output may be a host or a
+/* Wait for the work THIS context has queued (on whichever streams its calls were given; other work on the
+ * device is not waited for) and copy tallies out.  Each output may be a host or a
  * device pointer (detected), or NULL to skip: atm_abs nvox int64 in [z][y][x]; the others ncol
  * int64 in [y][x]; counters is a HOST pointer or NULL.  Energy closure: sum(atm_abs) +
  * sum(sfc_abs) + sum(toa_up) + capped_energy == n_photons * RT_W0 exactly. */
@@ -138,8 +128,8 @@ int rt_read_tallies_async(rt_ctx* ctx, int64_t* atm_abs, int64_t* sfc_dir, int64
  * cell.  Any majorant >= k_ext gives the same expectations, so only the sample paths change.
  * mx, my, mz: powers of two, at most 64, dividing the acceleration grid's extents; 1,1,1 (the default after
  * rt_create_grid) = single-level grid.  merge_ratio >= 1.  Takes effect at the next rt_set_optics;
- * a context that already holds optics must be given them again before the next rt_trace
- * (RT_ESTATE otherwise).  Errors: RT_EINVAL. */
+ * a context that already holds optics (in any slot) must be given them again before the next rt_trace or
+ * rt_trace_batch: every majorant table was built for the old factors (RT_ESTATE otherwise).  Errors: RT_EINVAL. */
 int rt_set_merge(rt_ctx* ctx, int mx, int my, int mz, float merge_ratio);
 
 /* Absorption scheme of the following rt_trace calls.
@@ -174,10 +164,13 @@ int rt_set_source(rt_ctx* ctx, float diffuse_fraction, int sampler);
  * and slot: 112 points of the 512x512x128 grid = 57 GB of the B200's 180 GB), and ONE launch traces the photons
  * of all points, so that no launch drains between points and the host does not wait per point.
  * rt_set_slots: (re)allocates the slots (n_slots * nvox < 2^32; the 16 B x nvox records of the slots above 0 are
- *   allocated when the first of them is set); slot 0 is the one rt_set_optics and rt_trace use; every slot must be given optics again afterwards.  Synchronises the device.
- * rt_set_optics_slot: rt_set_optics into slot `slot`, asynchronous on `cuda_stream`: range errors accumulate on
- *   the device and are reported by the next rt_trace_batch (RT_EOPTICS).  Host fields are accepted but make
- *   the call wait for the stream.
+ *   allocated when the first of them is set); every slot must be given optics again afterwards.  Waits for the
+ *   context's queued work.  Slot 0 is the one rt_set_optics writes and rt_trace reads; rt_trace itself needs
+ *   rt_set_optics (which validates before returning): after rt_set_optics_slot(0), rt_set_optics_factored(0) or
+ *   rt_set_point(0) slot 0 serves rt_trace_batch only and rt_trace returns RT_ESTATE until rt_set_optics is called.
+ * rt_set_optics_slot: rt_set_optics into slot `slot`, asynchronous on `cuda_stream`: range errors are kept per
+ *   slot on the device (setting a slot again clears its mask) and the next rt_trace_batch that launches the slot
+ *   reports them, naming it (RT_EOPTICS).  Host fields are accepted but make the call wait for the stream.
  * rt_trace_batch: point j (first_point <= j < first_point + n_points <= n_slots) is traced with
  *   counts[j - first_point] photons (HOST array), stream id j, slot j, global photon ids first_photon_id + (index within the point), its own column stratification
  *   (full passes over the columns + remainder), i.e. exactly what rt_trace(..., counts[j], first_photon_id, seed,
@@ -194,8 +187,8 @@ int rt_set_optics_slot(rt_ctx* ctx, int slot, const float* k_ext, const float* k
  * k_cloud ([z][y][x], nvox) and sfc_albedo (ncol) are DEVICE pointers (the cloud field is shared by all points
  * and uploaded once); k_abs, k_ray (nz each) may be HOST or DEVICE.  Reads 4 B per voxel instead of 16 and
  * needs 2 nz numbers per point from the host.  Asynchronous like rt_set_optics_slot (errors of the field values
- * at the next rt_trace_batch).  Requires nx % 4 == 0, bx in {1, 2, 4}, by * bz <= 64.  Errors: RT_EINVAL,
- * RT_EOPTICS (cloud_ssa, cloud_g out of range), RT_ENOMEM, RT_ECUDA. */
+ * at the next rt_trace_batch).  Requires rt_set_slots beforehand (RT_ESTATE), nx % 4 == 0, bx in {1, 2, 4},
+ * by * bz <= 64.  Errors: RT_EINVAL, RT_ESTATE, RT_EOPTICS (cloud_ssa, cloud_g out of range), RT_ENOMEM, RT_ECUDA. */
 int rt_set_optics_factored(rt_ctx* ctx, int slot, const float* k_cloud, const float* k_abs, const float* k_ray,
                            float cloud_ssa, float cloud_g, const float* sfc_albedo, void* cuda_stream);
 /* Factored optics kept factored in the trace as well (NEXT-3 in full).  rt_set_cloud stores the cloud extinction

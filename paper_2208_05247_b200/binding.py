@@ -11,10 +11,8 @@ LIB_PATH = os.path.join(HERE, "librt_b200.so")
 W0 = 1 << 32
 FATE_ATM_ABS, FATE_SFC_ABS, FATE_TOD_EXIT, FATE_CAPPED, FATE_ROULETTE = 1, 2, 3, 4, 5
 MODE_ANALOG, MODE_WEIGHTED = 0, 1
-KERNEL_POOL, KERNEL_LANES = 0, 1
-DEFAULT_KERNEL = None   # None = the library's default (the pool kernel); tests set it to run both kernels
 
-EXPORTS = ("rt_create_grid", "rt_set_merge", "rt_set_mode", "rt_set_source", "rt_set_optics", "rt_set_slots", "rt_set_optics_slot", "rt_set_optics_factored", "rt_set_cloud", "rt_set_point", "rt_trace_batch", "rt_trace", "rt_trace_records", "rt_trace_range", "rt_set_kernel", "rt_read_tallies", "rt_read_tallies_async",
+EXPORTS = ("rt_create_grid", "rt_set_merge", "rt_set_mode", "rt_set_source", "rt_set_optics", "rt_set_slots", "rt_set_optics_slot", "rt_set_optics_factored", "rt_set_cloud", "rt_set_point", "rt_trace_batch", "rt_trace", "rt_trace_records", "rt_trace_range", "rt_read_tallies", "rt_read_tallies_async",
            "rt_reset_tallies", "rt_set_heating_split", "rt_read_heating_direct", "rt_tally_to_flux", "rt_read_majorant", "rt_read_packed_optics", "rt_gather_bench",
            "rt_last_trace_ms", "rt_launch_count", "rt_philox_words", "rt_last_error", "rt_destroy")
 
@@ -62,7 +60,6 @@ def lib():
     L.rt_trace.argtypes = [vp, f64, f64, u64, u64, u64, u32, vp]
     L.rt_trace_records.argtypes = [vp, f64, f64, u64, u64, u64, u32, vp, vp]
     L.rt_trace_range.argtypes = [vp, f64, f64, u64, u64, u64, u32, vp, u64, u64, vp]
-    L.rt_set_kernel.argtypes = [vp, i32]
     L.rt_read_tallies.argtypes = [vp, vp, vp, vp, vp, vp, C.POINTER(rt_counters)]
     L.rt_read_tallies_async.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
     L.rt_reset_tallies.argtypes = [vp, vp]
@@ -145,8 +142,6 @@ class Grid:
             raise RtError("rt_create_grid failed (%d): %s" % (rc, msg))
         if tuple(merge) != (1, 1, 1):
             self.set_merge(*merge, merge_ratio=merge_ratio)
-        if DEFAULT_KERNEL is not None:
-            self.set_kernel(DEFAULT_KERNEL)
 
     def set_merge(self, mx, my, mz, merge_ratio=1.25):
         """Merged acceleration cells (include/rt.h rt_set_merge); call before set_optics."""
@@ -245,10 +240,6 @@ class Grid:
                                           int(seed), int(stream_id), _stream(self.device), int(range_begin),
                                           int(range_count), _ptr(rec)), "rt_trace_range")
         return rec[:int(range_count)] if records else None
-
-    def set_kernel(self, kernel):
-        """include/rt.h rt_set_kernel: KERNEL_POOL (default) or KERNEL_LANES; same photons either way."""
-        self._check(self.L.rt_set_kernel(self.ctx, int(kernel)), "rt_set_kernel")
 
     def read_tallies(self, host=True, atm_abs=True, out=None):
         """Copy tallies out.  `out` = an earlier Tallies whose (e.g. pinned host) buffers are reused."""

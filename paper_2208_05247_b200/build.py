@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "librt_b200.so")
 SOURCES = ["rt.cu"]
-DEPS = ["rt.cu", "rt_device.cuh", "rt_setup.cuh", "rt_trace.cuh", "rt_trace_pool.cuh", os.path.join("..", "..", "include", "rt.h")]
+DEPS = ["rt.cu", "rt_device.cuh", "rt_setup.cuh", "rt_trace.cuh", os.path.join("..", "..", "include", "rt.h")]
 
 # -fmad=false: no implicit contraction; every FMA in the kernels is written explicitly so the
 # fp32 decisions are reproducible operation by operation.
@@ -33,8 +33,7 @@ def up_to_date() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and up_to_date():
         return OUT
-    extra = os.environ.get("RT_NVCC_EXTRA", "").split()   # e.g. -DRT_TRAVERSE_WEIGHT=3 when tuning
-    cmd = [_nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + \
+    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
           [os.path.join(CSRC, s) for s in SOURCES] + ["-o", OUT]
     subprocess.check_call(cmd)
     return OUT

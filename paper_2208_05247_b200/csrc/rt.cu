@@ -7,11 +7,11 @@
 #include <cstdio>
 #include <cstring>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "rt_setup.cuh"
 #include "rt_trace.cuh"
-#include "rt_trace_pool.cuh"
 
 struct rt_ctx {
   int device = 0;
@@ -43,14 +43,16 @@ struct rt_ctx {
   float* albedo = nullptr;
   unsigned long long* tallies = nullptr;  // atm_abs | sfc_dir | sfc_dif | sfc_abs | toa_up
   unsigned long long* counters = nullptr; // C_COUNT words, then the work counter
-  int* bad = nullptr;
+  int* bad = nullptr;                     // range-error masks on the device: one word per slot, then one for rt_set_cloud
   float* sink = nullptr;
   float* stage = nullptr;                 // 4 nvox + ncol floats; only allocated when a caller passes host fields
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   bool have_optics = false, have_trace = false;
-  int kernel = RT_KERNEL_LANES;           // rt_set_kernel: which scheduler traces (same photons either way)
-  bool pool_fits = true;                  // the grid fits the pool kernel's packed cell index
-  int trace_blocks[2][16] = {};           // persistent grid size per kernel instantiation, [pool][records | pow2 | weighted | batch]; 0 = not asked yet
+  int trace_blocks[16] = {};              // persistent grid size per kernel instantiation [records | pow2 | weighted | batch]; 0 = not asked yet
+  // streams this context has queued work on since the last wait, each with an event recorded after the latest
+  // piece of work: rt_read_tallies waits for these instead of the whole device
+  std::vector<std::pair<cudaStream_t, cudaEvent_t>> pending;
+  cudaStream_t copy_stream = nullptr;     // non-blocking stream of the synchronous read-outs
   int sm_count = 0;
   uint64_t launches = 0;
   std::string err;
@@ -78,6 +80,22 @@ int fail(rt_ctx* c, int code, const char* what, cudaError_t ce = cudaSuccess) {
     if (ce_ != cudaSuccess) return fail(ctx, ce_ == cudaErrorMemoryAllocation ? RT_ENOMEM : RT_ECUDA, #call, ce_); \
   } while (0)
 
+// Remember that `st` now carries work of this context (an event after it), for rt_read_tallies' wait.
+int mark(rt_ctx* c, cudaStream_t st) {
+  for (auto& p : c->pending)
+    if (p.first == st) { RT_CUDA(c, cudaEventRecord(p.second, st)); return RT_OK; }
+  cudaEvent_t ev = nullptr;
+  RT_CUDA(c, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+  c->pending.emplace_back(st, ev);
+  RT_CUDA(c, cudaEventRecord(ev, st));
+  return RT_OK;
+}
+// Wait for everything this context has queued, on whichever streams (not for other work on the device).
+int wait_pending(rt_ctx* c) {
+  for (auto& p : c->pending) RT_CUDA(c, cudaEventSynchronize(p.second));
+  return RT_OK;
+}
+
 unsigned long long* tally_ptr(rt_ctx* c, int which) {  // 0 atm_abs, 1..4 the column tallies
   return which == 0 ? c->tallies : c->tallies + c->nvox + (size_t)(which - 1) * c->ncol;
 }
@@ -99,31 +117,22 @@ const float* stage_input(rt_ctx* c, const float* p, size_t n, size_t slot_offset
   return dst;
 }
 
-// One source, 16 instantiations per scheduler: <records, power-of-two wrap, weighted, batch>.
-struct KernelInfo { const void* fn; int threads; size_t smem; };
-template <bool R, bool P, bool W, bool B> KernelInfo kernel_info(bool pool) {
-  if (pool) return {(const void*)rt::trace_pool_kernel<R, P, W, B>, rt::kPoolThreads, rt::pool_smem_bytes(R || W || B)};
-  return {(const void*)rt::trace_kernel<R, P, W, B>, rt::kTraceThreads, 0};
-}
-KernelInfo pick_kernel(int variant, bool pool) {
+// One source, 16 instantiations: <records, power-of-two wrap, weighted, batch>.
+const void* pick_kernel(int variant) {
   switch (variant) {
-#define RT_CASE(v) case v: return kernel_info<((v) & 1) != 0, ((v) & 2) != 0, ((v) & 4) != 0, ((v) & 8) != 0>(pool);
+#define RT_CASE(v) case v: return (const void*)rt::trace_kernel<((v) & 1) != 0, ((v) & 2) != 0, ((v) & 4) != 0, ((v) & 8) != 0>;
     RT_CASE(0) RT_CASE(1) RT_CASE(2) RT_CASE(3) RT_CASE(4) RT_CASE(5) RT_CASE(6) RT_CASE(7)
     RT_CASE(8) RT_CASE(9) RT_CASE(10) RT_CASE(11) RT_CASE(12) RT_CASE(13) RT_CASE(14) RT_CASE(15)
 #undef RT_CASE
   }
-  return {nullptr, 0, 0};
+  return nullptr;
 }
-// Persistent grid of one instantiation: resident blocks per SM (occupancy query, once) x SM count.
-int trace_grid(rt_ctx* c, int variant, bool pool, const KernelInfo& k, int* blocks_out) {
-  int& cached = c->trace_blocks[pool ? 1 : 0][variant];
+// Persistent grid of one instantiation: resident blocks per SM (occupancy query, once per instantiation) x SM count.
+int trace_grid(rt_ctx* c, int variant, const void* fn, int* blocks_out) {
+  int& cached = c->trace_blocks[variant];
   if (cached == 0) {
-    if (k.smem > 0)   // static + dynamic shared memory pass the 48 KB that need no opt-in
-      RT_CUDA(c, cudaFuncSetAttribute(k.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.smem));
-    if (pool)   // the photon pools want the shared-memory side of the L1 / shared-memory split
-      RT_CUDA(c, cudaFuncSetAttribute(k.fn, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     int per_sm = 0;
-    RT_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k.fn, k.threads, k.smem));
+    RT_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, rt::kTraceThreads, 0));
     if (per_sm < 1) return fail(c, RT_ECUDA, "rt_trace: the trace kernel does not fit on an SM");
     cached = c->sm_count * per_sm;
   }
@@ -168,13 +177,10 @@ int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photon
   A.n_photons = n_photons; A.first_id = first_id; A.ncol = c->ncol; A.index_base = index_base;
   A.n_full = (job_photons / c->ncol) * c->ncol;
   const bool pow2 = !(c->ncx & (c->ncx - 1)) && !(c->ncy & (c->ncy - 1));
-  // the pool kernel keeps a photon's index in 32 bits and its cell index packed: larger launches and grids go to
-  // the one-photon-per-lane kernel (same photons)
-  const bool pool = c->kernel == RT_KERNEL_POOL && c->pool_fits && n_photons < (1ull << 32);
   const int variant = (records ? 1 : 0) | (pow2 ? 2 : 0) | (c->weighted ? 4 : 0) | (n_points > 0 ? 8 : 0);
-  const KernelInfo kinfo = pick_kernel(variant, pool);
+  const void* fn = pick_kernel(variant);
   int blocks = 0;
-  if (int rcg = trace_grid(c, variant, pool, kinfo, &blocks)) return rcg;
+  if (int rcg = trace_grid(c, variant, fn, &blocks)) return rcg;
   {
     // ids per work-counter atomic: 128, or fewer (a multiple of 32) when the launch has under ~8 chunks per warp,
     // so that short launches (one spectral point of config 4) balance over all resident warps
@@ -193,13 +199,13 @@ int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photon
   RT_CUDA(c, cudaEventRecord(c->ev0, st));
   if (n_photons > 0) {
     void* kargs[1] = {(void*)&A};
-    RT_CUDA(c, cudaLaunchKernel(kinfo.fn, dim3((unsigned)blocks), dim3((unsigned)kinfo.threads), kargs, kinfo.smem, st));
+    RT_CUDA(c, cudaLaunchKernel(fn, dim3((unsigned)blocks), dim3((unsigned)rt::kTraceThreads), kargs, 0, st));
     ++c->launches;
   }
   RT_CUDA(c, cudaEventRecord(c->ev1, st));
   RT_CUDA(c, cudaGetLastError());
   c->have_trace = true;
-  return RT_OK;
+  return mark(c, st);
 }
 
 }  // namespace
@@ -230,15 +236,15 @@ int rt_create_grid(rt_ctx** out, int nx, int ny, int nz, float dx, float dy, flo
   RT_CUDA(c, cudaMalloc(&c->albedo, c->ncol * sizeof(float)));
   RT_CUDA(c, cudaMalloc(&c->tallies, ntally * sizeof(unsigned long long)));
   RT_CUDA(c, cudaMalloc(&c->counters, (rt::C_COUNT + 1) * sizeof(unsigned long long)));
-  RT_CUDA(c, cudaMalloc(&c->bad, sizeof(int)));
+  RT_CUDA(c, cudaMalloc(&c->bad, 2 * sizeof(int)));
+  RT_CUDA(c, cudaMemset(c->bad, 0, 2 * sizeof(int)));
+  RT_CUDA(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
   RT_CUDA(c, cudaMalloc(&c->sink, sizeof(float)));
   RT_CUDA(c, cudaMemset(c->tallies, 0, ntally * sizeof(unsigned long long)));
   RT_CUDA(c, cudaMemset(c->counters, 0, (rt::C_COUNT + 1) * sizeof(unsigned long long)));
   RT_CUDA(c, cudaEventCreate(&c->ev0));
   RT_CUDA(c, cudaEventCreate(&c->ev1));
   RT_CUDA(c, cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, cuda_device));
-  // the pool kernel packs (cx, cy, cz + 64) into 11 + 11 + 10 bits (rt_trace_pool.cuh)
-  c->pool_fits = c->ncx <= 2048 && c->ncy <= 2048 && c->ncz <= 896;
   return RT_OK;
 }
 
@@ -251,7 +257,7 @@ namespace {
 int ensure_optics_slots(rt_ctx* c, int slot) {
   if (slot < c->optics_slots) return RT_OK;
   DeviceGuard guard(c->device);
-  RT_CUDA(c, cudaDeviceSynchronize());
+  if (int rcw = wait_pending(c)) return rcw;
   float4* grown = nullptr;
   RT_CUDA(c, cudaMalloc(&grown, (size_t)c->n_slots * c->nvox * sizeof(float4)));
   RT_CUDA(c, cudaMemcpy(grown, c->optics, (size_t)c->optics_slots * c->nvox * sizeof(float4), cudaMemcpyDeviceToDevice));
@@ -261,8 +267,9 @@ int ensure_optics_slots(rt_ctx* c, int slot) {
   return RT_OK;
 }
 
-// S0 + S1 into optics / majorant / albedo slot `slot`.  sync: wait for the kernels and report range errors now
-// (rt_set_optics); otherwise the error mask accumulates on the device until rt_trace_batch reads it.
+// S0 + S1 into optics / majorant / albedo slot `slot`.  Range errors go to the slot's own mask word (cleared here,
+// so re-setting a slot with good data heals it).  sync: wait for the kernels and report the mask now
+// (rt_set_optics); otherwise rt_trace_batch reads the masks of the slots it launches.
 int set_optics_impl(rt_ctx* c, int slot, const float* k_ext, const float* k_ext_cloud, const float* ssa,
                     const float* g, const float* sfc_albedo, cudaStream_t st, bool sync, const char* who) {
   if (!k_ext || !k_ext_cloud || !ssa || !g || !sfc_albedo) return fail(c, RT_EINVAL, "rt_set_optics: NULL field");
@@ -283,7 +290,8 @@ int set_optics_impl(rt_ctx* c, int slot, const float* k_ext, const float* k_ext_
   float* albedo = c->albedo + (size_t)slot * c->ncol;
   const bool rows = (c->nx % 4 == 0) && !(((uintptr_t)k_ext | (uintptr_t)k_ext_cloud | (uintptr_t)ssa | (uintptr_t)g) & 15u);
   const bool cellrows = rows && (c->bx == 1 || c->bx == 2 || c->bx == 4) && c->by * c->bz <= 64;   // no atomics, no zeroing
-  if (sync) RT_CUDA(c, cudaMemsetAsync(c->bad, 0, sizeof(int), st));
+  int* bad = c->bad + slot;
+  RT_CUDA(c, cudaMemsetAsync(bad, 0, sizeof(int), st));
   if (!cellrows) RT_CUDA(c, cudaMemsetAsync(khat, 0, c->ncell * sizeof(float), st));
   RT_CUDA(c, cudaMemcpyAsync(albedo, sfc_albedo, c->ncol * sizeof(float), cudaMemcpyDeviceToDevice, st));
   const int blocks = c->sm_count * 8;
@@ -295,16 +303,16 @@ int set_optics_impl(rt_ctx* c, int slot, const float* k_ext, const float* k_ext_
   if (cellrows)
     rt::pack_optics_cellrows_kernel<<<c->sm_count * 16, 128, 0, st>>>(
         (const float4*)k_ext, (const float4*)k_ext_cloud, (const float4*)ssa, (const float4*)g, optics,
-        khat, merging ? c->kmin : nullptr, c->nx, c->ny, c->nz, c->bx, c->by, c->bz, c->bad);
+        khat, merging ? c->kmin : nullptr, c->nx, c->ny, c->nz, c->bx, c->by, c->bz, bad);
   else if (rows)
     rt::pack_optics_rows_kernel<<<c->sm_count * 16, 128, 0, st>>>(
         (const float4*)k_ext, (const float4*)k_ext_cloud, (const float4*)ssa, (const float4*)g, optics,
-        (int*)khat, merging ? (int*)c->kmin : nullptr, c->nx, c->ny, c->nz, c->bx, c->by, c->bz, c->bad);
+        (int*)khat, merging ? (int*)c->kmin : nullptr, c->nx, c->ny, c->nz, c->bx, c->by, c->bz, bad);
   else
     rt::pack_optics_kernel<<<blocks, 256, 0, st>>>(k_ext, k_ext_cloud, ssa, g, optics, (int*)khat,
                                                   merging ? (int*)c->kmin : nullptr, c->nx,
-                                                  c->ny, c->nz, c->bx, c->by, c->bz, c->bad);
-  rt::check_albedo_kernel<<<c->sm_count, 256, 0, st>>>(albedo, c->ncol, c->bad);
+                                                  c->ny, c->nz, c->bx, c->by, c->bz, bad);
+  rt::check_albedo_kernel<<<c->sm_count, 256, 0, st>>>(albedo, c->ncol, bad);
   c->launches += 2;
   if (merging) {
     const size_t nblk = c->ncell / ((size_t)c->mx * c->my * c->mz);
@@ -313,13 +321,14 @@ int set_optics_impl(rt_ctx* c, int slot, const float* k_ext, const float* k_ext_
     ++c->launches;
   }
   RT_CUDA(c, cudaGetLastError());
+  if (int rcm = mark(c, st)) return rcm;
   if (sync) {
-    int bad = 0;
-    RT_CUDA(c, cudaMemcpyAsync(&bad, c->bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+    int hbad = 0;
+    RT_CUDA(c, cudaMemcpyAsync(&hbad, bad, sizeof(int), cudaMemcpyDeviceToHost, st));
     RT_CUDA(c, cudaStreamSynchronize(st));
-    if (bad) {
+    if (hbad) {
       char msg[176];
-      snprintf(msg, sizeof msg, "%s: input out of range (mask 0x%x: 1 k_ext, 2 k_ext_cloud, 4 ssa, 8 g, 16 albedo)", who, bad);
+      snprintf(msg, sizeof msg, "%s: input out of range (mask 0x%x: 1 k_ext, 2 k_ext_cloud, 4 ssa, 8 g, 16 albedo)", who, hbad);
       return fail(c, RT_EOPTICS, msg);
     }
   } else if (staged) {
@@ -345,9 +354,9 @@ int rt_set_slots(rt_ctx* c, int n_slots) {
   if (n_slots < 1 || (unsigned long long)n_slots * c->nvox >= (1ull << 32))
     return fail(c, RT_EINVAL, "rt_set_slots: need 1 <= n_slots and n_slots * nvox < 2^32");
   DeviceGuard guard(c->device);
-  RT_CUDA(c, cudaDeviceSynchronize());
-  cudaFree(c->optics); cudaFree(c->khat); cudaFree(c->albedo); cudaFree(c->batch_tab); cudaFree(c->gas_tab); cudaFree(c->point_par);
-  c->optics = nullptr; c->khat = nullptr; c->albedo = nullptr; c->batch_tab = nullptr; c->gas_tab = nullptr; c->point_par = nullptr;
+  if (int rcw = wait_pending(c)) return rcw;
+  cudaFree(c->optics); cudaFree(c->khat); cudaFree(c->albedo); cudaFree(c->batch_tab); cudaFree(c->gas_tab); cudaFree(c->point_par); cudaFree(c->bad);
+  c->optics = nullptr; c->khat = nullptr; c->albedo = nullptr; c->batch_tab = nullptr; c->gas_tab = nullptr; c->point_par = nullptr; c->bad = nullptr;
   c->have_optics = false;
   c->n_slots = n_slots;
   c->slot_ok.assign((size_t)n_slots, 0);
@@ -356,7 +365,8 @@ int rt_set_slots(rt_ctx* c, int n_slots) {
   RT_CUDA(c, cudaMalloc(&c->khat, (size_t)n_slots * c->ncell * sizeof(float)));
   RT_CUDA(c, cudaMalloc(&c->albedo, (size_t)n_slots * c->ncol * sizeof(float)));
   RT_CUDA(c, cudaMalloc(&c->batch_tab, 2 * (2 * (size_t)n_slots + 1) * sizeof(unsigned long long)));   // two launches may be in flight
-  RT_CUDA(c, cudaMemset(c->bad, 0, sizeof(int)));
+  RT_CUDA(c, cudaMalloc(&c->bad, ((size_t)n_slots + 1) * sizeof(int)));
+  RT_CUDA(c, cudaMemset(c->bad, 0, ((size_t)n_slots + 1) * sizeof(int)));
   return RT_OK;
 }
 
@@ -372,6 +382,7 @@ int rt_set_optics_factored(rt_ctx* c, int slot, const float* k_cloud, const floa
                            float cloud_ssa, float cloud_g, const float* sfc_albedo, void* cuda_stream) {
   if (!c) return RT_EINVAL;
   if (slot < 0 || slot >= c->n_slots) return fail(c, RT_EINVAL, "rt_set_optics_factored: slot out of range (rt_set_slots)");
+  if (!c->batch_tab) return fail(c, RT_ESTATE, "rt_set_optics_factored: call rt_set_slots first");
   if (!k_cloud || !k_abs || !k_ray || !sfc_albedo) return fail(c, RT_EINVAL, "rt_set_optics_factored: NULL argument");
   if (c->nx % 4 || !(c->bx == 1 || c->bx == 2 || c->bx == 4) || c->by * c->bz > 64 || ((uintptr_t)k_cloud & 15u))
     return fail(c, RT_EINVAL, "rt_set_optics_factored: needs nx % 4 == 0, bx in {1, 2, 4}, by * bz <= 64, 16-byte aligned k_cloud");
@@ -399,10 +410,11 @@ int rt_set_optics_factored(rt_ctx* c, int slot, const float* k_cloud, const floa
   RT_CUDA(c, cudaMemcpyAsync(albedo, sfc_albedo, c->ncol * sizeof(float), cudaMemcpyDeviceToDevice, st));
   const bool merging = c->mx * c->my * c->mz > 1;
   if (merging && !c->kmin) RT_CUDA(c, cudaMalloc(&c->kmin, c->ncell * sizeof(float)));
+  RT_CUDA(c, cudaMemsetAsync(c->bad + slot, 0, sizeof(int), st));
   rt::pack_factored_cellrows_kernel<<<c->sm_count * 16, 128, 0, st>>>(
       (const float4*)k_cloud, tab, tab + c->nz, cloud_ssa, cloud_g, optics, khat, merging ? c->kmin : nullptr,
-      c->nx, c->ny, c->nz, c->bx, c->by, c->bz, c->bad);
-  rt::check_albedo_kernel<<<c->sm_count, 256, 0, st>>>(albedo, c->ncol, c->bad);
+      c->nx, c->ny, c->nz, c->bx, c->by, c->bz, c->bad + slot);
+  rt::check_albedo_kernel<<<c->sm_count, 256, 0, st>>>(albedo, c->ncol, c->bad + slot);
   c->launches += 2;
   if (merging) {
     const size_t nblk = c->ncell / ((size_t)c->mx * c->my * c->mz);
@@ -412,7 +424,7 @@ int rt_set_optics_factored(rt_ctx* c, int slot, const float* k_cloud, const floa
   }
   RT_CUDA(c, cudaGetLastError());
   c->slot_ok[slot] = 1;
-  return RT_OK;
+  return mark(c, st);
 }
 
 int rt_set_cloud(rt_ctx* c, const float* k_cloud, void* cuda_stream) {
@@ -425,13 +437,15 @@ int rt_set_cloud(rt_ctx* c, const float* k_cloud, void* cuda_stream) {
   if (!c->cloud_max) RT_CUDA(c, cudaMalloc(&c->cloud_max, c->ncell * c->bz * sizeof(float)));
   if (!c->cloud_min) RT_CUDA(c, cudaMalloc(&c->cloud_min, c->ncell * c->bz * sizeof(float)));
   RT_CUDA(c, cudaMemcpyAsync(c->cloud, k_cloud, c->nvox * sizeof(float), cudaMemcpyDefault, st));
-  RT_CUDA(c, cudaMemsetAsync(c->bad, 0, sizeof(int), st));
+  int* cbad = c->bad + c->n_slots;        // the cloud field's own mask word: the slots' masks are not touched
+  RT_CUDA(c, cudaMemsetAsync(cbad, 0, sizeof(int), st));
   rt::cloud_levels_kernel<<<c->sm_count * 8, 256, 0, st>>>(c->cloud, c->cloud_max, c->cloud_min, c->nx, c->ny, c->nz,
-                                                           c->bx, c->by, c->bz, c->bad);
+                                                           c->bx, c->by, c->bz, cbad);
   ++c->launches;
   RT_CUDA(c, cudaGetLastError());
+  if (int rcm = mark(c, st)) return rcm;
   int bad = 0;
-  RT_CUDA(c, cudaMemcpyAsync(&bad, c->bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+  RT_CUDA(c, cudaMemcpyAsync(&bad, cbad, sizeof(int), cudaMemcpyDeviceToHost, st));
   RT_CUDA(c, cudaStreamSynchronize(st));
   if (bad) return fail(c, RT_EOPTICS, "rt_set_cloud: the cloud extinction must be finite and >= 0");
   c->cloud_ok = true;
@@ -443,12 +457,14 @@ int rt_set_point(rt_ctx* c, int slot, const float* k_abs, const float* k_ray, fl
   if (!c) return RT_EINVAL;
   if (slot < 0 || slot >= c->n_slots) return fail(c, RT_EINVAL, "rt_set_point: slot out of range (rt_set_slots)");
   if (!k_abs || !k_ray || !sfc_albedo) return fail(c, RT_EINVAL, "rt_set_point: NULL argument");
+  if (!c->batch_tab) return fail(c, RT_ESTATE, "rt_set_point: call rt_set_slots first");
   if (!c->cloud_ok) return fail(c, RT_ESTATE, "rt_set_point: call rt_set_cloud first");
   if (!(cloud_ssa >= 0.0f && cloud_ssa <= 1.0f) || !(std::fabs(cloud_g) < 1.0f))
     return fail(c, RT_EOPTICS, "rt_set_point: cloud_ssa must be in [0, 1] and |cloud_g| < 1");
   DeviceGuard guard(c->device);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   c->slot_ok[slot] = 0;
+  if (slot == 0) c->have_optics = false;  // slot 0's majorant and albedo no longer belong to rt_set_optics' packed record
   if (!c->gas_tab) RT_CUDA(c, cudaMalloc(&c->gas_tab, (size_t)c->n_slots * 2 * c->nz * sizeof(float)));
   if (!c->point_par) RT_CUDA(c, cudaMalloc(&c->point_par, (size_t)c->n_slots * sizeof(float2)));
   float* tab = c->gas_tab + (size_t)slot * 2 * c->nz;
@@ -461,9 +477,10 @@ int rt_set_point(rt_ctx* c, int slot, const float* k_abs, const float* k_ray, fl
   RT_CUDA(c, cudaMemcpyAsync(albedo, sfc_albedo, c->ncol * sizeof(float), cudaMemcpyDefault, st));
   const bool merging = c->mx * c->my * c->mz > 1;
   if (merging && !c->kmin) RT_CUDA(c, cudaMalloc(&c->kmin, c->ncell * sizeof(float)));
+  RT_CUDA(c, cudaMemsetAsync(c->bad + slot, 0, sizeof(int), st));
   rt::point_majorant_kernel<<<c->sm_count * 8, 256, 0, st>>>(c->cloud_max, c->cloud_min, tab, tab + c->nz, khat,
-                                                             merging ? c->kmin : nullptr, c->ncx, c->ncy, c->ncz, c->bz, c->bad);
-  rt::check_albedo_kernel<<<c->sm_count, 256, 0, st>>>(albedo, c->ncol, c->bad);
+                                                             merging ? c->kmin : nullptr, c->ncx, c->ncy, c->ncz, c->bz, c->bad + slot);
+  rt::check_albedo_kernel<<<c->sm_count, 256, 0, st>>>(albedo, c->ncol, c->bad + slot);
   c->launches += 2;
   if (merging) {
     const size_t nblk = c->ncell / ((size_t)c->mx * c->my * c->mz);
@@ -473,14 +490,15 @@ int rt_set_point(rt_ctx* c, int slot, const float* k_abs, const float* k_ray, fl
   }
   RT_CUDA(c, cudaGetLastError());
   c->slot_ok[slot] = 2;
-  return RT_OK;
+  return mark(c, st);
 }
 
 int rt_trace_batch(rt_ctx* c, double zenith_deg, double azimuth_deg, int first_point, int n_points,
                    const uint64_t* counts, uint64_t first_photon_id, uint64_t seed, void* cuda_stream,
                    uint32_t* records_out) {
   if (!c) return RT_EINVAL;
-  if (first_point < 0 || n_points < 1 || first_point + n_points > c->n_slots || !counts || !c->batch_tab)
+  if (!c->batch_tab) return fail(c, RT_ESTATE, "rt_trace_batch: call rt_set_slots first");
+  if (first_point < 0 || n_points < 1 || first_point + n_points > c->n_slots || !counts)
     return fail(c, RT_EINVAL, "rt_trace_batch: points must lie within the slots (rt_set_slots), counts not NULL");
   const char kind = c->slot_ok[first_point];
   for (int j = first_point; j < first_point + n_points; ++j)
@@ -490,15 +508,17 @@ int rt_trace_batch(rt_ctx* c, double zenith_deg, double azimuth_deg, int first_p
     if (!c->slot_ok[j]) return fail(c, RT_ESTATE, "rt_trace_batch: a slot below n_points has no optics (rt_set_optics_slot)");
   DeviceGuard guard(c->device);
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  // range errors of the slots' fields, accumulated on the device since rt_set_slots
-  int bad = 0;
-  RT_CUDA(c, cudaMemcpyAsync(&bad, c->bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+  // range errors of the fields of the slots this launch reads (one mask word per slot, cleared when a slot is set again)
+  std::vector<int> bad((size_t)n_points, 0);
+  RT_CUDA(c, cudaMemcpyAsync(bad.data(), c->bad + first_point, (size_t)n_points * sizeof(int), cudaMemcpyDeviceToHost, st));
   RT_CUDA(c, cudaStreamSynchronize(st));
-  if (bad) {
-    char msg[176];
-    snprintf(msg, sizeof msg, "rt_trace_batch: a slot's input is out of range (mask 0x%x: 1 k_ext, 2 k_ext_cloud, 4 ssa, 8 g, 16 albedo)", bad);
-    return fail(c, RT_EOPTICS, msg);
-  }
+  for (int j = 0; j < n_points; ++j)
+    if (bad[(size_t)j]) {
+      char msg[192];
+      snprintf(msg, sizeof msg, "rt_trace_batch: slot %d holds input out of range (mask 0x%x: 1 k_ext, 2 k_ext_cloud, 4 ssa, 8 g, 16 albedo)",
+               first_point + j, bad[(size_t)j]);
+      return fail(c, RT_EOPTICS, msg);
+    }
   std::vector<unsigned long long> tab(2 * (size_t)c->n_slots + 1, 0ull);
   unsigned long long total = 0;
   for (int j = 0; j < n_points; ++j) {
@@ -528,13 +548,6 @@ int rt_trace_range(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t jo
                   0, 0, nullptr, false, range_begin, job_photons);
 }
 
-int rt_set_kernel(rt_ctx* c, int kernel) {
-  if (!c) return RT_EINVAL;
-  if (kernel != RT_KERNEL_POOL && kernel != RT_KERNEL_LANES) return fail(c, RT_EINVAL, "rt_set_kernel: unknown kernel");
-  c->kernel = kernel;
-  return RT_OK;
-}
-
 int rt_trace_records(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photons,
                      uint64_t first_photon_id, uint64_t seed, uint32_t stream_id, void* cuda_stream,
                      uint32_t* records_out) {
@@ -546,14 +559,15 @@ int rt_read_tallies(rt_ctx* c, int64_t* atm_abs, int64_t* sfc_dir, int64_t* sfc_
                     int64_t* toa_up, rt_counters* counters) {
   if (!c) return RT_EINVAL;
   DeviceGuard guard(c->device);
-  RT_CUDA(c, cudaDeviceSynchronize());
+  if (int rcw = wait_pending(c)) return rcw;   // this context's work only, not the whole device
   int64_t* outs[5] = {atm_abs, sfc_dir, sfc_dif, sfc_abs, toa_up};
   for (int k = 0; k < 5; ++k)
     if (outs[k])
-      RT_CUDA(c, cudaMemcpy(outs[k], tally_ptr(c, k), (k == 0 ? c->nvox : c->ncol) * sizeof(int64_t), cudaMemcpyDefault));
+      RT_CUDA(c, cudaMemcpyAsync(outs[k], tally_ptr(c, k), (k == 0 ? c->nvox : c->ncol) * sizeof(int64_t), cudaMemcpyDefault, c->copy_stream));
+  unsigned long long h[rt::C_COUNT];
+  if (counters) RT_CUDA(c, cudaMemcpyAsync(h, c->counters, sizeof h, cudaMemcpyDeviceToHost, c->copy_stream));
+  RT_CUDA(c, cudaStreamSynchronize(c->copy_stream));
   if (counters) {
-    unsigned long long h[rt::C_COUNT];
-    RT_CUDA(c, cudaMemcpy(h, c->counters, sizeof h, cudaMemcpyDeviceToHost));
     counters->n_null = h[rt::C_NULL]; counters->n_rayleigh = h[rt::C_RAY]; counters->n_hg = h[rt::C_HG];
     counters->n_atm_abs = h[rt::C_ATM_ABS]; counters->n_sfc_hits = h[rt::C_SFC_HITS];
     counters->n_sfc_abs = h[rt::C_SFC_ABS]; counters->n_toa = h[rt::C_TOA]; counters->n_capped = h[rt::C_CAPPED];
@@ -603,7 +617,7 @@ int rt_read_tallies_async(rt_ctx* c, int64_t* atm_abs, int64_t* sfc_dir, int64_t
     RT_CUDA(c, cudaMemcpyAsync(counters, c->d_counters, sizeof(rt_counters), cudaMemcpyDefault, st));
   }
   RT_CUDA(c, cudaGetLastError());
-  return RT_OK;
+  return mark(c, st);
 }
 
 int rt_set_merge(rt_ctx* c, int mx, int my, int mz, float merge_ratio) {
@@ -613,7 +627,8 @@ int rt_set_merge(rt_ctx* c, int mx, int my, int mz, float merge_ratio) {
     return fail(c, RT_EINVAL, "rt_set_merge: factors must be powers of two <= 64 dividing the acceleration grid");
   if (!(merge_ratio >= 1.0f) || !std::isfinite(merge_ratio)) return fail(c, RT_EINVAL, "rt_set_merge: merge_ratio must be >= 1");
   c->mx = mx; c->my = my; c->mz = mz; c->merge_ratio = merge_ratio;
-  c->have_optics = false;                 // the majorant table is rebuilt by the next rt_set_optics
+  c->have_optics = false;                 // every majorant table was built for the old factors: all slots
+  for (auto& ok : c->slot_ok) ok = 0;     // must be given optics again (RT_ESTATE otherwise)
   return RT_OK;
 }
 
@@ -640,8 +655,9 @@ int rt_read_heating_direct(rt_ctx* c, int64_t* out) {
   if (!c || !out) return RT_EINVAL;
   if (!c->atm_dir) return fail(c, RT_ESTATE, "rt_read_heating_direct: call rt_set_heating_split(ctx, 1) first");
   DeviceGuard guard(c->device);
-  RT_CUDA(c, cudaDeviceSynchronize());
-  RT_CUDA(c, cudaMemcpy(out, c->atm_dir, c->nvox * sizeof(int64_t), cudaMemcpyDefault));
+  if (int rcw = wait_pending(c)) return rcw;
+  RT_CUDA(c, cudaMemcpyAsync(out, c->atm_dir, c->nvox * sizeof(int64_t), cudaMemcpyDefault, c->copy_stream));
+  RT_CUDA(c, cudaStreamSynchronize(c->copy_stream));
   return RT_OK;
 }
 
@@ -668,22 +684,24 @@ int rt_reset_tallies(rt_ctx* c, void* cuda_stream) {
   RT_CUDA(c, cudaMemsetAsync(c->tallies, 0, (c->nvox + 4 * c->ncol) * sizeof(unsigned long long), st));
   RT_CUDA(c, cudaMemsetAsync(c->counters, 0, (rt::C_COUNT + 1) * sizeof(unsigned long long), st));
   if (c->atm_dir) RT_CUDA(c, cudaMemsetAsync(c->atm_dir, 0, c->nvox * sizeof(unsigned long long), st));
-  return RT_OK;
+  return mark(c, st);
 }
 
 int rt_read_majorant(rt_ctx* c, float* khat_out) {
   if (!c || !khat_out) return RT_EINVAL;
   DeviceGuard guard(c->device);
-  RT_CUDA(c, cudaDeviceSynchronize());
-  RT_CUDA(c, cudaMemcpy(khat_out, c->khat, c->ncell * sizeof(float), cudaMemcpyDefault));
+  if (int rcw = wait_pending(c)) return rcw;
+  RT_CUDA(c, cudaMemcpyAsync(khat_out, c->khat, c->ncell * sizeof(float), cudaMemcpyDefault, c->copy_stream));
+  RT_CUDA(c, cudaStreamSynchronize(c->copy_stream));
   return RT_OK;
 }
 
 int rt_read_packed_optics(rt_ctx* c, float* packed_out) {
   if (!c || !packed_out) return RT_EINVAL;
   DeviceGuard guard(c->device);
-  RT_CUDA(c, cudaDeviceSynchronize());
-  RT_CUDA(c, cudaMemcpy(packed_out, c->optics, c->nvox * sizeof(float4), cudaMemcpyDefault));
+  if (int rcw = wait_pending(c)) return rcw;
+  RT_CUDA(c, cudaMemcpyAsync(packed_out, c->optics, c->nvox * sizeof(float4), cudaMemcpyDefault, c->copy_stream));
+  RT_CUDA(c, cudaStreamSynchronize(c->copy_stream));
   return RT_OK;
 }
 
@@ -744,6 +762,8 @@ void rt_destroy(rt_ctx* c) {
     cudaFree(c->cloud); cudaFree(c->cloud_max); cudaFree(c->cloud_min); cudaFree(c->batch_tab); cudaFree(c->sink); cudaFree(c->stage);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
+    for (auto& p : c->pending) cudaEventDestroy(p.second);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
   }
   delete c;
 }

@@ -29,33 +29,13 @@ constexpr uint32_t kEventCap = 1u << 20;        // §3.12
 constexpr float kTiny = 1e-30f;                 // direction components are nudged away from 0
 constexpr int kTraceThreads = 256;
 constexpr int kChunk = 128;                     // photon ids a warp takes per global atomic (fewer in small launches)
-#ifndef RT_MIN_BLOCKS
-#define RT_MIN_BLOCKS 4
-#endif
-#ifndef RT_REGEN_BATCH
-#define RT_REGEN_BATCH 6
-#endif
-#ifndef RT_SCATTER_BATCH
-#define RT_SCATTER_BATCH 8
-#endif
-#ifndef RT_COLLIDE_BATCH
-#define RT_COLLIDE_BATCH 8
-#endif
-#ifndef RT_MOVE_STEPS
-#define RT_MOVE_STEPS 3
-#endif
-#ifndef RT_MOVE_MIN
-#define RT_MOVE_MIN 0
-#endif
-#ifndef RT_BOUNDARY_BATCH
-#define RT_BOUNDARY_BATCH 4
-#endif
-constexpr int kRegenBatch = RT_REGEN_BATCH;       // refill when this many lanes are idle (or nothing else to do)
-constexpr int kScatterBatch = RT_SCATTER_BATCH;   // run SCATTER when this many lanes wait for it (or nothing moves)
-constexpr int kCollideBatch = RT_COLLIDE_BATCH;   // ... COLLIDE
-constexpr int kBoundaryBatch = RT_BOUNDARY_BATCH; // ... BOUNDARY
-constexpr int kMoveSteps = RT_MOVE_STEPS;         // MOVE steps between two votes (at most)
-constexpr int kMoveMin = RT_MOVE_MIN;             // ... cut short when fewer lanes than this still move (0: never)
+// Vote thresholds (profiles/r1_block_sweep.md, profiles/r2_pool_kernel.md: sweeps of each around these values)
+constexpr int kMinBlocks = 4;          // resident blocks per SM the launch bounds ask for (64 registers)
+constexpr int kRegenBatch = 6;         // refill when this many lanes are idle (or nothing else to do)
+constexpr int kScatterBatch = 8;       // run SCATTER when this many lanes wait for it (or nothing moves)
+constexpr int kCollideBatch = 8;       // ... COLLIDE
+constexpr int kBoundaryBatch = 4;      // ... BOUNDARY
+constexpr int kMoveSteps = 3;          // MOVE steps between two votes
 
 enum Counter { C_NULL = 0, C_RAY, C_HG, C_ATM_ABS, C_SFC_HITS, C_SFC_ABS, C_TOA, C_CAPPED, C_CELLS,
                C_CAPPED_E, C_RELEVEL, C_ROUL_KILLED, C_ROUL_KEPT, C_ROUL_LOST, C_ROUL_GAINED, C_COUNT };
@@ -121,7 +101,7 @@ __device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
 // absorption: integer weight wq (tally quanta), deposits at every tentative collision, roulette ledger.
 // kBatch: several spectral points in one launch, each with its own optics and majorant slot (see TraceArgs).
 template <bool kRecords, bool kPow2, bool kWeighted, bool kBatch = false>
-__global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(const TraceArgs A) {
+__global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const TraceArgs A) {
   __shared__ unsigned long long s_cnt[C_COUNT];
   if (threadIdx.x < C_COUNT) s_cnt[threadIdx.x] = 0ull;
   __syncthreads();
@@ -348,7 +328,6 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
       const int sx = (int)(stp << 24) >> 24, sy = (int)(stp << 16) >> 24, sz = (int)(stp << 8) >> 24;
 #pragma unroll
       for (int rep = 0; rep < kMoveSteps; ++rep) {
-      if (kMoveMin > 0 && rep > 0 && __popc(__ballot_sync(0xffffffffu, st == ST_MOVE)) < kMoveMin) break;
       if (st == ST_MOVE) {
         const bool ax0 = (rx <= ry) && (rx <= rz);
         const bool ax1 = !ax0 && (ry <= rz);
@@ -403,12 +382,12 @@ __global__ void __launch_bounds__(kTraceThreads, RT_MIN_BLOCKS) trace_kernel(con
         const bool lev = __float_as_int(kh) < 0;
         const float qx = local(da, rx, lev ? A.Lx1 : A.Lx), qy = local(db, ry, lev ? A.Ly1 : A.Ly),
                     qz = local(dc, rz, lev ? A.Lz1 : A.Lz);
-        float mu;
-        if (sg < 1.5f) { mu = sample_hg(sg, u24(sw2)); ++t_hg; }
-        else           { mu = sample_rayleigh(u24(sw2)); }
+        float mu, sn;
+        if (sg < 1.5f) { sample_hg(sg, u24(sw2), mu, sn); ++t_hg; }
+        else           { sample_rayleigh(u24(sw2), mu, sn); }
         float sp, cp;
         sincos_2pi(u24(sw3), sp, cp);
-        rotate_dir(da, db, dc, mu, cp, sp);
+        rotate_dir(da, db, dc, mu, sn, cp, sp);
         place(qx, qy, qz);
         direct = false; ++t_sc;
         st = ST_MOVE;

@@ -19,6 +19,13 @@ def photon_range(rank: int, world: int, n_total: int, first_photon_id: int = 0):
     return first, count
 
 
+def job_range(rank: int, world: int, job_photons: int):
+    """(range_begin, range_count) of `rank` for include/rt.h rt_trace_range: the job's photon INDICES split over
+    the ranks.  Every rank passes the same job_photons and first_photon_id, so columns, passes and ids are the
+    job's, and the all-reduced integer tallies equal the one-GPU call bit for bit."""
+    return photon_range(rank, world, job_photons, 0)
+
+
 def weak_range(rank: int, world: int, step: int, n_per_gpu: int):
     """Id range of `rank` at `step` when every GPU traces n_per_gpu new photons per step (weak scaling)."""
     return (step * world + rank) * n_per_gpu, n_per_gpu

@@ -73,15 +73,15 @@ def _worker(rank, world, port, n_total, out):
     sys.path.insert(0, ROOT)
     os.environ["MASTER_ADDR"], os.environ["MASTER_PORT"] = "127.0.0.1", str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
-    import oracle as O          # stands in for the per-GPU trace: tests may call the oracle
-    from paper_2208_05247_b200.shard import photon_range, allreduce_tallies
+    import oracle as O          # stands in for the per-GPU rt_trace_range: tests may call the oracle
+    from paper_2208_05247_b200.shard import job_range, allreduce_tallies
     from rt_inputs import CONFIGS, make_optics
     cfg = CONFIGS[1]
     opt = make_optics(cfg)
-    first, count = photon_range(rank, world, n_total)
-    # every rank keeps the column stratification of the whole job: ids map to columns by id mod ncol
-    t, _, _ = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, count, first_photon_id=first, seed=3,
-                      precision=32)
+    begin, count = job_range(rank, world, n_total)
+    # the shard keeps the JOB's column stratification and ids (include/rt.h rt_trace_range; oracle index_range)
+    t, _, _ = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n_total, seed=3, precision=32,
+                      index_range=(begin, count))
     ts = [torch.from_numpy(getattr(t, k)) for k in ("atm_abs", "sfc_dir", "sfc_dif", "sfc_abs", "toa_up")]
     allreduce_tallies(ts)
     if rank == 0:
@@ -89,16 +89,41 @@ def _worker(rank, world, port, n_total, out):
     dist.destroy_process_group()
 
 
-def test_two_rank_sharding_closes_energy_exactly(tmp_path):
-    """Two gloo ranks trace disjoint id ranges and all-reduce: the merged int64 tallies close energy
-    exactly and every photon of the job is accounted for once."""
+def test_two_rank_sharding_equals_the_single_call(tmp_path):
+    """Two gloo ranks trace the two halves of ONE job (job-indexed ranges) and all-reduce: the merged int64
+    tallies equal the single-call tallies bit for bit (so a multi-GPU run reproduces the one-GPU sample) and
+    close energy exactly."""
     import oracle as O
-    n_total = 2 * 1024 * 3 + 1           # odd: the ranks get different counts
+    from rt_inputs import CONFIGS, make_optics
+    n_total = 2 * 1024 * 3 + 1           # odd: the ranks get different counts; a remainder pass exists
     out = str(tmp_path / "merged.npz")
     mp.spawn(_worker, args=(2, _free_port(), n_total, out), nprocs=2, join=True)
     m = np.load(out)
     assert int(m["atm_abs"].sum()) + int(m["sfc_abs"].sum()) + int(m["toa_up"].sum()) == n_total * O.W0
-    assert int(m["sfc_dir"].sum()) % O.W0 == 0 and int(m["sfc_dir"].sum()) > 0
+    cfg = CONFIGS[1]
+    one, _, _ = O.trace(cfg.grid, make_optics(cfg), cfg.zenith_deg, cfg.azimuth_deg, n_total, seed=3, precision=32)
+    for k in ("atm_abs", "sfc_dir", "sfc_dif", "sfc_abs", "toa_up"):
+        assert (m[k] == getattr(one, k)).all(), k
+
+
+def test_oracle_index_ranges_tile_the_job():
+    """The oracle's index_range (the shard definition both sides implement): three ragged ranges of a job with a
+    remainder pass and Sobol entry points add up to the single call, record by record."""
+    import oracle as O
+    from rt_inputs import CONFIGS, make_optics
+    cfg = CONFIGS[1]
+    opt = make_optics(cfg)
+    n = 3 * cfg.ncol + 333
+    kw = dict(seed=9, precision=32, records=True, sobol=True, first_photon_id=(1 << 33) + 5)
+    one, rec1, _ = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, **kw)
+    acc, rec = None, np.zeros_like(rec1)
+    for b, cnt in ((0, 700), (700, 2 * cfg.ncol), (700 + 2 * cfg.ncol, n - 700 - 2 * cfg.ncol)):
+        acc, r, _ = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, tallies=acc, index_range=(b, cnt), **kw)
+        rec[b:b + cnt] = r[b:b + cnt]
+    assert (rec == rec1).all()
+    for k in ("atm_abs", "sfc_dir", "sfc_dif", "sfc_abs", "toa_up"):
+        assert (getattr(acc, k) == getattr(one, k)).all()
+    assert acc.counters.asdict() == one.counters.asdict()
 
 
 def test_tally_to_flux_host_helper():

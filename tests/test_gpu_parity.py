@@ -127,10 +127,9 @@ def test_config2_sample():
     cfg = CONFIGS[2]
     opt = make_optics(cfg)
     n = 1 << 20  # 64 full passes over the columns; the oracle finishes in seconds
-    # ~200 tentative collisions per photon: fp32 position rounding (2^-24 of a 400 m cell per
-    # operation, accumulating as a random walk) flips a voxel decision in ~1 % of photons relative
-    # to fp64 geometry; identity proper is the 100 % match in kernel precision above.
-    t, o64, same = _compare(cfg, opt, n, min_same64=0.98)
+    # ~70 tentative collisions per photon: fp32 rounding, amplified where DESIGN.md §7 says, takes ~0.4 % of the
+    # photons off the fp64 path; identity proper is the 100 % match in kernel precision above.
+    t, o64, same = _compare(cfg, opt, n, min_same64=0.994)
     rms, nb = _block_rms(t.sfc_dir.numpy() + t.sfc_dif.numpy(), o64.sfc_dir + o64.sfc_dif, (16, 16))
     assert nb > 0 and rms < 0.02, (rms, nb)
 

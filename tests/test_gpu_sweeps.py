@@ -143,6 +143,11 @@ def test_config5_convergence_sweep():
         c = [r[key] / np.sqrt(1.0 / r["photons_per_column"] + 1.0 / ref["photons_per_column"]) for r in rows]
         assert max(c) / min(c) < 1.15, (key, c)
         assert rows[0][key] > 4 * rows[3][key]        # 64x the photons: ~ sqrt((1+1/256)/(1/64+1/256)) = 7.2
+    # P:78 "the run time scales linearly with the number of samples": the same photons per second at 16, 64 and 256
+    # photons per column (the 1- and 4-per-column launches last 2-8 ms, where the drain of the persistent kernel shows)
+    pps = [r["paths_per_s"] for r in rows if r["photons_per_column"] >= 16]
+    assert max(pps) / min(pps) < 1.15, pps
+    assert rows[1]["paths_per_s"] > 0.6 * max(pps)
 
 
 def test_batched_points_equal_separate_traces():
