@@ -531,6 +531,8 @@ def run_ours(args):
         "dtype": "f32", "data": "synthetic",
         "collision_events_per_s": total_events / (elapsed_ms * 1e-3),
         "events_per_photon": total_events / total_photons,
+        "per_photon": {k: per[k] / n for k in ("n_events", "n_null", "n_hg", "n_rayleigh", "n_cell_steps", "n_relevel",
+                                               "n_sfc_hits")},
         "trace_kernel": {"ms": ms_avg, "paths_per_s": n / (ms_avg * 1e-3), "events_per_s": trace_events_per_s},
         "config": {"workload": cfg.name, "grid": [cfg.nx, cfg.ny, cfg.nz], "photons_per_gpu_per_step": n,
                    "block": list(cfg.block), "merge": list(cfg.merge), "merge_ratio": cfg.merge_ratio,

@@ -382,6 +382,7 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
     auto set_dir = [&]() {
       for (int a = 0; a < 3; ++a) {
         v[a] = (std::fabs(d[a]) < TINY) ? TINY : d[a];
+        d[a] = v[a];                             // Q20 (round 2): the nudged component IS the direction from here on
         iv[a] = (R)1 / v[a];
         del[0][a] = Lv[0][a] * std::fabs(iv[a]);
         del[1][a] = Lv[1][a] * std::fabs(iv[a]);

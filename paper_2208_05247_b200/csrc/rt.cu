@@ -158,16 +158,19 @@ int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photon
   A.rdx = 1.0f / c->dx; A.rdy = 1.0f / c->dy; A.rdz = 1.0f / c->dz;
   A.Lx = (float)c->bx * c->dx; A.Ly = (float)c->by * c->dy; A.Lz = (float)c->bz * c->dz;
   A.mx = c->mx; A.my = c->my; A.mz = c->mz;
+  A.unit = (c->bx == 1 && c->by == 1 && c->bz == 1) ? 1 : 0;
+  A.vote_bias = rt::vote_bias(A.unit ? rt::kCollideBatchUnit : rt::kCollideBatch);
+  A.move_steps = A.unit ? rt::kMoveStepsUnit : rt::kMoveSteps;
   A.rmx = 1.0f / (float)c->mx; A.rmy = 1.0f / (float)c->my; A.rmz = 1.0f / (float)c->mz;
   A.Lx1 = (float)(c->mx * c->bx) * c->dx; A.Ly1 = (float)(c->my * c->by) * c->dy; A.Lz1 = (float)(c->mz * c->bz) * c->dz;
   // sun direction evaluated in double on the host, rounded once to fp32
   const double deg = 3.14159265358979323846 / 180.0;
   const double th = zenith_deg * deg, ph = azimuth_deg * deg;
-  A.sun_x = (float)(-std::sin(th) * std::sin(ph));
-  A.sun_y = (float)(-std::sin(th) * std::cos(ph));
-  A.sun_z = (float)(-std::cos(th));
-  auto inv = [](float d) { return 1.0f / (std::fabs(d) < rt::kTiny ? rt::kTiny : d); };  // IEEE fp32, as set_inverse
-  A.sun_ix = inv(A.sun_x); A.sun_iy = inv(A.sun_y); A.sun_iz = inv(A.sun_z);
+  auto nudged = [](double d) { const float f = (float)d; return std::fabs(f) < rt::kTiny ? rt::kTiny : f; };   // Q20
+  A.sun_x = nudged(-std::sin(th) * std::sin(ph));
+  A.sun_y = nudged(-std::sin(th) * std::cos(ph));
+  A.sun_z = nudged(-std::cos(th));
+  A.sun_ix = 1.0f / A.sun_x; A.sun_iy = 1.0f / A.sun_y; A.sun_iz = 1.0f / A.sun_z;   // IEEE fp32, as place()
   A.optics = c->optics; A.khat = c->khat; A.albedo = c->albedo;
   A.atm_dir = c->split ? c->atm_dir : nullptr;
   A.atm_abs = tally_ptr(c, 0); A.sfc_dir = tally_ptr(c, 1); A.sfc_dif = tally_ptr(c, 2);
@@ -195,9 +198,16 @@ int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photon
   A.n_points = n_points; A.first_point = first_point; A.offsets = tab; A.nfull = tab ? tab + c->n_slots + 1 : nullptr;
   A.nvox32 = (unsigned)c->nvox; A.ncell32 = (unsigned)c->ncell; A.ncol32 = (unsigned)c->ncol;
   A.cloud = factored_trace ? c->cloud : nullptr; A.gas = c->gas_tab; A.point_par = c->point_par;
-  RT_CUDA(c, cudaMemsetAsync(A.next_photon, 0, sizeof(unsigned long long), st));
   RT_CUDA(c, cudaEventRecord(c->ev0, st));
-  if (n_photons > 0) {
+  // one launch per 2^31 photons at most (the kernel counts a block's finished photons in 32-bit words); the parts
+  // are consecutive index ranges of the same job, so photons and tallies do not depend on the split
+  const unsigned long long kMaxLaunch = 1ull << 31;
+  for (unsigned long long off = 0; off < n_photons; off += kMaxLaunch) {
+    if (n_points > 0 && n_photons > kMaxLaunch) return fail(c, RT_EINVAL, "rt_trace_batch: at most 2^31 photons per launch");
+    A.n_photons = n_photons - off < kMaxLaunch ? n_photons - off : kMaxLaunch;
+    A.index_base = index_base + off;
+    A.records = records ? records + 4ull * off : nullptr;
+    RT_CUDA(c, cudaMemsetAsync(A.next_photon, 0, sizeof(unsigned long long), st));
     void* kargs[1] = {(void*)&A};
     RT_CUDA(c, cudaLaunchKernel(fn, dim3((unsigned)blocks), dim3((unsigned)rt::kTraceThreads), kargs, 0, st));
     ++c->launches;

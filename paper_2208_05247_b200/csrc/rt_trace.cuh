@@ -29,13 +29,20 @@ constexpr uint32_t kEventCap = 1u << 20;        // §3.12
 constexpr float kTiny = 1e-30f;                 // direction components are nudged away from 0
 constexpr int kTraceThreads = 256;
 constexpr int kChunk = 128;                     // photon ids a warp takes per global atomic (fewer in small launches)
-// Vote thresholds (profiles/r1_block_sweep.md, profiles/r2_pool_kernel.md: sweeps of each around these values)
+// Vote thresholds: a parked phase runs when this many lanes wait for it (or nothing can move).  COLLIDE's threshold and
+// the MOVE steps between two votes depend on the acceleration grid (TraceArgs::vote_bias, move_steps, set by rt.cu):
+// with voxel-sized cells a photon crosses ~5 cells per collision instead of ~1.5, so batches take longer to fill
+// (sweeps: profiles/r1_block_sweep.md, r2_pool_kernel.md, r2_trace_kernel.md).
 constexpr int kMinBlocks = 4;          // resident blocks per SM the launch bounds ask for (64 registers)
 constexpr int kRegenBatch = 6;         // refill when this many lanes are idle (or nothing else to do)
-constexpr int kScatterBatch = 8;       // run SCATTER when this many lanes wait for it (or nothing moves)
-constexpr int kCollideBatch = 8;       // ... COLLIDE
-constexpr int kBoundaryBatch = 4;      // ... BOUNDARY
-constexpr int kMoveSteps = 3;          // MOVE steps between two votes
+constexpr int kScatterBatch = 8;       // SCATTER
+constexpr int kCollideBatch = 8, kCollideBatchUnit = 12;   // COLLIDE: cells of several voxels / voxel-sized cells
+constexpr int kBoundaryBatch = 4;      // BOUNDARY
+constexpr int kMoveSteps = 3, kMoveStepsUnit = 4;           // MOVE steps between two votes
+constexpr unsigned vote_bias(int collide_batch) {
+  return (32u - kRegenBatch) | ((32u - 1u) << 6) | ((32u - (unsigned)collide_batch) << 12) |
+         ((32u - kScatterBatch) << 18) | ((32u - kBoundaryBatch) << 24);
+}
 
 enum Counter { C_NULL = 0, C_RAY, C_HG, C_ATM_ABS, C_SFC_HITS, C_SFC_ABS, C_TOA, C_CAPPED, C_CELLS,
                C_CAPPED_E, C_RELEVEL, C_ROUL_KILLED, C_ROUL_KEPT, C_ROUL_LOST, C_ROUL_GAINED, C_COUNT };
@@ -48,6 +55,10 @@ struct TraceArgs {
   // §3.5b merged cells: factors (powers of two), their reciprocals, merged-cell extents (m b) d
   int mx, my, mz;
   float rmx, rmy, rmz, Lx1, Ly1, Lz1;
+  unsigned vote_bias;                  // thresholds of the vote (vote_bias() above)
+  int move_steps;                      // MOVE steps between two votes: kMoveSteps or kMoveStepsUnit
+  int unit;                            // bx = by = bz = 1: a level-0 acceleration cell IS a voxel (no position needed to
+                                       // find the collision's voxel, and no null collisions outside merged cells)
   float sun_x, sun_y, sun_z, sun_ix, sun_iy, sun_iz;  // beam direction and 1/nudge(component), host-computed
   const float4* __restrict__ optics;   // [z][y][x] (c1, c2, c3, g)
   const float* __restrict__ khat;      // [cz][cy][cx]
@@ -103,7 +114,11 @@ __device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
 template <bool kRecords, bool kPow2, bool kWeighted, bool kBatch = false>
 __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const TraceArgs A) {
   __shared__ unsigned long long s_cnt[C_COUNT];
+  // finished photons of this block per fate (1..5): 32-bit words, because a 64-bit shared-memory atomic is a
+  // compare-and-swap loop; a launch holds fewer than 2^32 photons (rt.cu splits longer calls)
+  __shared__ unsigned s_fate[8];
   if (threadIdx.x < C_COUNT) s_cnt[threadIdx.x] = 0ull;
+  if (threadIdx.x < 8) s_fate[threadIdx.x] = 0u;
   __syncthreads();
 
   const unsigned lane = threadIdx.x & 31u;
@@ -134,6 +149,10 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
   uint32_t t_ev = 0, t_sc = 0, t_hg = 0, t_sfc = 0, t_cells = 0, t_relevel = 0;
   unsigned long long wq = kW0;            // weighted mode: the photon's weight in tally quanta
   unsigned long long t_rlost = 0, t_rgain = 0;   // roulette ledger of this thread
+  // weighted mode: deposits of consecutive tentative collisions in the SAME voxel are summed here and reach the
+  // tally as one atomic when the voxel changes or the photon ends (integer sums: the tally is the same)
+  unsigned long long pend_a = 0;
+  uint32_t pend_vox = 0xffffffffu;
   uint32_t t_rkept = 0;
   uint32_t b_ev = 0, b_sc = 0, b_sfc = 0;  // totals when the current photon was launched (records only)
 
@@ -144,20 +163,20 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
     tau = neg_log(1.0f - u24(X.x)); u1 = u24(X.y); w2 = X.z; w3 = X.w;
   };
   // local coordinate from a remaining distance: q = face - v r, face = L if v > 0 else 0
-  auto local = [&](float d, float r, float L) {
-    const float v = nudge(d);
+  auto local = [&](float v, float r, float L) {   // v: a direction component as set by place(), i.e. nudged (Q20)
     return fminf(L, fmaxf(0.0f, fmaf(-v, r, v > 0.0f ? L : 0.0f)));
   };
   // after a change of direction at local position (qx, qy, qz): reciprocals, face spacings, distances
   auto set_steps = [&](bool lev) {
-    const int ax_ = (da > -kTiny) ? 1 : -1, ay_ = (db > -kTiny) ? 1 : -1, az_ = (dc > -kTiny) ? 1 : -1;
+    const int ax_ = (da > 0.0f) ? 1 : -1, ay_ = (db > 0.0f) ? 1 : -1, az_ = (dc > 0.0f) ? 1 : -1;
     const int sx = lev ? ax_ * A.mx : ax_, sy = lev ? ay_ * A.my : ay_, sz = lev ? az_ * A.mz : az_;
     stp = ((uint32_t)sx & 0xffu) | (((uint32_t)sy & 0xffu) << 8) | (((uint32_t)sz & 0xffu) << 16);
   };
   auto place = [&](float qx, float qy, float qz) {
     const bool lev = __float_as_int(kh) < 0;
+    da = nudge(da); db = nudge(db); dc = nudge(dc);   // Q20: the nudged components are the direction from here on
     set_steps(lev);
-    const float va = nudge(da), vb = nudge(db), vc = nudge(dc);
+    const float va = da, vb = db, vc = dc;
     const float ia = 1.0f / va, ib = 1.0f / vb, ic = 1.0f / vc;
     const float Lx = lev ? A.Lx1 : A.Lx, Ly = lev ? A.Ly1 : A.Ly, Lz = lev ? A.Lz1 : A.Lz;
     delx = Lx * fabsf(ia); dely = Ly * fabsf(ib); delz = Lz * fabsf(ic);
@@ -198,16 +217,31 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
     v = warp_sum(t_ev - t_sc);  if (lane == 0 && v) atomicAdd(&s_cnt[C_NULL], v);
   };
 
+  // ---- SCATTER: phase-function angle, rotation, new distances to the faces (§3.9) ----------------------
+  auto scatter_phase = [&]() {
+    if (st == ST_SCATTER) {
+      const bool lev = __float_as_int(kh) < 0;
+      const float qx = local(da, rx, lev ? A.Lx1 : A.Lx), qy = local(db, ry, lev ? A.Ly1 : A.Ly),
+                  qz = local(dc, rz, lev ? A.Lz1 : A.Lz);
+      float mu, sn;
+      if (sg < 1.5f) { sample_hg(sg, u24(sw2), mu, sn); ++t_hg; }
+      else           { sample_rayleigh(u24(sw2), mu, sn); }
+      float sp, cp;
+      sincos_2pi(u24(sw3), sp, cp);
+      rotate_dir(da, db, dc, mu, sn, cp, sp);
+      place(qx, qy, qz);
+      direct = false; ++t_sc;
+      st = ST_MOVE;
+    }
+  };
 
   for (;;) {
     // the vote: one warp-wide integer add counts the lanes in each of the five states (6 bits each)
     const unsigned votes = __reduce_add_sync(0xffffffffu, 1u << (6u * st));
     // count >= threshold for all five states at once: adding 32 - threshold to a 6-bit field sets its top bit
     // exactly when the count (<= 32) has reached the threshold, and never carries into the next field
-    constexpr unsigned kBias = (32u - kRegenBatch) | ((32u - 1u) << 6) | ((32u - kCollideBatch) << 12) |
-                               ((32u - kScatterBatch) << 18) | ((32u - kBoundaryBatch) << 24);
     constexpr unsigned bD = 32u, bM = 32u << 6, bC = 32u << 12, bS = 32u << 18, bB = 32u << 24;
-    const unsigned full = (votes + kBias) & (bD | bM | bC | bS | bB);
+    const unsigned full = (votes + A.vote_bias) & (bD | bM | bC | bS | bB);
 
     if (!exhausted && (full & bD)) {
       // ---- regeneration: hand photon ids to the idle lanes -------------------------------------
@@ -327,7 +361,8 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
       // index step per axis: +-1 cell, or +-m cells inside a merged cell
       const int sx = (int)(stp << 24) >> 24, sy = (int)(stp << 16) >> 24, sz = (int)(stp << 8) >> 24;
 #pragma unroll
-      for (int rep = 0; rep < kMoveSteps; ++rep) {
+      for (int rep = 0; rep < kMoveStepsUnit; ++rep) {
+      if (rep >= A.move_steps) break;              // warp-uniform
       if (st == ST_MOVE) {
         const bool ax0 = (rx <= ry) && (rx <= rz);
         const bool ax1 = !ax0 && (ry <= rz);
@@ -376,24 +411,7 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
       phase = (full & bC) ? ST_COLLIDE : ((full & bS) ? ST_SCATTER : ST_BOUNDARY);
     }
 
-    if (phase == ST_SCATTER) {
-      // ---- SCATTER: phase-function angle, rotation, new distances to the faces (§3.9) --------------
-      if (st == ST_SCATTER) {
-        const bool lev = __float_as_int(kh) < 0;
-        const float qx = local(da, rx, lev ? A.Lx1 : A.Lx), qy = local(db, ry, lev ? A.Ly1 : A.Ly),
-                    qz = local(dc, rz, lev ? A.Lz1 : A.Lz);
-        float mu, sn;
-        if (sg < 1.5f) { sample_hg(sg, u24(sw2), mu, sn); ++t_hg; }
-        else           { sample_rayleigh(u24(sw2), mu, sn); }
-        float sp, cp;
-        sincos_2pi(u24(sw3), sp, cp);
-        rotate_dir(da, db, dc, mu, sn, cp, sp);
-        place(qx, qy, qz);
-        direct = false; ++t_sc;
-        st = ST_MOVE;
-      }
-      continue;
-    }
+    if (phase == ST_SCATTER) { scatter_phase(); continue; }
 
     fate = 0;
     term = 0;
@@ -406,18 +424,25 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
         const float rk = 1.0f / fabsf(kh);
         const float s = tau * rk;
         rx = fmaxf(0.0f, rx - s); ry = fmaxf(0.0f, ry - s); rz = fmaxf(0.0f, rz - s);
-        const float qx = local(da, rx, lev ? A.Lx1 : A.Lx), qy = local(db, ry, lev ? A.Ly1 : A.Ly),
-                    qz = local(dc, rz, lev ? A.Lz1 : A.Lz);
-        const int lx = min((int)(qx * A.rdx), (lev ? A.mx * A.bx : A.bx) - 1);
-        const int ly = min((int)(qy * A.rdy), (lev ? A.my * A.by : A.by) - 1);
-        const int lz = min((int)(qz * A.rdz), (lev ? A.mz * A.bz : A.bz) - 1);
         // 32-bit indices: rt_create_grid refuses grids of 2^32 voxels or more
-        const unsigned vox = ((unsigned)(cz * A.bz + lz) * (unsigned)A.ny + (unsigned)(cy * A.by + ly)) * (unsigned)A.nx
-                             + (unsigned)(cx * A.bx + lx);
+        unsigned vox;
+        int vz;
+        if (A.unit && !lev) {                         // voxel-sized cell: the cell index is the voxel index
+          vz = cz;
+          vox = ((unsigned)cz * (unsigned)A.ny + (unsigned)cy) * (unsigned)A.nx + (unsigned)cx;
+        } else {
+          const float qx = local(da, rx, lev ? A.Lx1 : A.Lx), qy = local(db, ry, lev ? A.Ly1 : A.Ly),
+                      qz = local(dc, rz, lev ? A.Lz1 : A.Lz);
+          const int lx = min((int)(qx * A.rdx), (lev ? A.mx * A.bx : A.bx) - 1);
+          const int ly = min((int)(qy * A.rdy), (lev ? A.my * A.by : A.by) - 1);
+          const int lz = min((int)(qz * A.rdz), (lev ? A.mz * A.bz : A.bz) - 1);
+          vz = cz * A.bz + lz;
+          vox = ((unsigned)vz * (unsigned)A.ny + (unsigned)(cy * A.by + ly)) * (unsigned)A.nx + (unsigned)(cx * A.bx + lx);
+        }
         float4 v;
         if (kBatch && A.cloud) {
           const float kc = __ldg(A.cloud + vox);
-          const int z = cz * A.bz + lz;
+          const int z = vz;
           const float ka = __ldg(A.gas + (size_t)jpt * 2u * (unsigned)A.nz + z);
           const float kr = __ldg(A.gas + (size_t)jpt * 2u * (unsigned)A.nz + (unsigned)A.nz + z);
           const float2 pp = __ldg(A.point_par + jpt);
@@ -440,8 +465,17 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
           const float f = v.x * rk;
           const unsigned long long pq = min(1u << 24, (unsigned)(f * 16777216.0f));
           const unsigned long long a = (wq * pq) >> 24;
-          if (a) atomicAdd(A.atm_abs + vox, a);
-          if (a && direct && A.atm_dir) atomicAdd(A.atm_dir + vox, a);
+          if (a) {
+            if (A.atm_dir) {                          // heating split on: deposit at once, the direct part twice
+              atomicAdd(A.atm_abs + vox, a);
+              if (direct) atomicAdd(A.atm_dir + vox, a);
+            } else if (vox == pend_vox) {
+              pend_a += a;
+            } else {
+              if (pend_a) atomicAdd(A.atm_abs + pend_vox, pend_a);
+              pend_vox = vox; pend_a = a;
+            }
+          }
           wq -= a;
           if (wq == 0) { fate = 1; term = (uint32_t)vox; }
           xi = fmaf(u1, fabsf(kh) - v.x, v.x);      // what happens instead: uniform on [c1, k_hat)
@@ -473,7 +507,7 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
       // ---- BOUNDARY: arrival at the surface (§3.10), exit through the domain top (§3.11), or a change
       //      of level at the face of a merged cell (§3.7b) -------------------------------------------
       if (st == ST_BOUNDARY && (unsigned)cz < (unsigned)A.ncz) {
-        const bool px = da > -kTiny, py = db > -kTiny, pz = dc > -kTiny;   // nudged component positive
+        const bool px = da > 0.0f, py = db > 0.0f, pz = dc > 0.0f;
         const int ax = (int)(stp >> 24);
         const bool lev = !(__float_as_int(kh) < 0);   // kh already holds the ENTERED cell's word
         if (!lev) {
@@ -547,6 +581,7 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
       }
     }
     if (fate != 0) st = ST_DEAD;
+    if (kWeighted && fate != 0 && pend_a) { atomicAdd(A.atm_abs + pend_vox, pend_a); pend_a = 0; pend_vox = 0xffffffffu; }
 
     // ---- tallies (converged): warp-aggregated 64-bit integer atomics -----------------------------
     const unsigned ma = __ballot_sync(0xffffffffu, tally_a != nullptr);
@@ -559,20 +594,14 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
       // photons finished: count their fates per warp, write their records
       const unsigned f1 = __ballot_sync(0xffffffffu, fate == 1), f2 = __ballot_sync(0xffffffffu, fate == 2);
       const unsigned f3 = __ballot_sync(0xffffffffu, fate == 3), f4 = __ballot_sync(0xffffffffu, fate == 4);
+      unsigned f5 = 0u;
       if (kWeighted) {
-        const unsigned f5 = __ballot_sync(0xffffffffu, fate == 5);
-        if (lane == 0 && f5) atomicAdd(&s_cnt[C_ROUL_KILLED], (unsigned long long)__popc(f5));
-        if (fate == 4) atomicAdd(&s_cnt[C_CAPPED_E], wq);
+        f5 = __ballot_sync(0xffffffffu, fate == 5);
+        if (fate == 4) atomicAdd(&s_cnt[C_CAPPED_E], wq);     // rare: a 64-bit shared atomic is a CAS loop
       }
-      if (lane == 0) {
-        if (f1) atomicAdd(&s_cnt[C_ATM_ABS], (unsigned long long)__popc(f1));
-        if (f2) atomicAdd(&s_cnt[C_SFC_ABS], (unsigned long long)__popc(f2));
-        if (f3) atomicAdd(&s_cnt[C_TOA], (unsigned long long)__popc(f3));
-        if (f4) {
-          atomicAdd(&s_cnt[C_CAPPED], (unsigned long long)__popc(f4));
-          if (!kWeighted) atomicAdd(&s_cnt[C_CAPPED_E], kW0 * (unsigned long long)__popc(f4));
-        }
-      }
+      // lanes 1..5 add the number of photons that ended with fate = lane to the block's 32-bit counters
+      const unsigned mine = lane == 1 ? f1 : (lane == 2 ? f2 : (lane == 3 ? f3 : (lane == 4 ? f4 : (lane == 5 ? f5 : 0u))));
+      if (mine) atomicAdd(&s_fate[lane], (unsigned)__popc(mine));
       if (kRecords && fate != 0) {
         uint4 r;
         r.x = (uint32_t)fate | (min(t_sfc - b_sfc, 0xFFFFFFu) << 8);
@@ -584,7 +613,12 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
 
   flush_thread_counters();
   __syncthreads();
-  if (threadIdx.x == 0) s_cnt[C_NULL] -= s_cnt[C_ATM_ABS];   // events - scatters - absorptions
+  if (threadIdx.x == 0) {
+    s_cnt[C_ATM_ABS] += s_fate[1]; s_cnt[C_SFC_ABS] += s_fate[2]; s_cnt[C_TOA] += s_fate[3];
+    s_cnt[C_CAPPED] += s_fate[4]; s_cnt[C_ROUL_KILLED] += s_fate[5];
+    if (!kWeighted) s_cnt[C_CAPPED_E] += kW0 * (unsigned long long)s_fate[4];
+    s_cnt[C_NULL] -= s_cnt[C_ATM_ABS];   // events - scatters - absorptions
+  }
   __syncthreads();
   if (threadIdx.x < C_COUNT && s_cnt[threadIdx.x] != 0ull)
     atomicAdd(&A.counters[threadIdx.x], s_cnt[threadIdx.x]);

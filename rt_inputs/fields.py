@@ -26,8 +26,8 @@ class Config:
     cloud_ssa: float = 0.9999
     cloud_g: float = 0.86
     seed: int = 1              # Philox trace seed
-    block: tuple = (8, 8, 8)   # acceleration-grid block, voxels (Q1: the paper gives no size;
-                               # 2^3 is the fastest on the LES-scale fields, measured in profiles/)
+    block: tuple = (8, 8, 8)   # acceleration-grid block, voxels (Q1: the paper gives no size; on the
+                               # LES-scale fields voxel-sized cells merged 8^3 in clear air are the fastest, profiles/)
     merge: tuple = (1, 1, 1)   # merged acceleration cells: blocks of this many cells with
     merge_ratio: float = 1.25  # max k_ext <= merge_ratio * min k_ext are traversed as one cell
 
@@ -56,11 +56,11 @@ CONFIGS = {
     2: Config("cumulus_128x128x64", 128, 128, 64, 50.0, 50.0, 25.0, 45.0, 0.0, 1 << 22, 0.2, n_blobs=40,
               block=(4, 4, 4)),
     3: Config("cumulus_512x512x128", 512, 512, 128, 50.0, 50.0, 25.0, 60.0, 120.0, 1 << 26, 0.2,
-              n_blobs=600, block=(2, 2, 2), merge=(8, 8, 4)),
+              n_blobs=600, block=(1, 1, 1), merge=(8, 8, 8)),
     4: Config("spectral_512x512x128", 512, 512, 128, 50.0, 50.0, 25.0, 60.0, 120.0, 1 << 26, 0.2,
               n_blobs=600, block=(2, 2, 2), merge=(8, 8, 4)),
     5: Config("convergence_1024x1024x192", 1024, 1024, 192, 25.0, 25.0, 20.0, 50.0, 0.0, 1 << 28, 0.15,
-              n_blobs=2400, block=(2, 2, 2), merge=(8, 8, 4)),
+              n_blobs=2400, block=(1, 1, 1), merge=(8, 8, 8)),
 }
 
 

@@ -144,6 +144,17 @@ def test_config2_merged_cells():
     assert t.counters.n_relevel > (1 << 20)
 
 
+def test_config2_voxel_sized_cells():
+    """The bench configuration of configs 3 and 5 on BASELINE.json configs[1]'s field: acceleration cells of one
+    voxel (the kernel then takes the collision's voxel from the cell index and votes with its own thresholds),
+    merged 8 x 8 x 8 in clear air."""
+    from dataclasses import replace
+    cfg = replace(CONFIGS[2], block=(1, 1, 1), merge=(8, 8, 8))
+    opt = make_optics(cfg)
+    t, o64, same = _compare(cfg, opt, 1 << 20, min_same64=0.99)
+    assert t.counters.n_relevel > (1 << 20) and t.counters.n_null < 0.01 * t.counters.n_events
+
+
 def test_merged_cells_non_power_of_two_grid():
     """Acceleration grid of 24 x 12 x 16 cells (wrap by compare, not by mask), merged 4 x 2 x 4, sun from the
     north-east so photons wrap in both x and y."""

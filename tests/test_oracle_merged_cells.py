@@ -148,3 +148,32 @@ def test_merged_cells_leave_expectations_unchanged():
     msk = (ha + hb) >= 50
     chi2h = float(((ha - hb)[msk] ** 2 / (ha + hb)[msk]).sum())
     assert chi2h < msk.sum() + 4 * np.sqrt(2 * msk.sum()), (chi2h, int(msk.sum()))
+
+
+def test_voxel_sized_cells_have_no_null_collisions_and_the_same_expectations():
+    """Acceleration cells of ONE voxel (Q1: the bench configuration of configs 3 and 5), merged 4 x 4 x 4 in
+    clear air: the majorant of an unmerged cell is the voxel's own extinction, so a null collision can only happen
+    inside a merged cell (n_null <= the events of photons at level 1, here under 1 % of all events), every other
+    event is real; and the expectations are those of the 4^3-voxel single-level grid of BASELINE.json configs[1]
+    (domain means within 4 sigma, 16 x 16-column surface sums bin by bin)."""
+    cfg = CONFIGS[2]
+    opt = make_optics(cfg)
+    n = 1 << 19
+    a, _, _ = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, seed=31, n_threads=T)
+    b, _, _ = O.trace(cfg.grid[:6] + (1, 1, 1), opt, cfg.zenith_deg, cfg.azimuth_deg, n, seed=32, n_threads=T,
+                      merge=(4, 4, 4))
+    assert a.closure() == n * W0 and b.closure() == n * W0
+    ca, cb = a.counters, b.counters
+    assert ca.n_null > 2 * (ca.n_hg + ca.n_rayleigh)           # the coarse grid spends most events on null collisions
+    assert cb.n_null < 0.01 * cb.n_events and cb.n_relevel > n
+    # the REAL events are the physics: same rate in both (Poisson-like totals of ~8e6)
+    ra, rb = ca.n_events - ca.n_null, cb.n_events - cb.n_null
+    assert abs(ra - rb) < 0.01 * ra
+    for name in ("atm_abs", "sfc_dir", "sfc_dif", "sfc_abs", "toa_up"):
+        pa, pb = frac(getattr(a, name), n), frac(getattr(b, name), n)
+        pm = 0.5 * (pa + pb)
+        assert abs(pa - pb) < 4 * np.sqrt(2 * pm * (1 - pm) / n), (name, pa, pb)
+    sa = (a.sfc_dir + a.sfc_dif).reshape(8, 16, 8, 16).sum(axis=(1, 3)).astype(np.float64) / W0
+    sb = (b.sfc_dir + b.sfc_dif).reshape(8, 16, 8, 16).sum(axis=(1, 3)).astype(np.float64) / W0
+    chi2 = float(((sa - sb) ** 2 / (sa + sb)).sum())
+    assert chi2 < 64 + 4 * np.sqrt(2 * 64), chi2
