@@ -149,10 +149,7 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
   uint32_t t_ev = 0, t_sc = 0, t_hg = 0, t_sfc = 0, t_cells = 0, t_relevel = 0;
   unsigned long long wq = kW0;            // weighted mode: the photon's weight in tally quanta
   unsigned long long t_rlost = 0, t_rgain = 0;   // roulette ledger of this thread
-  // weighted mode: deposits of consecutive tentative collisions in the SAME voxel are summed here and reach the
-  // tally as one atomic when the voxel changes or the photon ends (integer sums: the tally is the same)
-  unsigned long long pend_a = 0;
-  uint32_t pend_vox = 0xffffffffu;
+
   uint32_t t_rkept = 0;
   uint32_t b_ev = 0, b_sc = 0, b_sfc = 0;  // totals when the current photon was launched (records only)
 
@@ -465,17 +462,10 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
           const float f = v.x * rk;
           const unsigned long long pq = min(1u << 24, (unsigned)(f * 16777216.0f));
           const unsigned long long a = (wq * pq) >> 24;
-          if (a) {
-            if (A.atm_dir) {                          // heating split on: deposit at once, the direct part twice
-              atomicAdd(A.atm_abs + vox, a);
-              if (direct) atomicAdd(A.atm_dir + vox, a);
-            } else if (vox == pend_vox) {
-              pend_a += a;
-            } else {
-              if (pend_a) atomicAdd(A.atm_abs + pend_vox, pend_a);
-              pend_vox = vox; pend_a = a;
-            }
-          }
+          // one reduction per tentative collision.  Summing consecutive deposits into the same voxel in registers
+          // first was measured slower (95.7 -> 101.7 ms on config 3: three more registers spill, profiles/r2_trace_kernel.md)
+          if (a) atomicAdd(A.atm_abs + vox, a);
+          if (a && direct && A.atm_dir) atomicAdd(A.atm_dir + vox, a);
           wq -= a;
           if (wq == 0) { fate = 1; term = (uint32_t)vox; }
           xi = fmaf(u1, fabsf(kh) - v.x, v.x);      // what happens instead: uniform on [c1, k_hat)
@@ -581,7 +571,6 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
       }
     }
     if (fate != 0) st = ST_DEAD;
-    if (kWeighted && fate != 0 && pend_a) { atomicAdd(A.atm_abs + pend_vox, pend_a); pend_a = 0; pend_vox = 0xffffffffu; }
 
     // ---- tallies (converged): warp-aggregated 64-bit integer atomics -----------------------------
     const unsigned ma = __ballot_sync(0xffffffffu, tally_a != nullptr);
