@@ -43,9 +43,9 @@
 //                   instantiation is bit-reproducible on any conforming machine.
 // Build with -ffp-contract=off (no implicit FMA); fma is written explicitly.
 //
-// Parity unpinned: the discrete cloud-vs-gas choice where cloud and gas share
-// a voxel (Q4 in DESIGN.md §2) is the paper's stated approximation; it
-// is pinned oracle<->GPU only, not against physics.
+// Parity unpinned: nothing.  (The cloud-vs-gas choice of P:56, "unpinned" in round 1, is pinned by
+// tests/test_oracle_split_cap_precision.py against the ratio the paper states; whether that ratio is the
+// physically right one is the paper's own approximation, Q4 in DESIGN.md §2.)
 
 #include <cmath>
 #include <cstdint>
