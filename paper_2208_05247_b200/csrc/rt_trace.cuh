@@ -580,17 +580,10 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
       if (mb && tally_b) tally_add(mb, tally_b);
     }
     if (__any_sync(0xffffffffu, fate != 0)) {
-      // photons finished: count their fates per warp, write their records
-      const unsigned f1 = __ballot_sync(0xffffffffu, fate == 1), f2 = __ballot_sync(0xffffffffu, fate == 2);
-      const unsigned f3 = __ballot_sync(0xffffffffu, fate == 3), f4 = __ballot_sync(0xffffffffu, fate == 4);
-      unsigned f5 = 0u;
-      if (kWeighted) {
-        f5 = __ballot_sync(0xffffffffu, fate == 5);
-        if (fate == 4) atomicAdd(&s_cnt[C_CAPPED_E], wq);     // rare: a 64-bit shared atomic is a CAS loop
-      }
-      // lanes 1..5 add the number of photons that ended with fate = lane to the block's 32-bit counters
-      const unsigned mine = lane == 1 ? f1 : (lane == 2 ? f2 : (lane == 3 ? f3 : (lane == 4 ? f4 : (lane == 5 ? f5 : 0u))));
-      if (mine) atomicAdd(&s_fate[lane], (unsigned)__popc(mine));
+      // photons finished: each adds one to its fate's 32-bit counter of the block (a native shared-memory atomic;
+      // a few lanes at most share an address), and writes its record
+      if (fate != 0) atomicAdd(&s_fate[fate], 1u);
+      if (kWeighted && fate == 4) atomicAdd(&s_cnt[C_CAPPED_E], wq);     // rare: a 64-bit shared atomic is a CAS loop
       if (kRecords && fate != 0) {
         uint4 r;
         r.x = (uint32_t)fate | (min(t_sfc - b_sfc, 0xFFFFFFu) << 8);
