@@ -43,6 +43,8 @@
 //                   instantiation is bit-reproducible on any conforming machine.
 // Build with -ffp-contract=off (no implicit FMA); fma is written explicitly.
 //
+// Independent witness of the traversal and level-change arithmetic: tests/reference_walk.py (global
+// coordinates, no levels, pure Python) must give the same photons, record by record.
 // Parity unpinned: nothing.  (The cloud-vs-gas choice of P:56, "unpinned" in round 1, is pinned by
 // tests/test_oracle_split_cap_precision.py against the ratio the paper states; whether that ratio is the
 // physically right one is the paper's own approximation, Q4 in DESIGN.md §2.)

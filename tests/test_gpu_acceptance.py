@@ -53,26 +53,27 @@ def finest_block(ref, min_hits, min_blocks):
         blk[ax] //= 2
 
 
-def accept(cfg, opt, n, heat_blk=None, col_blk=(8, 8), stream_id=0, min_blocks=4, heat_min_hits=10_000):
+def accept(cfg, opt, n, heat_blk=None, col_blk=(8, 8), stream_id=0, min_blocks=4, heat_min_hits=10_000, weighted=False):
     """GPU and fp64 oracle on the same n photon ids: closure, 4-sigma domain means, < 2 % block RMS of the surface
     irradiance AND the heating over blocks with >= 1e4 hits (the block sizes are chosen so that such blocks exist:
     a test over no block would be vacuous; heat_blk = None takes the finest block size that leaves min_blocks of
     them); returns the identical-record fraction."""
     rt = _rt()
     g = rt.Grid(*cfg.grid, device=0, **cfg.accel)
+    g.set_mode(weighted)
     g.set_optics(opt["k_ext"], opt["k_ext_cloud"], opt["ssa"], opt["g"], opt["sfc_albedo"])
     rec = g.trace(cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed, stream_id=stream_id, records=True)
     t = g.read_tallies()
     rec = rec.cpu().numpy().view(np.uint32)
     g.close()
     o64, rec64, _ = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed, stream_id=stream_id,
-                            precision=64, records=True, n_threads=T, **cfg.accel)
-    assert t.closure() == n * rt.W0 and o64.closure() == n * rt.W0
+                            precision=64, records=True, n_threads=T, weighted=weighted, **cfg.accel)
+    assert t.closure() == n * rt.W0 and o64.closure() == n * rt.W0      # the roulette ledger included (weighted)
     assert t.counters.n_capped == 0 and t.counters.n_photons == n
     for name in NAMES:
         pg = float(getattr(t, name).sum()) / (n * rt.W0)
         po = float(getattr(o64, name).sum()) / (n * rt.W0)
-        sigma = np.sqrt(max(po * (1 - po), 1e-12) / n)
+        sigma = np.sqrt(max(po * (1 - po), 1e-12) / n)     # binomial: an upper bound for the weighted estimator too
         assert abs(pg - po) <= 4 * sigma, (name, pg, po, sigma)
     sfc_g = t.sfc_dir.numpy() + t.sfc_dif.numpy()
     sfc_o = o64.sfc_dir + o64.sfc_dif
@@ -122,6 +123,16 @@ def test_acceptance_config4_three_points():
     for j in (3, 56, 108):
         opt = make_optics(cfg, pts[j])
         accept(replace(cfg, name="%s point %d" % (cfg.name, j)), opt, 1 << 22, col_blk=None, stream_id=j)
+
+
+def test_acceptance_weighted_mode_configs_2_and_3():
+    """The paper's own scheme (weights + Russian roulette) against the fp64 oracle in the
+    same mode: config 2 in full and 2^22 photons of config 3.  Deposits at every collision fill the heating bins
+    far faster than analog absorptions, so the heating is compared at a much finer resolution."""
+    cfg = CONFIGS[2]
+    accept(cfg, make_optics(cfg), cfg.n_photons, weighted=True)
+    cfg = CONFIGS[3]
+    accept(cfg, make_optics(cfg), 1 << 22, col_blk=(32, 32), weighted=True)
 
 
 def test_acceptance_config5_sample():
