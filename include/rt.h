@@ -84,7 +84,8 @@ int rt_set_optics(rt_ctx* ctx, const float* k_ext, const float* k_ext_cloud, con
  * (DESIGN.md §3.6-3.12).  Sun at zenith_deg in [0, 90) and azimuth_deg clockwise from
  * north (position of the sun).  Random numbers: Philox4x32-10, key = seed, counter =
  * (photon id, event index, stream_id).  ADDS to the tallies and counters.  Asynchronous on
- * `cuda_stream`. */
+ * `cuda_stream`.  A call of more than 2^31 photons runs as consecutive launches of 2^31 (same photons: the parts are
+ * index ranges of the one job); rt_trace_batch takes at most 2^31 photons per call. */
 int rt_trace(rt_ctx* ctx, double zenith_deg, double azimuth_deg, uint64_t n_photons,
              uint64_t first_photon_id, uint64_t seed, uint32_t stream_id, void* cuda_stream);
 

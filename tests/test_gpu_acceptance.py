@@ -127,8 +127,8 @@ def test_acceptance_config4_three_points():
 
 def test_acceptance_weighted_mode_configs_2_and_3():
     """The paper's own scheme (weights + Russian roulette) against the fp64 oracle in the
-    same mode: config 2 in full and 2^22 photons of config 3.  Deposits at every collision fill the heating bins
-    far faster than analog absorptions, so the heating is compared at a much finer resolution."""
+    same mode: config 2 in full and 2^22 photons of config 3 (closure with the roulette ledger, domain means, block
+    RMS of irradiance and heating; "hits" are deposited quanta / W0)."""
     cfg = CONFIGS[2]
     accept(cfg, make_optics(cfg), cfg.n_photons, weighted=True)
     cfg = CONFIGS[3]
