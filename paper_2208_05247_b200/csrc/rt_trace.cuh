@@ -2,23 +2,23 @@
 //
 // One thread carries one photon at a time.  Its position inside the current acceleration cell is held
 // as the remaining distances (rx, ry, rz) along the flight direction to the cell's next face on each
-// axis: a cell crossing is ~25 instructions (smallest of three, two subtractions, one
-// reset to the face spacing, index step, one 4-byte load of the majorant), a null collision updates the
-// three distances and nothing else.  With cheap crossings a fine acceleration grid (2^3 voxels per
-// cell) pays: 38 tentative collisions and 168 crossings per photon on the 512x512x128 cumulus field
-// instead of 202 and 42 with 8^3 cells.
+// axis: a cell crossing is ~25 arithmetic instructions (smallest of three, two subtractions, one
+// reset to the face spacing, index step) and one 4-byte load of the majorant.  With crossings that cheap the
+// acceleration grid can be as fine as the simulation grid where the medium is not homogeneous: cells of ONE voxel
+// (merged 8^3 where the air is clear) have the voxel's own extinction as majorant, so there are no
+// null collisions outside merged cells: 15.8 tentative collisions and 77 crossings per photon on the 512x512x128
+// cumulus field, against 38 + 58 with 2^3-voxel cells and 202 + 42 with 8^3.
 //
-// Divergence.  The cheap step, MOVE (find the nearest face; cross it, or notice that the tentative
-// collision comes first), is what live lanes do by default.  The expensive steps are each wanted by few
-// lanes per iteration -- a collision (voxel gather, classification, Philox draw, logarithm: ~180
-// instructions) by ~5 of 32, a real scatter (phase-function inversion, rotation, three IEEE divisions:
-// ~250) by ~2, a surface or domain-top arrival by fewer -- and run inline they executed with 2-6 lanes
-// active (ncu, profiles/r1_*: 11-14 active threads per instruction overall).  So a lane that needs one
-// PARKS in COLLIDE, SCATTER or BOUNDARY, and the warp votes (ballot/popc) to run that phase once enough
-// lanes wait for it; DEAD lanes are refilled kRegenBatch at a time from a warp-private pool of photon
-// ids taken in chunks from a global counter (BASELINE.json north_star: "compacted and regenerated
-// persistently with warp-level ballot/shuffle").  A photon's own sequence of arithmetic operations does
-// not depend on the scheduling, so neither do the results.
+// Divergence.  The cheap step, MOVE (find the nearest face; cross it, change level if the entered cell is at the
+// other level, or notice that the tentative collision comes first), is what live lanes do by default, in a ROLLED
+// loop (one copy: the kernel is larger than the instruction cache and reacts to every added copy).  The expensive
+// steps are each wanted by few lanes per iteration -- a collision (voxel gather, classification, Philox draw,
+// logarithm), a real scatter (phase-function inversion, rotation, three reciprocals), a surface or domain-top
+// arrival -- and run inline they executed with 2-6 lanes active.  So a lane that needs one PARKS in COLLIDE, SCATTER
+// or BOUNDARY, and the warp votes to run that phase once enough lanes wait for it; DEAD lanes are refilled
+// kRegenBatch at a time from a warp-private pool of photon ids taken in chunks from a global counter
+// (BASELINE.json north_star: "compacted and regenerated persistently with warp-level ballot/shuffle").  A photon's own
+// sequence of arithmetic operations does not depend on the scheduling, so neither do the results.
 #pragma once
 #include "rt_device.cuh"
 
@@ -37,7 +37,7 @@ constexpr int kMinBlocks = 4;          // resident blocks per SM the launch boun
 constexpr int kRegenBatch = 6;         // refill when this many lanes are idle (or nothing else to do)
 constexpr int kScatterBatch = 8;       // SCATTER
 constexpr int kCollideBatch = 8, kCollideBatchUnit = 12;   // COLLIDE: cells of several voxels / voxel-sized cells
-constexpr int kBoundaryBatch = 4;      // BOUNDARY
+constexpr int kBoundaryBatch = 8;      // BOUNDARY: surface and domain-top arrivals (1 per photon)
 constexpr int kMoveSteps = 3, kMoveStepsUnit = 4;           // MOVE steps between two votes
 constexpr unsigned vote_bias(int collide_batch) {
   return (32u - kRegenBatch) | ((32u - 1u) << 6) | ((32u - (unsigned)collide_batch) << 12) |
@@ -231,6 +231,38 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
       st = ST_MOVE;
     }
   };
+  // ---- §3.7b change of level at the face of a merged cell, right where MOVE finds it (ax = the axis just crossed;
+  //      kh already holds the ENTERED cell's word).  It used to be a parked phase of its own: 3 per photon, batches
+  //      of 4-6 lanes, one visit running both directions and often the arrival code too (31 % of the kernel's
+  //      instructions, profiles/r2_trace_kernel.md); inline it runs for the 1-2 lanes that need it at that step.
+  auto relevel = [&](int ax) {
+    const bool px = da > 0.0f, py = db > 0.0f, pz = dc > 0.0f;
+    if (__float_as_int(kh) < 0) {
+      // into a merged cell: distances to ITS faces (n whole cells further on the other two axes),
+      // the index becomes its origin
+      const int ox = cx & (A.mx - 1), oy = cy & (A.my - 1), oz = cz & (A.mz - 1);   // powers of two
+      const float fx = (float)A.mx, fy = (float)A.my, fz = (float)A.mz;
+      rx = (ax == 0) ? delx * fx : fmaf((float)(px ? A.mx - 1 - ox : ox), delx, rx);
+      ry = (ax == 1) ? dely * fy : fmaf((float)(py ? A.my - 1 - oy : oy), dely, ry);
+      rz = (ax == 2) ? delz * fz : fmaf((float)(pz ? A.mz - 1 - oz : oz), delz, rz);
+      delx *= fx; dely *= fy; delz *= fz;       // exact: the factors are powers of two
+      cx -= ox; cy -= oy; cz -= oz;
+      set_steps(true);
+    } else {
+      // out of a merged cell into single cells: which cell of the entered block on the other two
+      // axes (k whole cells before the block's face), and the distances to that cell's faces
+      delx *= A.rmx; dely *= A.rmy; delz *= A.rmz;
+      if (ax == 0) { rx = delx; if (!px) cx += A.mx - 1; }
+      else { const int k = min(A.mx - 1, (int)(rx / delx)); rx = fmaxf(0.0f, fmaf(-(float)k, delx, rx)); cx += px ? A.mx - 1 - k : k; }
+      if (ax == 1) { ry = dely; if (!py) cy += A.my - 1; }
+      else { const int k = min(A.my - 1, (int)(ry / dely)); ry = fmaxf(0.0f, fmaf(-(float)k, dely, ry)); cy += py ? A.my - 1 - k : k; }
+      if (ax == 2) { rz = delz; if (!pz) cz += A.mz - 1; }
+      else { const int k = min(A.mz - 1, (int)(rz / delz)); rz = fmaxf(0.0f, fmaf(-(float)k, delz, rz)); cz += pz ? A.mz - 1 - k : k; }
+      kh = __ldg(A.khat + cell_of());             // the single cell's own majorant (sign bit clear)
+      set_steps(false);
+    }
+    ++t_relevel;
+  };
 
   for (;;) {
     // the vote: one warp-wide integer add counts the lanes in each of the five states (6 bits each)
@@ -355,12 +387,12 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
     // a lane moves and no parked phase has reached its batch size
     if ((full & (bM | bC | bS | bB)) == bM) {
       // ---- MOVE: nearest face of the current cell (ties x < y < z), then cross or park (§3.7) -------
-      // index step per axis: +-1 cell, or +-m cells inside a merged cell
-      const int sx = (int)(stp << 24) >> 24, sy = (int)(stp << 16) >> 24, sz = (int)(stp << 8) >> 24;
-#pragma unroll
-      for (int rep = 0; rep < kMoveStepsUnit; ++rep) {
-      if (rep >= A.move_steps) break;              // warp-uniform
+      // (rolled loop: one copy of the step and of the level change; the kernel is larger than the instruction cache)
+#pragma unroll 1
+      for (int rep = 0; rep < A.move_steps; ++rep) {
       if (st == ST_MOVE) {
+        // index step per axis: +-1 cell, or +-m cells inside a merged cell
+        const int sx = (int)(stp << 24) >> 24, sy = (int)(stp << 16) >> 24, sz = (int)(stp << 8) >> 24;
         const bool ax0 = (rx <= ry) && (rx <= rz);
         const bool ax1 = !ax0 && (ry <= rz);
         const bool ax2 = !ax0 && !ax1;
@@ -387,11 +419,9 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
           if ((unsigned)cz >= (unsigned)A.ncz) st = ST_BOUNDARY;   // surface (cz < 0) or domain top
           else {
             const float raw = __ldg(A.khat + cell_of());
-            if ((__float_as_int(raw) ^ __float_as_int(kh)) < 0) {   // §3.7b: the entered cell is at the other level
-              st = ST_BOUNDARY;
-              stp = (stp & 0x00ffffffu) | (ax0 ? 0u : (ax1 ? 0x01000000u : 0x02000000u));
-            }
+            const bool other = (__float_as_int(raw) ^ __float_as_int(kh)) < 0;   // §3.7b: the entered cell is at the other level
             kh = raw;
+            if (other) relevel(ax0 ? 0 : (ax1 ? 1 : 2));
           }
         }
       }
@@ -494,39 +524,8 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
         }
       }
     } else {
-      // ---- BOUNDARY: arrival at the surface (§3.10), exit through the domain top (§3.11), or a change
-      //      of level at the face of a merged cell (§3.7b) -------------------------------------------
-      if (st == ST_BOUNDARY && (unsigned)cz < (unsigned)A.ncz) {
-        const bool px = da > 0.0f, py = db > 0.0f, pz = dc > 0.0f;
-        const int ax = (int)(stp >> 24);
-        const bool lev = !(__float_as_int(kh) < 0);   // kh already holds the ENTERED cell's word
-        if (!lev) {
-          // into a merged cell: distances to ITS faces (n whole cells further on the other two axes),
-          // the index becomes its origin
-          const int ox = cx & (A.mx - 1), oy = cy & (A.my - 1), oz = cz & (A.mz - 1);   // powers of two
-          const float fx = (float)A.mx, fy = (float)A.my, fz = (float)A.mz;
-          rx = (ax == 0) ? delx * fx : fmaf((float)(px ? A.mx - 1 - ox : ox), delx, rx);
-          ry = (ax == 1) ? dely * fy : fmaf((float)(py ? A.my - 1 - oy : oy), dely, ry);
-          rz = (ax == 2) ? delz * fz : fmaf((float)(pz ? A.mz - 1 - oz : oz), delz, rz);
-          delx *= fx; dely *= fy; delz *= fz;       // exact: the factors are powers of two
-          cx -= ox; cy -= oy; cz -= oz;
-          set_steps(true);
-        } else {
-          // out of a merged cell into single cells: which cell of the entered block on the other two
-          // axes (k whole cells before the block's face), and the distances to that cell's faces
-          delx *= A.rmx; dely *= A.rmy; delz *= A.rmz;
-          if (ax == 0) { rx = delx; if (!px) cx += A.mx - 1; }
-          else { const int k = min(A.mx - 1, (int)(rx / delx)); rx = fmaxf(0.0f, fmaf(-(float)k, delx, rx)); cx += px ? A.mx - 1 - k : k; }
-          if (ax == 1) { ry = dely; if (!py) cy += A.my - 1; }
-          else { const int k = min(A.my - 1, (int)(ry / dely)); ry = fmaxf(0.0f, fmaf(-(float)k, dely, ry)); cy += py ? A.my - 1 - k : k; }
-          if (ax == 2) { rz = delz; if (!pz) cz += A.mz - 1; }
-          else { const int k = min(A.mz - 1, (int)(rz / delz)); rz = fmaxf(0.0f, fmaf(-(float)k, delz, rz)); cz += pz ? A.mz - 1 - k : k; }
-          kh = __ldg(A.khat + cell_of());             // the single cell's own majorant (sign bit clear)
-          set_steps(false);
-        }
-        ++t_relevel;
-        st = ST_MOVE;
-      } else if (st == ST_BOUNDARY) {
+      // ---- BOUNDARY: arrival at the surface (§3.10) or exit through the domain top (§3.11) ---------------
+      if (st == ST_BOUNDARY) {
         const bool lev = __float_as_int(kh) < 0;
         const float qx = local(da, rx, lev ? A.Lx1 : A.Lx), qy = local(db, ry, lev ? A.Ly1 : A.Ly);
         const int hx = cx * A.bx + min((int)(qx * A.rdx), (lev ? A.mx * A.bx : A.bx) - 1);
