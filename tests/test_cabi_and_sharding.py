@@ -169,3 +169,24 @@ def test_bench_reference_arm_prints_the_contract_line():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1",
                           "--warmup", "0"], capture_output=True, text=True, env=env, timeout=600)
     assert out.returncode == 0 and out.stdout.strip() == ""
+
+
+def test_committed_ncu_counters_belong_to_the_kernel_as_it_stands():
+    """bench.py's roofline uses profiles/trace_kernel_counters.json only for the kernel it was captured from (sha256 of
+    rt_trace.cuh + rt_device.cuh).  A kernel edit without a new capture would silently fall back to the algorithmic
+    model: this test makes that visible.  Also checks the fields bench.py reads."""
+    import json
+    sys.path.insert(0, ROOT)
+    import bench
+    from rt_inputs import CONFIGS
+    with open(bench.COUNTERS_FILE) as f:
+        entries = json.load(f)["entries"]
+    sha = bench._kernel_sha16()
+    assert entries and all(e["kernel_sha16"] == sha for e in entries), (sha, [e["kernel_sha16"] for e in entries])
+    cfg = CONFIGS[3]
+    e = bench._ncu_counters(cfg, "analog", cfg.n_photons)
+    assert e is not None and e["block"] == list(cfg.block) and e["merge"] == list(cfg.merge)
+    for k in ("lts_t_sectors_op_read", "dram_bytes_read", "dram_bytes_write", "inst_executed", "thread_inst_executed",
+              "issue_active_pct"):
+        assert e[k] > 0
+    assert bench._ncu_counters(cfg, "weighted", cfg.n_photons) is not None
