@@ -219,10 +219,13 @@ def run_ours(args):
         facs = None
         if factored:
             # FACTORED inputs (rt_set_optics_factored): one cloud field on the device + 2 nz numbers per point
+            import numpy as np
             from rt_inputs import factored_point
             facs = [factored_point(cfg, p) for p in pts]
             kc_dev = torch.from_numpy(facs[0]["k_cloud"]).to(dev)
             al_dev = torch.from_numpy(facs[0]["sfc_albedo"]).to(dev)
+            ka_all = torch.from_numpy(np.stack([f["k_abs"] for f in facs])).pin_memory()     # [112][nz]
+            kr_all = torch.from_numpy(np.stack([f["k_ray"] for f in facs])).pin_memory()
             resident = None
         else:
             resident = [[make_optics_torch(cfg, p, device=dev)[k] for k in names] for p in pts]
@@ -254,9 +257,13 @@ def run_ours(args):
                 g.set_optics_factored(j, kc, f["k_abs"], f["k_ray"], f["cloud_ssa"], f["cloud_g"], al)
         else:
             g.set_cloud(kc)
-            for j, f in enumerate(facs):
-                g.set_point(j, f["k_abs"], f["k_ray"], f["cloud_ssa"], f["cloud_g"], al)
+            if args.point_by_point:
+                for j, f in enumerate(facs):
+                    g.set_point(j, f["k_abs"], f["k_ray"], f["cloud_ssa"], f["cloud_g"], al)
+            else:                          # rt_set_points: all 112 in one call (one albedo for all points)
+                g.set_points(0, ka_all, kr_all, [f["cloud_ssa"] for f in facs], [f["cloud_g"] for f in facs], al)
 
+    sweep_ms = []                      # spectral sweep: device time of set-up + trace per step
     def step(i, fields, out):
         g.reset_tallies()
         first = weak_range(rank, world, i, n)[0]
@@ -284,7 +291,10 @@ def run_ours(args):
                     setattr(t.counters, name, getattr(t.counters, name) + getattr(t2.counters, name))
             if t.counters.n_photons != n or t.counters.n_capped != 0:
                 raise SystemExit("bench.py: photon count mismatch (%d of %d)" % (t.counters.n_photons, n))
-            return t, ea.elapsed_time(eb)
+            # one launch traces the whole sweep (batched): its own device time is the kernel's; the events around the
+            # sweep also hold the set-up of the 112 points and the host's gaps between those calls
+            sweep_ms.append(ea.elapsed_time(eb))
+            return t, (g.last_trace_ms() if batched else sweep_ms[-1])
         else:
             g.set_optics(*fields)                                    # S0 pack, S1 majorant
             g.trace(cfg.zenith_deg, cfg.azimuth_deg, n, first_photon_id=first, seed=cfg.seed)  # S2-S10
@@ -297,6 +307,7 @@ def run_ours(args):
 
     for i in range(args.warmup):
         step(i, resident, pinned_cols)
+    sweep_ms.clear()
 
     # ---- device-timed region: inputs resident in HBM ---------------------------------------------------
     uuid = None
@@ -484,7 +495,7 @@ def run_ours(args):
     for label, foot in (("hbm_whole_array", 0), ("l2_16MiB", min(1 << 20, cfg.nvox))):
         gb_ms, gb_loads = g.gather_bench(64, foot)
         gather[label] = gb_loads / (gb_ms * 1e-3)
-    ncu = _ncu_counters(cfg, args.mode, n) if not spectral else None
+    ncu = _ncu_counters(cfg, args.mode, n) if (not spectral or (args.contexts == 0 and not args.packed_slots and not args.full_fields)) else None
     if ncu:
         t_l2 = ncu["lts_t_sectors_op_read"] / gather["l2_16MiB"]
         t_hbm = ncu["dram_bytes_read"] / SECTOR / gather["hbm_whole_array"]
@@ -533,6 +544,8 @@ def run_ours(args):
         "events_per_photon": total_events / total_photons,
         "per_photon": {k: per[k] / n for k in ("n_events", "n_null", "n_hg", "n_rayleigh", "n_cell_steps", "n_relevel",
                                                "n_sfc_hits")},
+        "spectral_sweep": ({"device_ms": sum(sweep_ms) / len(sweep_ms), "trace_ms": ms_avg,
+                            "set_up_ms": sum(sweep_ms) / len(sweep_ms) - ms_avg} if sweep_ms else None),
         "trace_kernel": {"ms": ms_avg, "paths_per_s": n / (ms_avg * 1e-3), "events_per_s": trace_events_per_s},
         "config": {"workload": cfg.name, "grid": [cfg.nx, cfg.ny, cfg.nz], "photons_per_gpu_per_step": n,
                    "block": list(cfg.block), "merge": list(cfg.merge), "merge_ratio": cfg.merge_ratio,
@@ -542,7 +555,7 @@ def run_ours(args):
                    "l2": ("inputs exceed L2 (%d MiB packed optics + %d MiB tallies vs 126 MB)" % (
                        cfg.nvox * 16 >> 20, cfg.nvox * 8 >> 20)) if cfg.nvox * 24 > (126 << 20) else
                          "inputs fit L2; every step traces new photon ids",
-                   "step": ("reset_tallies + set_cloud + 112 x set_point (--packed-slots: 112 x set_optics_factored; "
+                   "step": ("reset_tallies + set_cloud + set_points for the 112 points (--point-by-point: 112 x set_point; --packed-slots: 112 x set_optics_factored; "
                             "--full-fields: 112 x set_optics_slot) + one trace_batch launch (stream_id = point) + "
                             "read_tallies" if spectral and args.contexts == 0 else
                             "reset_tallies + 112 x (set_optics + trace, stream_id = point; points alternating over "
@@ -582,6 +595,8 @@ def main():
     ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
     ap.add_argument("--workload", type=int, choices=(1, 2, 3, 4, 5), default=WORKLOAD,
                     help="BASELINE.json configs[N-1]; the default (3) is the configuration the metric is quoted on")
+    ap.add_argument("--point-by-point", action="store_true",
+                    help="workload 4: one rt_set_point call per spectral point instead of one rt_set_points call")
     ap.add_argument("--block", default=None, help="acceleration-grid block bx,by,bz (default: the config's)")
     ap.add_argument("--mode", choices=("analog", "weighted"), default="analog",
                     help="absorption scheme: analog (the metric's, default) or the paper's weights + roulette")

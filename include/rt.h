@@ -202,10 +202,25 @@ int rt_set_optics_factored(rt_ctx* ctx, int slot, const float* k_cloud, const fl
  * slots.  k_abs, k_ray (nz), sfc_albedo (ncol): HOST or DEVICE.  Needs rt_set_slots (any n >= 1) beforehand; the
  * points of one rt_trace_batch launch must all be of the same kind.  Per point this costs a pass over the cell
  * tables (a few MB) instead of over the voxel fields, and no 16 B x nvox slot.  Errors: RT_EINVAL, RT_ESTATE
- * (rt_set_point before rt_set_cloud), RT_EOPTICS, RT_ENOMEM, RT_ECUDA. */
+ * (rt_set_point before rt_set_cloud), RT_EOPTICS, RT_ENOMEM, RT_ECUDA.
+ * Voxel-sized acceleration cells (bx = by = bz = 1) with merging on (rt_set_merge): no majorant
+ *   table is built per point at all.  A voxel-sized cell's majorant IS the voxel's extinction
+ *   fl((k_abs[z] + k_ray[z]) + k_cloud), which the trace reads from the shared cloud field; rt_set_cloud derives the
+ *   cloud extrema per block of mx x my x mz cells and level, and a point keeps one word per block (merged or not,
+ *   and the block's maximum) plus nz gas sums.  Photons are bit-identical to those traced with the table
+ *   (rt_set_optics_slot on the assembled fields).  In this mode rt_read_majorant returns RT_ESTATE after
+ *   rt_set_point(0), and rt_set_merge also invalidates the cloud field (call rt_set_cloud again).
+ * rt_set_points: the slots first_slot .. first_slot + n_points - 1 in one call.  k_abs, k_ray: [n_points][nz], HOST or
+ *   DEVICE; cloud_ssa, cloud_g: HOST arrays of n_points; point p's albedo at sfc_albedo + p * albedo_stride (HOST or
+ *   DEVICE; albedo_stride = 0: one albedo for all points, else >= ncol).  Same result as n_points rt_set_point calls;
+ *   on voxel-sized merged cells it costs a fixed number of copies and two kernels whatever n_points is (the host's
+ *   per-point call overhead is what a sweep over 112 points otherwise spends a tenth of its time on). */
 int rt_set_cloud(rt_ctx* ctx, const float* k_cloud, void* cuda_stream);
 int rt_set_point(rt_ctx* ctx, int slot, const float* k_abs, const float* k_ray, float cloud_ssa, float cloud_g,
                  const float* sfc_albedo, void* cuda_stream);
+int rt_set_points(rt_ctx* ctx, int first_slot, int n_points, const float* k_abs, const float* k_ray,
+                  const float* cloud_ssa, const float* cloud_g, const float* sfc_albedo, uint64_t albedo_stride,
+                  void* cuda_stream);
 int rt_trace_batch(rt_ctx* ctx, double zenith_deg, double azimuth_deg, int first_point, int n_points,
                    const uint64_t* counts, uint64_t first_photon_id, uint64_t seed, void* cuda_stream,
                    uint32_t* records_out);

@@ -12,7 +12,7 @@ W0 = 1 << 32
 FATE_ATM_ABS, FATE_SFC_ABS, FATE_TOD_EXIT, FATE_CAPPED, FATE_ROULETTE = 1, 2, 3, 4, 5
 MODE_ANALOG, MODE_WEIGHTED = 0, 1
 
-EXPORTS = ("rt_create_grid", "rt_set_merge", "rt_set_mode", "rt_set_source", "rt_set_optics", "rt_set_slots", "rt_set_optics_slot", "rt_set_optics_factored", "rt_set_cloud", "rt_set_point", "rt_trace_batch", "rt_trace", "rt_trace_records", "rt_trace_range", "rt_read_tallies", "rt_read_tallies_async",
+EXPORTS = ("rt_create_grid", "rt_set_merge", "rt_set_mode", "rt_set_source", "rt_set_optics", "rt_set_slots", "rt_set_optics_slot", "rt_set_optics_factored", "rt_set_cloud", "rt_set_point", "rt_set_points", "rt_trace_batch", "rt_trace", "rt_trace_records", "rt_trace_range", "rt_read_tallies", "rt_read_tallies_async",
            "rt_reset_tallies", "rt_set_heating_split", "rt_read_heating_direct", "rt_tally_to_flux", "rt_read_majorant", "rt_read_packed_optics", "rt_gather_bench",
            "rt_last_trace_ms", "rt_launch_count", "rt_philox_words", "rt_last_error", "rt_destroy")
 
@@ -56,6 +56,7 @@ def lib():
     L.rt_set_optics_factored.argtypes = [vp, i32, vp, vp, vp, f32, f32, vp, vp]
     L.rt_set_cloud.argtypes = [vp, vp, vp]
     L.rt_set_point.argtypes = [vp, i32, vp, vp, f32, f32, vp, vp]
+    L.rt_set_points.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp, u64, vp]
     L.rt_trace_batch.argtypes = [vp, f64, f64, i32, i32, C.POINTER(u64), u64, u64, vp, vp]
     L.rt_trace.argtypes = [vp, f64, f64, u64, u64, u64, u32, vp]
     L.rt_trace_records.argtypes = [vp, f64, f64, u64, u64, u64, u32, vp, vp]
@@ -210,6 +211,20 @@ class Grid:
         ka, kr, al = self._f32(k_abs, nz), self._f32(k_ray, nz), self._f32(sfc_albedo, nx * ny)
         self._check(self.L.rt_set_point(self.ctx, int(slot), _ptr(ka), _ptr(kr), float(cloud_ssa), float(cloud_g),
                                         _ptr(al), _stream(self.device)), "rt_set_point")
+
+    def set_points(self, first_slot, k_abs, k_ray, cloud_ssa, cloud_g, sfc_albedo):
+        """include/rt.h rt_set_points: len(cloud_ssa) consecutive slots in one call.  k_abs, k_ray: [n][nz];
+        sfc_albedo: ncol values (one albedo for all points) or [n][ncol]."""
+        nz, ny, nx = self.shape
+        n = len(cloud_ssa)
+        ka, kr = self._f32(k_abs, n * nz), self._f32(k_ray, n * nz)
+        al = torch.as_tensor(sfc_albedo)
+        shared = al.numel() == nx * ny
+        al = self._f32(al, nx * ny * (1 if shared else n))
+        ssa = (C.c_float * n)(*[float(x) for x in cloud_ssa])
+        cg = (C.c_float * n)(*[float(x) for x in cloud_g])
+        self._check(self.L.rt_set_points(self.ctx, int(first_slot), n, _ptr(ka), _ptr(kr), ssa, cg, _ptr(al),
+                                         0 if shared else nx * ny, _stream(self.device)), "rt_set_points")
 
     def trace_batch(self, zenith_deg, azimuth_deg, counts, first_photon_id=0, seed=1, records=False, first_point=0):
         """One launch for the spectral points first_point .. first_point + len(counts) - 1 (slot = stream id =

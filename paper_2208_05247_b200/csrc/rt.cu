@@ -2,6 +2,7 @@
 // Host logic only: argument checks, device memory, launches.  No step of the method runs on the CPU.
 #include "../../include/rt.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
@@ -28,6 +29,15 @@ struct rt_ctx {
   float* cloud_min = nullptr;
   float2* point_par = nullptr;            // rt_set_point: (cloud_ssa, cloud_g) per slot
   bool cloud_ok = false;
+  // voxel-sized cells + merging with the optics kept factored ("fly"): no majorant table per point;
+  // per cloud field the extrema per block of merged cells and level ([block][mz]), per point one word per block and
+  // the gas sums per level
+  float* blk_max = nullptr;
+  float* blk_min = nullptr;
+  float* blk_tab = nullptr;               // [slot][block]: -(block maximum) if merged, else +maximum
+  float* gas_sum = nullptr;               // [slot][nz]: fl(k_abs + k_ray)
+  size_t blk_cap = 0;                     // floats blk_max / blk_min were allocated for
+  int khat_slots = 1;                     // slots the majorant array currently holds (grown on demand, like optics)
   float* gas_tab = nullptr;               // rt_set_optics_factored: per slot k_abs[nz] then k_ray[nz] (device)
   unsigned batch_calls = 0;
   unsigned long long* batch_tab = nullptr; // device: offsets (n_slots + 1) then nfull (n_slots), for rt_trace_batch
@@ -117,6 +127,11 @@ const float* stage_input(rt_ctx* c, const float* p, size_t n, size_t slot_offset
   return dst;
 }
 
+bool fly_mode(const rt_ctx* c) {          // rt_set_cloud / rt_set_point without majorant tables
+  return c->bx == 1 && c->by == 1 && c->bz == 1 && c->mx * c->my * c->mz > 1;
+}
+size_t n_blocks(const rt_ctx* c) { return c->ncell / ((size_t)c->mx * c->my * c->mz); }
+
 // One source, 16 instantiations: <records, power-of-two wrap, weighted, batch>.
 const void* pick_kernel(int variant) {
   switch (variant) {
@@ -198,6 +213,12 @@ int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photon
   A.n_points = n_points; A.first_point = first_point; A.offsets = tab; A.nfull = tab ? tab + c->n_slots + 1 : nullptr;
   A.nvox32 = (unsigned)c->nvox; A.ncell32 = (unsigned)c->ncell; A.ncol32 = (unsigned)c->ncol;
   A.cloud = factored_trace ? c->cloud : nullptr; A.gas = c->gas_tab; A.point_par = c->point_par;
+  A.fly = (factored_trace && fly_mode(c)) ? 1 : 0;
+  if (A.fly) A.move_steps = rt::kMoveStepsFly;
+  A.btab = c->blk_tab; A.gsum = c->gas_sum;
+  auto log2i = [](int v) { int l = 0; while ((1 << l) < v) ++l; return l; };
+  A.lmx = log2i(c->mx); A.lmy = log2i(c->my); A.lmz = log2i(c->mz);
+  A.nbx = c->ncx / c->mx; A.nby = c->ncy / c->my; A.nblk32 = (unsigned)n_blocks(c);
   RT_CUDA(c, cudaEventRecord(c->ev0, st));
   // one launch per 2^31 photons at most (the kernel counts a block's finished photons in 32-bit words); the parts
   // are consecutive index ranges of the same job, so photons and tallies do not depend on the split
@@ -264,6 +285,19 @@ namespace {
 
 // The packed-optics array holds one slot until a packed slot > 0 is asked for; then it is grown to all n_slots
 // (16 B per voxel and slot), keeping what it holds.
+int ensure_khat_slots(rt_ctx* c, int slot) {
+  if (slot < c->khat_slots) return RT_OK;
+  DeviceGuard guard(c->device);
+  if (int rcw = wait_pending(c)) return rcw;
+  float* grown = nullptr;
+  RT_CUDA(c, cudaMalloc(&grown, (size_t)c->n_slots * c->ncell * sizeof(float)));
+  RT_CUDA(c, cudaMemcpy(grown, c->khat, (size_t)c->khat_slots * c->ncell * sizeof(float), cudaMemcpyDeviceToDevice));
+  cudaFree(c->khat);
+  c->khat = grown;
+  c->khat_slots = c->n_slots;
+  return RT_OK;
+}
+
 int ensure_optics_slots(rt_ctx* c, int slot) {
   if (slot < c->optics_slots) return RT_OK;
   DeviceGuard guard(c->device);
@@ -285,6 +319,7 @@ int set_optics_impl(rt_ctx* c, int slot, const float* k_ext, const float* k_ext_
   if (!k_ext || !k_ext_cloud || !ssa || !g || !sfc_albedo) return fail(c, RT_EINVAL, "rt_set_optics: NULL field");
   DeviceGuard guard(c->device);
   if (int rce = ensure_optics_slots(c, slot)) return rce;
+  if (int rce = ensure_khat_slots(c, slot)) return rce;
   c->slot_ok[slot] = 0;
   if (slot == 0) c->have_optics = false;
   int rc = RT_OK;
@@ -366,13 +401,15 @@ int rt_set_slots(rt_ctx* c, int n_slots) {
   DeviceGuard guard(c->device);
   if (int rcw = wait_pending(c)) return rcw;
   cudaFree(c->optics); cudaFree(c->khat); cudaFree(c->albedo); cudaFree(c->batch_tab); cudaFree(c->gas_tab); cudaFree(c->point_par); cudaFree(c->bad);
+  cudaFree(c->blk_tab); cudaFree(c->gas_sum); c->blk_tab = nullptr; c->gas_sum = nullptr;
   c->optics = nullptr; c->khat = nullptr; c->albedo = nullptr; c->batch_tab = nullptr; c->gas_tab = nullptr; c->point_par = nullptr; c->bad = nullptr;
   c->have_optics = false;
   c->n_slots = n_slots;
   c->slot_ok.assign((size_t)n_slots, 0);
   RT_CUDA(c, cudaMalloc(&c->optics, c->nvox * sizeof(float4)));   // one slot; grown when a packed slot > 0 is set
   c->optics_slots = 1;
-  RT_CUDA(c, cudaMalloc(&c->khat, (size_t)n_slots * c->ncell * sizeof(float)));
+  RT_CUDA(c, cudaMalloc(&c->khat, c->ncell * sizeof(float)));     // one slot; grown when a slot > 0 needs a table
+  c->khat_slots = 1;
   RT_CUDA(c, cudaMalloc(&c->albedo, (size_t)n_slots * c->ncol * sizeof(float)));
   RT_CUDA(c, cudaMalloc(&c->batch_tab, 2 * (2 * (size_t)n_slots + 1) * sizeof(unsigned long long)));   // two launches may be in flight
   RT_CUDA(c, cudaMalloc(&c->bad, ((size_t)n_slots + 1) * sizeof(int)));
@@ -408,6 +445,7 @@ int rt_set_optics_factored(rt_ctx* c, int slot, const float* k_cloud, const floa
     }
   }
   if (int rce = ensure_optics_slots(c, slot)) return rce;
+  if (int rce = ensure_khat_slots(c, slot)) return rce;
   c->slot_ok[slot] = 0;
   if (slot == 0) c->have_optics = false;
   if (!c->gas_tab) RT_CUDA(c, cudaMalloc(&c->gas_tab, (size_t)c->n_slots * 2 * c->nz * sizeof(float)));
@@ -444,13 +482,29 @@ int rt_set_cloud(rt_ctx* c, const float* k_cloud, void* cuda_stream) {
   c->cloud_ok = false;
   for (auto& ok : c->slot_ok) if (ok == 2) ok = 0;      // points built on the old cloud field
   if (!c->cloud) RT_CUDA(c, cudaMalloc(&c->cloud, c->nvox * sizeof(float)));
-  if (!c->cloud_max) RT_CUDA(c, cudaMalloc(&c->cloud_max, c->ncell * c->bz * sizeof(float)));
-  if (!c->cloud_min) RT_CUDA(c, cudaMalloc(&c->cloud_min, c->ncell * c->bz * sizeof(float)));
+  const bool fly = fly_mode(c);
+  if (fly) {
+    const size_t need = n_blocks(c) * c->mz;                // sized by the merge factors
+    if (need > c->blk_cap) {
+      if (int rcw = wait_pending(c)) return rcw;
+      cudaFree(c->blk_max); cudaFree(c->blk_min); c->blk_max = c->blk_min = nullptr; c->blk_cap = 0;
+      RT_CUDA(c, cudaMalloc(&c->blk_max, need * sizeof(float)));
+      RT_CUDA(c, cudaMalloc(&c->blk_min, need * sizeof(float)));
+      c->blk_cap = need;
+    }
+  } else {
+    if (!c->cloud_max) RT_CUDA(c, cudaMalloc(&c->cloud_max, c->ncell * c->bz * sizeof(float)));
+    if (!c->cloud_min) RT_CUDA(c, cudaMalloc(&c->cloud_min, c->ncell * c->bz * sizeof(float)));
+  }
   RT_CUDA(c, cudaMemcpyAsync(c->cloud, k_cloud, c->nvox * sizeof(float), cudaMemcpyDefault, st));
   int* cbad = c->bad + c->n_slots;        // the cloud field's own mask word: the slots' masks are not touched
   RT_CUDA(c, cudaMemsetAsync(cbad, 0, sizeof(int), st));
-  rt::cloud_levels_kernel<<<c->sm_count * 8, 256, 0, st>>>(c->cloud, c->cloud_max, c->cloud_min, c->nx, c->ny, c->nz,
-                                                           c->bx, c->by, c->bz, cbad);
+  if (fly)
+    rt::cloud_blocks_kernel<<<(unsigned)((n_blocks(c) * 32 + 127) / 128), 128, 0, st>>>(
+        c->cloud, c->blk_max, c->blk_min, c->nx, c->ny, c->nz, c->mx, c->my, c->mz, cbad);
+  else
+    rt::cloud_levels_kernel<<<c->sm_count * 8, 256, 0, st>>>(c->cloud, c->cloud_max, c->cloud_min, c->nx, c->ny, c->nz,
+                                                             c->bx, c->by, c->bz, cbad);
   ++c->launches;
   RT_CUDA(c, cudaGetLastError());
   if (int rcm = mark(c, st)) return rcm;
@@ -460,6 +514,69 @@ int rt_set_cloud(rt_ctx* c, const float* k_cloud, void* cuda_stream) {
   if (bad) return fail(c, RT_EOPTICS, "rt_set_cloud: the cloud extinction must be finite and >= 0");
   c->cloud_ok = true;
   return RT_OK;
+}
+
+// rt_set_point / rt_set_points on voxel-sized merged cells: the gas profiles, (cloud_ssa, cloud_g) and albedo of n
+// consecutive slots with a fixed number of copies and two kernels, whatever n is.
+static int set_points_fly(rt_ctx* c, int first, int n, const float* k_abs, const float* k_ray, const float* cloud_ssa,
+                          const float* cloud_g, const float* sfc_albedo, uint64_t albedo_stride, cudaStream_t st) {
+  const size_t nz = (size_t)c->nz, nblk = n_blocks(c);
+  if (!c->blk_tab) RT_CUDA(c, cudaMalloc(&c->blk_tab, (size_t)c->n_slots * nblk * sizeof(float)));
+  if (!c->gas_sum) RT_CUDA(c, cudaMalloc(&c->gas_sum, (size_t)c->n_slots * nz * sizeof(float)));
+  float* tab = c->gas_tab + (size_t)first * 2 * nz;
+  RT_CUDA(c, cudaMemcpy2DAsync(tab, 2 * nz * sizeof(float), k_abs, nz * sizeof(float), nz * sizeof(float), (size_t)n, cudaMemcpyDefault, st));
+  RT_CUDA(c, cudaMemcpy2DAsync(tab + nz, 2 * nz * sizeof(float), k_ray, nz * sizeof(float), nz * sizeof(float), (size_t)n, cudaMemcpyDefault, st));
+  std::vector<float2> pp((size_t)n);
+  for (int p = 0; p < n; ++p) pp[(size_t)p] = make_float2(cloud_ssa[p], cloud_g[p]);
+  RT_CUDA(c, cudaMemcpyAsync(c->point_par + first, pp.data(), (size_t)n * sizeof(float2), cudaMemcpyHostToDevice, st));   // pageable: staged before return
+  float* albedo = c->albedo + (size_t)first * c->ncol;
+  const bool broadcast = n > 1 && albedo_stride == 0;
+  if (broadcast || n == 1)
+    RT_CUDA(c, cudaMemcpyAsync(albedo, sfc_albedo, c->ncol * sizeof(float), cudaMemcpyDefault, st));
+  else
+    RT_CUDA(c, cudaMemcpy2DAsync(albedo, c->ncol * sizeof(float), sfc_albedo, albedo_stride * sizeof(float),
+                                 c->ncol * sizeof(float), (size_t)n, cudaMemcpyDefault, st));
+  RT_CUDA(c, cudaMemsetAsync(c->bad + first, 0, (size_t)n * sizeof(int), st));
+  const unsigned gx = (unsigned)std::min<size_t>((nblk + 255) / 256, (size_t)c->sm_count * 2);
+  rt::point_blocks_kernel<<<dim3(gx, (unsigned)n), 256, 0, st>>>(c->blk_max, c->blk_min, tab, c->gas_sum + (size_t)first * nz,
+                                                                 c->blk_tab + (size_t)first * nblk, c->ncx / c->mx,
+                                                                 c->ncy / c->my, c->ncz / c->mz, c->mz, c->nz,
+                                                                 c->merge_ratio, c->bad + first);
+  const unsigned ga = (unsigned)std::min<size_t>((c->ncol + 255) / 256, (size_t)c->sm_count * 2);
+  rt::albedo_points_kernel<<<dim3(ga, (unsigned)n), 256, 0, st>>>(albedo, c->ncol, broadcast ? 1 : 0, c->bad + first);
+  c->launches += 2;
+  RT_CUDA(c, cudaGetLastError());
+  for (int p = 0; p < n; ++p) c->slot_ok[(size_t)(first + p)] = 2;
+  return mark(c, st);
+}
+
+int rt_set_points(rt_ctx* c, int first_slot, int n_points, const float* k_abs, const float* k_ray,
+                  const float* cloud_ssa, const float* cloud_g, const float* sfc_albedo, uint64_t albedo_stride,
+                  void* cuda_stream) {
+  if (!c) return RT_EINVAL;
+  if (first_slot < 0 || n_points < 1 || first_slot + n_points > c->n_slots)
+    return fail(c, RT_EINVAL, "rt_set_points: slots out of range (rt_set_slots)");
+  if (!k_abs || !k_ray || !cloud_ssa || !cloud_g || !sfc_albedo) return fail(c, RT_EINVAL, "rt_set_points: NULL argument");
+  if (albedo_stride != 0 && albedo_stride < c->ncol) return fail(c, RT_EINVAL, "rt_set_points: albedo_stride must be 0 (one albedo for all points) or >= ncol");
+  if (!c->batch_tab) return fail(c, RT_ESTATE, "rt_set_points: call rt_set_slots first");
+  if (!c->cloud_ok) return fail(c, RT_ESTATE, "rt_set_points: call rt_set_cloud first");
+  for (int p = 0; p < n_points; ++p)
+    if (!(cloud_ssa[p] >= 0.0f && cloud_ssa[p] <= 1.0f) || !(std::fabs(cloud_g[p]) < 1.0f))
+      return fail(c, RT_EOPTICS, "rt_set_points: cloud_ssa must be in [0, 1] and |cloud_g| < 1");
+  if (!fly_mode(c)) {                      // cells of several voxels: a majorant table per point, point by point
+    for (int p = 0; p < n_points; ++p)
+      if (int rcp = rt_set_point(c, first_slot + p, k_abs + (size_t)p * c->nz, k_ray + (size_t)p * c->nz, cloud_ssa[p],
+                                 cloud_g[p], sfc_albedo + (size_t)p * albedo_stride, cuda_stream))
+        return rcp;
+    return RT_OK;
+  }
+  DeviceGuard guard(c->device);
+  for (int p = 0; p < n_points; ++p) c->slot_ok[(size_t)(first_slot + p)] = 0;
+  if (first_slot == 0) c->have_optics = false;
+  if (!c->gas_tab) RT_CUDA(c, cudaMalloc(&c->gas_tab, (size_t)c->n_slots * 2 * c->nz * sizeof(float)));
+  if (!c->point_par) RT_CUDA(c, cudaMalloc(&c->point_par, (size_t)c->n_slots * sizeof(float2)));
+  return set_points_fly(c, first_slot, n_points, k_abs, k_ray, cloud_ssa, cloud_g, sfc_albedo, albedo_stride,
+                        (cudaStream_t)cuda_stream);
 }
 
 int rt_set_point(rt_ctx* c, int slot, const float* k_abs, const float* k_ray, float cloud_ssa, float cloud_g,
@@ -477,17 +594,19 @@ int rt_set_point(rt_ctx* c, int slot, const float* k_abs, const float* k_ray, fl
   if (slot == 0) c->have_optics = false;  // slot 0's majorant and albedo no longer belong to rt_set_optics' packed record
   if (!c->gas_tab) RT_CUDA(c, cudaMalloc(&c->gas_tab, (size_t)c->n_slots * 2 * c->nz * sizeof(float)));
   if (!c->point_par) RT_CUDA(c, cudaMalloc(&c->point_par, (size_t)c->n_slots * sizeof(float2)));
+  if (fly_mode(c)) return set_points_fly(c, slot, 1, k_abs, k_ray, &cloud_ssa, &cloud_g, sfc_albedo, 0, st);
   float* tab = c->gas_tab + (size_t)slot * 2 * c->nz;
   const float2 pp = make_float2(cloud_ssa, cloud_g);
   RT_CUDA(c, cudaMemcpyAsync(tab, k_abs, c->nz * sizeof(float), cudaMemcpyDefault, st));
   RT_CUDA(c, cudaMemcpyAsync(tab + c->nz, k_ray, c->nz * sizeof(float), cudaMemcpyDefault, st));
   RT_CUDA(c, cudaMemcpyAsync(c->point_par + slot, &pp, sizeof pp, cudaMemcpyHostToDevice, st));   // pageable: staged before return
-  float* khat = c->khat + (size_t)slot * c->ncell;
   float* albedo = c->albedo + (size_t)slot * c->ncol;
   RT_CUDA(c, cudaMemcpyAsync(albedo, sfc_albedo, c->ncol * sizeof(float), cudaMemcpyDefault, st));
+  RT_CUDA(c, cudaMemsetAsync(c->bad + slot, 0, sizeof(int), st));
+  if (int rce = ensure_khat_slots(c, slot)) return rce;
+  float* khat = c->khat + (size_t)slot * c->ncell;
   const bool merging = c->mx * c->my * c->mz > 1;
   if (merging && !c->kmin) RT_CUDA(c, cudaMalloc(&c->kmin, c->ncell * sizeof(float)));
-  RT_CUDA(c, cudaMemsetAsync(c->bad + slot, 0, sizeof(int), st));
   rt::point_majorant_kernel<<<c->sm_count * 8, 256, 0, st>>>(c->cloud_max, c->cloud_min, tab, tab + c->nz, khat,
                                                              merging ? c->kmin : nullptr, c->ncx, c->ncy, c->ncz, c->bz, c->bad + slot);
   rt::check_albedo_kernel<<<c->sm_count, 256, 0, st>>>(albedo, c->ncol, c->bad + slot);
@@ -639,6 +758,12 @@ int rt_set_merge(rt_ctx* c, int mx, int my, int mz, float merge_ratio) {
   c->mx = mx; c->my = my; c->mz = mz; c->merge_ratio = merge_ratio;
   c->have_optics = false;                 // every majorant table was built for the old factors: all slots
   for (auto& ok : c->slot_ok) ok = 0;     // must be given optics again (RT_ESTATE otherwise)
+  c->cloud_ok = false;                    // ... and the cloud field's block tables (rt_set_cloud) too
+  if (c->blk_tab) {
+    DeviceGuard guard(c->device);
+    if (int rcw = wait_pending(c)) return rcw;
+    cudaFree(c->blk_tab); c->blk_tab = nullptr;
+  }
   return RT_OK;
 }
 
@@ -699,6 +824,8 @@ int rt_reset_tallies(rt_ctx* c, void* cuda_stream) {
 
 int rt_read_majorant(rt_ctx* c, float* khat_out) {
   if (!c || !khat_out) return RT_EINVAL;
+  if (c->slot_ok[0] == 2 && fly_mode(c))
+    return fail(c, RT_ESTATE, "rt_read_majorant: rt_set_point keeps no majorant table for voxel-sized merged cells");
   DeviceGuard guard(c->device);
   if (int rcw = wait_pending(c)) return rcw;
   RT_CUDA(c, cudaMemcpyAsync(khat_out, c->khat, c->ncell * sizeof(float), cudaMemcpyDefault, c->copy_stream));
@@ -770,6 +897,7 @@ void rt_destroy(rt_ctx* c) {
     cudaFree(c->optics); cudaFree(c->khat); cudaFree(c->kmin); cudaFree(c->atm_dir); cudaFree(c->albedo); cudaFree(c->tallies);
     cudaFree(c->counters); cudaFree(c->d_counters); cudaFree(c->bad); cudaFree(c->gas_tab); cudaFree(c->point_par);
     cudaFree(c->cloud); cudaFree(c->cloud_max); cudaFree(c->cloud_min); cudaFree(c->batch_tab); cudaFree(c->sink); cudaFree(c->stage);
+    cudaFree(c->blk_max); cudaFree(c->blk_min); cudaFree(c->blk_tab); cudaFree(c->gas_sum);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
     for (auto& p : c->pending) cudaEventDestroy(p.second);

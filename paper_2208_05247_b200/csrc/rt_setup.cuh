@@ -273,6 +273,82 @@ __global__ void point_majorant_kernel(const float* __restrict__ cmax, const floa
   }
 }
 
+// Voxel-sized cells with the optics kept factored: no majorant table per spectral point at all.  The level-0 majorant of
+// a voxel is fl((k_abs[z] + k_ray[z]) + k_cloud), which MOVE computes from the shared cloud field; what remains per
+// point is one word per BLOCK of mx x my x mz cells: -(block maximum) if the block is merged (§3.5b), else +maximum.
+// cloud_blocks_kernel (once per cloud field): per block and per level inside it, the extrema of the cloud extinction
+// ([block][mz * bz] floats); one warp per block.
+__global__ void cloud_blocks_kernel(const float* __restrict__ k_cloud, float* __restrict__ bmax, float* __restrict__ bmin,
+                                    int nx, int ny, int nz, int sx, int sy, int sz, int* __restrict__ bad) {
+  const int nbx = nx / sx, nby = ny / sy, nbz = nz / sz;
+  const size_t nblk = (size_t)nbx * nby * nbz;
+  const size_t b = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (b >= nblk) return;
+  const unsigned lane = threadIdx.x & 31u;
+  const int X = (int)(b % nbx), Y = (int)((b / nbx) % nby), Z = (int)(b / ((size_t)nbx * nby));
+  bool ok = true;
+  for (int lz = 0; lz < sz; ++lz) {
+    float hi = 0.0f, lo = INFINITY;
+    for (int k = (int)lane; k < sx * sy; k += 32) {
+      const int x = X * sx + k % sx, y = Y * sy + k / sx, z = Z * sz + lz;
+      const float v = k_cloud[((size_t)z * ny + y) * nx + x];
+      if (!(v >= 0.0f) || isinf(v)) ok = false;
+      hi = fmaxf(hi, v); lo = fminf(lo, v);
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+      hi = fmaxf(hi, __shfl_xor_sync(0xffffffffu, hi, off));
+      lo = fminf(lo, __shfl_xor_sync(0xffffffffu, lo, off));
+    }
+    if (lane == 0) { bmax[b * sz + lz] = hi; bmin[b * sz + lz] = lo; }
+  }
+  if (!ok) atomicOr(bad, 2);
+}
+
+// point_blocks_kernel (blockIdx.y = spectral point p of the call): gsum[p][z] = fl(k_abs[z] + k_ray[z]) and the block
+// words of the point.  fl(gsum + k_cloud) is monotone in k_cloud, so the block's extrema of k_ext follow exactly from
+// the cloud extrema per level.  gas: the points' profiles as rt.cu keeps them (per point k_abs[nz] then k_ray[nz]).
+__global__ void point_blocks_kernel(const float* __restrict__ bmax, const float* __restrict__ bmin,
+                                    const float* __restrict__ gas, float* __restrict__ gsum, float* __restrict__ btab,
+                                    int nbx, int nby, int nbz, int sz, int nz, float merge_ratio, int* __restrict__ bad) {
+  const size_t nblk = (size_t)nbx * nby * nbz;
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  const size_t pt = blockIdx.y;
+  const float* k_abs = gas + pt * 2 * (size_t)nz;
+  const float* k_ray = k_abs + nz;
+  gsum += pt * (size_t)nz; btab += pt * nblk; bad += pt;
+  for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < (size_t)nz; t += stride) {
+    const float ka = __ldg(k_abs + t), kr = __ldg(k_ray + t);
+    const float kg = ka + kr;
+    if (!(ka >= 0.0f) || !(kr >= 0.0f) || isinf(kg)) atomicOr(bad, 1);
+    gsum[t] = kg;
+  }
+  for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < nblk; t += stride) {
+    const int Z = (int)(t / ((size_t)nbx * nby));
+    float hi = 0.0f, lo = INFINITY;
+    for (int lz = 0; lz < sz; ++lz) {
+      const float kg = __ldg(k_abs + Z * sz + lz) + __ldg(k_ray + Z * sz + lz);
+      hi = fmaxf(hi, kg + bmax[t * sz + lz]);
+      lo = fminf(lo, kg + bmin[t * sz + lz]);
+    }
+    btab[t] = (hi <= merge_ratio * lo) ? -hi : hi;
+  }
+}
+
+// Albedo slots of several points at once (blockIdx.y = point of the call): range check into the point's mask word;
+// broadcast != 0: every point takes the first slot's albedo (already copied there).
+__global__ void albedo_points_kernel(float* __restrict__ albedo, size_t ncol, int broadcast, int* __restrict__ bad) {
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  const size_t pt = blockIdx.y;
+  bool ok = true;
+  for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < ncol; c += stride) {
+    const float a = broadcast ? albedo[c] : albedo[pt * ncol + c];
+    if (broadcast && pt > 0) albedo[pt * ncol + c] = a;
+    if (!(a >= 0.0f) || !(a <= 1.0f)) ok = false;
+  }
+  if (!ok) atomicOr(bad + pt, 16);
+}
+
 // §3.5b merged cells.  One WARP per block of mx x my x mz acceleration cells (lanes stride over the block's
 // cells, x fastest): if the block's highest extinction is at most merge_ratio times its lowest (one fp32
 // multiply), every cell of the block stores -(block maximum); the sign bit is what the trace kernel tests

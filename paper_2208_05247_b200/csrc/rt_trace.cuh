@@ -39,6 +39,7 @@ constexpr int kScatterBatch = 8;       // SCATTER
 constexpr int kCollideBatch = 8, kCollideBatchUnit = 12;   // COLLIDE: cells of several voxels / voxel-sized cells
 constexpr int kBoundaryBatch = 8;      // BOUNDARY: surface and domain-top arrivals (1 per photon)
 constexpr int kMoveSteps = 3, kMoveStepsUnit = 4;           // MOVE steps between two votes
+constexpr int kMoveStepsFly = 6;       // ... in a sweep over spectral points kept factored (8 crossings per collision)
 constexpr unsigned vote_bias(int collide_batch) {
   return (32u - kRegenBatch) | ((32u - 1u) << 6) | ((32u - (unsigned)collide_batch) << 12) |
          ((32u - kScatterBatch) << 18) | ((32u - kBoundaryBatch) << 24);
@@ -85,6 +86,14 @@ struct TraceArgs {
   const float* cloud;                  // [z][y][x] or nullptr (then the packed slots are used)
   const float* gas;                    // per point: k_abs[nz] then k_ray[nz]
   const float2* point_par;             // per point: (cloud_ssa, cloud_g)
+  // ... with voxel-sized cells and merging (fly): no majorant table per point.  A voxel's majorant is its own
+  // fl((k_abs[z] + k_ray[z]) + k_cloud), read from the shared cloud field; per point only one word per block of
+  // merged cells (sign bit set: merged, |word| = the block's maximum) and the gas sums per level
+  int fly;
+  const float* btab;                   // [point][block]
+  const float* gsum;                   // [point][nz]
+  int lmx, lmy, lmz, nbx, nby;         // log2 of the merge factors, blocks per row / column
+  unsigned nblk32;                     // slot stride of btab
   float diffuse_fraction;              // §3.15: share of photons launched diffusely (0: none)
   int sobol;                           // §3.15: entry points from the scrambled 2-D Sobol sequence
   uint32_t stream_id;
@@ -185,6 +194,22 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
     const unsigned c = ((unsigned)cz * (unsigned)A.ncy + (unsigned)cy) * (unsigned)A.ncx + (unsigned)cx;
     return kBatch ? c + jpt * A.ncell32 : c;
   };
+  // the majorant table's word for the cell (cx, cy, cz): the table itself, or (fly) the block's word if the block is
+  // merged, else the voxel's own extinction.  Both loads are issued at once; the indices are valid either way.
+  auto voxel_word = [&]() {
+    const unsigned vox = ((unsigned)cz * (unsigned)A.ny + (unsigned)cy) * (unsigned)A.nx + (unsigned)cx;
+    return __ldg(A.gsum + jpt * (unsigned)A.nz + (unsigned)cz) + __ldg(A.cloud + vox);
+  };
+  auto word_at = [&]() {
+    if (kBatch && A.fly) {
+      const unsigned blk = ((unsigned)(cz >> A.lmz) * (unsigned)A.nby + (unsigned)(cy >> A.lmy)) * (unsigned)A.nbx +
+                           (unsigned)(cx >> A.lmx);
+      const float B = __ldg(A.btab + jpt * A.nblk32 + blk);
+      const float k0 = voxel_word();   // (loading it only when the block is not merged was slower: 56.5 against 54.1 ms)
+      return (__float_as_int(B) < 0) ? B : k0;
+    }
+    return __ldg(A.khat + cell_of());
+  };
   // §3.14 roulette: below W0/2 survive with probability wq / W0 exactly (32-bit word of the Philox block at
   // counter e | 2^31 against wq) and continue with W0, else end; both branches go to the ledger
   int fate = 0;
@@ -258,7 +283,7 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
       else { const int k = min(A.my - 1, (int)(ry / dely)); ry = fmaxf(0.0f, fmaf(-(float)k, dely, ry)); cy += py ? A.my - 1 - k : k; }
       if (ax == 2) { rz = delz; if (!pz) cz += A.mz - 1; }
       else { const int k = min(A.mz - 1, (int)(rz / delz)); rz = fmaxf(0.0f, fmaf(-(float)k, delz, rz)); cz += pz ? A.mz - 1 - k : k; }
-      kh = __ldg(A.khat + cell_of());             // the single cell's own majorant (sign bit clear)
+      kh = (kBatch && A.fly) ? voxel_word() : __ldg(A.khat + cell_of());   // the single cell's own majorant (sign bit clear)
       set_steps(false);
     }
     ++t_relevel;
@@ -342,7 +367,7 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
         cx = ix / A.bx; cy = iy / A.by; cz = A.ncz - 1;
         da = A.sun_x; db = A.sun_y; dc = A.sun_z;
         // §3.5b: the sign bit of the stored majorant marks the cells of a merged cell
-        kh = __ldg(A.khat + cell_of());
+        kh = word_at();
         const bool lev = __float_as_int(kh) < 0;
         set_steps(lev);
         int wx = A.bx, wy = A.by;             // cell extent in voxels at this level
@@ -418,7 +443,7 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
           if (ax2) cz += sz;
           if ((unsigned)cz >= (unsigned)A.ncz) st = ST_BOUNDARY;   // surface (cz < 0) or domain top
           else {
-            const float raw = __ldg(A.khat + cell_of());
+            const float raw = word_at();
             const bool other = (__float_as_int(raw) ^ __float_as_int(kh)) < 0;   // §3.7b: the entered cell is at the other level
             kh = raw;
             if (other) relevel(ax0 ? 0 : (ax1 ? 1 : 2));
@@ -599,9 +624,8 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
       }
     }
     // With voxel-sized cells nearly every collision is a scattering, so SCATTER runs right behind COLLIDE without
-    // another vote: a jump back to the ONE copy of the phase (a second inlined copy costs more than the vote, and so
-    // does the same jump in the batch instantiations, which trace 2^3-voxel cells: 79.6 against 76.7 ms on config 4).
-    if (!kBatch && A.unit && phase == ST_COLLIDE) goto scatter;
+    // another vote: a jump back to the ONE copy of the phase (a second inlined copy costs more than the vote).
+    if (A.unit && phase == ST_COLLIDE) goto scatter;
   }
 
   flush_thread_counters();

@@ -58,7 +58,7 @@ CONFIGS = {
     3: Config("cumulus_512x512x128", 512, 512, 128, 50.0, 50.0, 25.0, 60.0, 120.0, 1 << 26, 0.2,
               n_blobs=600, block=(1, 1, 1), merge=(8, 8, 8)),
     4: Config("spectral_512x512x128", 512, 512, 128, 50.0, 50.0, 25.0, 60.0, 120.0, 1 << 26, 0.2,
-              n_blobs=600, block=(2, 2, 2), merge=(8, 8, 4)),
+              n_blobs=600, block=(1, 1, 1), merge=(8, 8, 8)),
     5: Config("convergence_1024x1024x192", 1024, 1024, 192, 25.0, 25.0, 20.0, 50.0, 0.0, 1 << 28, 0.15,
               n_blobs=2400, block=(1, 1, 1), merge=(8, 8, 8)),
 }

@@ -256,6 +256,9 @@ def test_factored_optics_slots():
     for k, f in enumerate(facs):
         g2.set_point(k, f["k_abs"], f["k_ray"], f["cloud_ssa"], f["cloud_g"], f["sfc_albedo"])
     assert np.array_equal(g2.read_majorant().numpy().view(np.uint32), kh.view(np.uint32))
+    # rt_set_points on cells of several voxels = the same calls point by point (slots 1, 2 set again that way)
+    g2.set_points(1, np.stack([f["k_abs"] for f in facs[1:]]), np.stack([f["k_ray"] for f in facs[1:]]),
+                  [f["cloud_ssa"] for f in facs[1:]], [f["cloud_g"] for f in facs[1:]], al_dev)
     for weighted in (False, True):
         g.reset_tallies(); g2.reset_tallies()
         g.set_mode(weighted); g2.set_mode(weighted)
@@ -273,4 +276,90 @@ def test_factored_optics_slots():
         g.set_optics_factored(0, kc_dev, facs[0]["k_abs"], facs[0]["k_ray"], 1.5, 0.8, al_dev)
     with pytest.raises(rt.RtError):
         g.set_optics_factored(0, facs[0]["k_cloud"], facs[0]["k_abs"], facs[0]["k_ray"], 0.9, 0.8, al_dev)   # host field
+    g.close()
+
+
+@pytest.mark.parametrize("merge", [(8, 8, 8), (4, 2, 16)])
+def test_points_on_voxel_sized_cells_keep_no_majorant_table(merge):
+    """rt_set_cloud + rt_set_point on voxel-sized cells with merging: the library builds no majorant
+    table per point; MOVE takes a voxel's majorant from the shared cloud field and the point's gas sums, and one word
+    per block of merged cells says whether the block is merged.  Every photon must equal the oracle's on the fields
+    assembled from the same factors (oracle: its own majorant table of voxel-sized cells), in both modes, with ragged
+    counts; and a changed merge setting must ask for the cloud field again."""
+    rt = _rt()
+    from dataclasses import replace
+    from rt_inputs import factored_point
+    cfg = replace(CONFIGS[2], block=(1, 1, 1), merge=merge)
+    pts = spectral_points(112)
+    sel = (0, 58, 111, 30)
+    facs = [factored_point(cfg, pts[j]) for j in sel]
+    for k, f in enumerate(facs):                            # a different albedo per point
+        f["sfc_albedo"] = np.clip(f["sfc_albedo"] * np.float32(0.5 + 0.25 * k), 0.0, 1.0).astype(np.float32)
+    fields = []
+    for f in facs:
+        asm = O.assemble_factored(f["k_cloud"], f["k_abs"], f["k_ray"], f["cloud_ssa"], f["cloud_g"])
+        asm["sfc_albedo"] = f["sfc_albedo"]
+        fields.append(asm)
+    g = rt.Grid(*cfg.grid, device=0, **cfg.accel)
+    g.set_slots(len(sel))
+    g.set_cloud(torch.from_numpy(facs[0]["k_cloud"]).cuda())
+    for k, f in enumerate(facs):
+        g.set_point(k, f["k_abs"], f["k_ray"], f["cloud_ssa"], f["cloud_g"], f["sfc_albedo"])
+    with pytest.raises(rt.RtError):
+        g.read_majorant()                                   # there is none in this mode
+    counts = [cfg.ncol + 99, 4000, cfg.ncol * 2, 0]
+    for weighted in (False, True):
+        g.reset_tallies()
+        g.set_mode(weighted)
+        rec = g.trace_batch(cfg.zenith_deg, cfg.azimuth_deg, counts, seed=cfg.seed, records=True).cpu().numpy().view(np.uint32)
+        t = g.read_tallies()
+        total = O.Tallies(cfg.nx, cfg.ny, cfg.nz)
+        off = 0
+        for k, (opt, n) in enumerate(zip(fields, counts)):
+            if n == 0:
+                continue
+            _, rec32, _ = O.trace(cfg.grid, opt, cfg.zenith_deg, cfg.azimuth_deg, n, seed=cfg.seed, stream_id=k,
+                                  precision=32, records=True, n_threads=8, tallies=total, weighted=weighted, **cfg.accel)
+            assert np.array_equal(rec[off:off + n], rec32), (k, weighted)
+            off += n
+        for name in TALLIES:
+            assert np.array_equal(getattr(t, name).numpy(), getattr(total, name)), (name, weighted)
+        assert t.counters.asdict() == total.counters.asdict() and t.closure() == sum(counts) * rt.W0
+        assert t.counters.n_relevel > 0                     # both levels were in use
+    # rt_set_points: the same slots in ONE call trace the same photons (weighted mode is still on), with one albedo
+    # per point and with one albedo for all points
+    g3 = rt.Grid(*cfg.grid, device=0, **cfg.accel)
+    g3.set_slots(len(sel))
+    g3.set_mode(True)
+    g3.set_cloud(facs[0]["k_cloud"])
+    ka, kr = np.stack([f["k_abs"] for f in facs]), np.stack([f["k_ray"] for f in facs])
+    ssa, cg = [f["cloud_ssa"] for f in facs], [f["cloud_g"] for f in facs]
+    g3.set_points(0, ka, kr, ssa, cg, torch.from_numpy(np.stack([f["sfc_albedo"] for f in facs])).cuda())
+    rec3 = g3.trace_batch(cfg.zenith_deg, cfg.azimuth_deg, counts, seed=cfg.seed, records=True).cpu().numpy().view(np.uint32)
+    assert np.array_equal(rec3, rec)
+    t3 = g3.read_tallies()
+    for name in TALLIES:
+        assert torch.equal(getattr(t3, name), getattr(t, name)), name
+    g3.reset_tallies(); g.reset_tallies()
+    g3.set_points(1, ka[1:], kr[1:], ssa[1:], cg[1:], facs[2]["sfc_albedo"])          # host albedo, shared; slots 1..3
+    for k in range(1, len(sel)):
+        f = facs[k]
+        g.set_point(k, f["k_abs"], f["k_ray"], f["cloud_ssa"], f["cloud_g"], facs[2]["sfc_albedo"])
+    ra = g.trace_batch(cfg.zenith_deg, cfg.azimuth_deg, counts, seed=cfg.seed, records=True)
+    rb = g3.trace_batch(cfg.zenith_deg, cfg.azimuth_deg, counts, seed=cfg.seed, records=True)
+    assert torch.equal(ra, rb) and not np.array_equal(rb.cpu().numpy().view(np.uint32), rec)
+    with pytest.raises(rt.RtError):
+        g3.set_points(2, ka, kr, ssa, cg, facs[0]["sfc_albedo"])                      # 4 points from slot 2 of 4
+    with pytest.raises(rt.RtError):
+        g3.set_points(0, ka, kr, [1.5] + ssa[1:], cg, facs[0]["sfc_albedo"])
+    g3.close()
+    # a bad cloud field is refused by rt_set_cloud in this mode too; new merge factors invalidate the cloud tables
+    bad = facs[0]["k_cloud"].copy()
+    bad[3, 4, 5] = -1.0
+    with pytest.raises(rt.RtError):
+        g.set_cloud(bad)
+    g.set_cloud(facs[0]["k_cloud"])
+    g.set_merge(2, 2, 2)
+    with pytest.raises(rt.RtError):
+        g.set_point(0, facs[0]["k_abs"], facs[0]["k_ray"], facs[0]["cloud_ssa"], facs[0]["cloud_g"], facs[0]["sfc_albedo"])
     g.close()
