@@ -275,6 +275,29 @@ uint64_t rt_launch_count(const rt_ctx* ctx);
 int rt_philox_words(int cuda_device, const uint32_t* ctr, uint32_t key0, uint32_t key1, uint32_t* out,
                     uint64_t n);
 
+/* The majorant table WITHOUT any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it).  Computes what rt_set_optics + rt_read_majorant give for the same
+ * extinction field (the maximum of the extinction over each acceleration cell, and the merged
+ * cells of §3.5b: every cell of a merged block holds -(block maximum)), bit for bit, with no context:
+ *   k_ext    DEVICE, [z][y][x], nx * ny * nz floats (the total extinction, i.e. c3 of §3.4), read only;
+ *   khat_out DEVICE, [cz][cy][cx], (nx/bx) * (ny/by) * (nz/bz) floats, written;
+ *   bad_out  DEVICE int or NULL: set to 0, then to 1 if a value of k_ext is negative, NaN or infinite (the table is
+ *            then unspecified); nothing is read back, so the call never waits for the GPU;
+ *   mx, my, mz, merge_ratio as rt_set_merge (1, 1, 1 = no merging); cuda_device, cuda_stream: where it runs.
+ * The per-cell minima the merge criterion needs are SCRATCH: they live in a file-scope device array of
+ * RT_NO_ALLOC_MAX_CELLS floats (4 MiB, held by every GPU that loads the library until the process exits), so the cell
+ * count must not exceed RT_NO_ALLOC_MAX_CELLS (RT_EINVAL, message via rt_no_alloc_last_error).  The call issues one
+ * memset (bad_out) and two kernels on the stream and calls no cudaMalloc, cudaFree or other allocating routine.  All
+ * calls on a device share that array: every call overwrites the part it reads before reading it (stale contents of an
+ * earlier call never matter), but two calls that OVERLAP on the GPU (different streams, no dependency) race on it
+ * and give wrong tables; put them on one stream or order them with events.
+ * Errors: RT_EINVAL (NULL pointer, sizes, factors not powers of two dividing the cell grid, too many cells),
+ * RT_ECUDA.  rt_no_alloc_last_error: the message of this thread's last failed rt_majorant_no_alloc call (never NULL). */
+#define RT_NO_ALLOC_MAX_CELLS (1u << 20)
+int rt_majorant_no_alloc(const float* k_ext, float* khat_out, int* bad_out, int nx, int ny, int nz, int bx, int by,
+                         int bz, int mx, int my, int mz, float merge_ratio, int cuda_device, void* cuda_stream);
+const char* rt_no_alloc_last_error(void);
+
 const char* rt_last_error(const rt_ctx* ctx); /* never NULL; valid until the next call on ctx */
 void rt_destroy(rt_ctx* ctx);                 /* frees all device memory; NULL is a no-op */
 

@@ -14,7 +14,7 @@ MODE_ANALOG, MODE_WEIGHTED = 0, 1
 
 EXPORTS = ("rt_create_grid", "rt_set_merge", "rt_set_mode", "rt_set_source", "rt_set_optics", "rt_set_slots", "rt_set_optics_slot", "rt_set_optics_factored", "rt_set_cloud", "rt_set_point", "rt_set_points", "rt_trace_batch", "rt_trace", "rt_trace_records", "rt_trace_range", "rt_read_tallies", "rt_read_tallies_async",
            "rt_reset_tallies", "rt_set_heating_split", "rt_read_heating_direct", "rt_tally_to_flux", "rt_read_majorant", "rt_read_packed_optics", "rt_gather_bench",
-           "rt_last_trace_ms", "rt_launch_count", "rt_philox_words", "rt_last_error", "rt_destroy")
+           "rt_last_trace_ms", "rt_launch_count", "rt_philox_words", "rt_majorant_no_alloc", "rt_no_alloc_last_error", "rt_last_error", "rt_destroy")
 
 COUNTER_FIELDS = ("n_photons", "n_events", "n_null", "n_rayleigh", "n_hg", "n_atm_abs", "n_sfc_hits",
                   "n_sfc_abs", "n_toa", "n_capped", "n_cell_steps", "n_relevel", "n_roulette_killed", "n_roulette_kept",
@@ -74,12 +74,15 @@ def lib():
     L.rt_launch_count.argtypes = [vp]
     L.rt_launch_count.restype = u64
     L.rt_philox_words.argtypes = [i32, vp, u32, u32, vp, u64]
+    L.rt_majorant_no_alloc.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, i32, i32, i32, i32, f32, i32, vp]
+    L.rt_no_alloc_last_error.argtypes = []
+    L.rt_no_alloc_last_error.restype = C.c_char_p
     L.rt_last_error.argtypes = [vp]
     L.rt_last_error.restype = C.c_char_p
     L.rt_destroy.argtypes = [vp]
     L.rt_destroy.restype = None
     for name in EXPORTS:
-        if name not in ("rt_launch_count", "rt_last_error", "rt_destroy"):
+        if name not in ("rt_launch_count", "rt_last_error", "rt_no_alloc_last_error", "rt_destroy"):
             getattr(L, name).restype = i32
     _lib = L
     return L
@@ -338,3 +341,28 @@ def philox_words(ctr, key, device=0):
     if rc != 0:
         raise RtError("rt_philox_words failed (%d)" % rc)
     return out
+
+
+NO_ALLOC_MAX_CELLS = 1 << 20
+
+
+def majorant_no_alloc(k_ext, khat_out, block=(1, 1, 1), merge=(1, 1, 1), merge_ratio=1.25, bad_out=None):
+    """include/rt.h rt_majorant_no_alloc: the majorant table of the DEVICE field k_ext [nz][ny][nx] (fp32, contiguous)
+    into the caller's DEVICE tensor khat_out, with the library allocating nothing (its scratch is a fixed device array
+    of NO_ALLOC_MAX_CELLS floats).  Asynchronous on the current stream; calls that overlap on the GPU race."""
+    for t in (k_ext, khat_out) + ((bad_out,) if bad_out is not None else ()):
+        if not (t.is_cuda and t.is_contiguous()):
+            raise RtError("rt_majorant_no_alloc takes contiguous device tensors")
+    if k_ext.dtype != torch.float32 or khat_out.dtype != torch.float32 or k_ext.dim() != 3:
+        raise RtError("rt_majorant_no_alloc: k_ext [nz][ny][nx] and khat_out must be fp32")
+    nz, ny, nx = k_ext.shape
+    bx, by, bz = block
+    if khat_out.numel() != (nx // bx) * (ny // by) * (nz // bz):
+        raise RtError("khat_out has %d elements, expected %d" % (khat_out.numel(), (nx // bx) * (ny // by) * (nz // bz)))
+    if bad_out is not None and (bad_out.dtype != torch.int32 or bad_out.numel() != 1):
+        raise RtError("bad_out must be one int32")
+    L = lib()
+    rc = L.rt_majorant_no_alloc(_ptr(k_ext), _ptr(khat_out), _ptr(bad_out), nx, ny, nz, bx, by, bz, int(merge[0]),
+                                int(merge[1]), int(merge[2]), float(merge_ratio), k_ext.device.index, _stream(k_ext.device))
+    if rc != 0:
+        raise RtError("rt_majorant_no_alloc failed (%d): %s" % (rc, L.rt_no_alloc_last_error().decode()))

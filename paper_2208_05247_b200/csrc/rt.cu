@@ -7,6 +7,7 @@
 #include <cstdint>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <utility>
 #include <vector>
@@ -904,6 +905,122 @@ void rt_destroy(rt_ctx* c) {
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
   }
   delete c;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------------------------
+// rt_majorant_no_alloc (include/rt.h): the majorant table of §3.5 + §3.5b for callers that must not allocate.
+// The scratch of the step (the per-cell minima of the merge criterion, which rt_set_optics keeps in a cudaMalloc'ed
+// array of the context) is this file-scope device array.  Device code names it directly; HOST code must not pass the
+// name to a kernel (on the host it is a stand-in, not a device address): the address is asked for once per device
+// with cudaGetSymbolAddress, below.
+static __device__ __align__(256) float g_no_alloc_cell_min[RT_NO_ALLOC_MAX_CELLS];
+
+namespace {
+
+// Variant of the cell-extrema step of the pack kernels for the extinction field alone: one thread per acceleration
+// cell; the cell's maximum goes to the caller's table, its minimum to the scratch array (every cell the merge step
+// reads is written here first, so what an earlier call left in the array never matters).
+__global__ void cell_extrema_no_alloc_kernel(const float* __restrict__ k_ext, float* __restrict__ khat, int nx, int ny,
+                                             int nz, int bx, int by, int bz, int* __restrict__ bad) {
+  const int ncx = nx / bx, ncy = ny / by, ncz = nz / bz;
+  const size_t ncell = (size_t)ncx * ncy * ncz;
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  bool ok = true;
+  for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < ncell; c += stride) {
+    const int cx = (int)(c % ncx), cy = (int)((c / ncx) % ncy), cz = (int)(c / ((size_t)ncx * ncy));
+    float hi = 0.0f, lo = INFINITY;
+    for (int z = cz * bz; z < (cz + 1) * bz; ++z)
+      for (int y = cy * by; y < (cy + 1) * by; ++y)
+        for (int x = cx * bx; x < (cx + 1) * bx; ++x) {
+          const float k = __ldg(k_ext + ((size_t)z * ny + y) * nx + x);
+          if (!(k >= 0.0f) || isinf(k)) ok = false;
+          hi = fmaxf(hi, k); lo = fminf(lo, k);
+        }
+    khat[c] = hi;
+    g_no_alloc_cell_min[c] = lo;
+  }
+  if (!ok && bad) atomicOr(bad, 1);
+}
+
+constexpr int kNoAllocMaxDevices = 64;
+float* g_no_alloc_ptr[kNoAllocMaxDevices] = {};   // device address of g_no_alloc_cell_min per device, once known
+int g_no_alloc_sms[kNoAllocMaxDevices] = {};
+std::mutex g_no_alloc_mutex;
+thread_local char g_no_alloc_err[256] = "";
+
+int no_alloc_fail(int code, const char* fmt, unsigned long long a = 0, unsigned long long b = 0) {
+  snprintf(g_no_alloc_err, sizeof g_no_alloc_err, fmt, a, b);
+  return code;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* rt_no_alloc_last_error(void) { return g_no_alloc_err; }
+
+int rt_majorant_no_alloc(const float* k_ext, float* khat_out, int* bad_out, int nx, int ny, int nz, int bx, int by,
+                         int bz, int mx, int my, int mz, float merge_ratio, int cuda_device, void* cuda_stream) {
+  if (!k_ext || !khat_out) return no_alloc_fail(RT_EINVAL, "rt_majorant_no_alloc: NULL field or table");
+  if (nx <= 0 || ny <= 0 || nz <= 0 || bx <= 0 || by <= 0 || bz <= 0 || nx % bx || ny % by || nz % bz)
+    return no_alloc_fail(RT_EINVAL, "rt_majorant_no_alloc: sizes must be positive and the block must divide the grid");
+  const int ncx = nx / bx, ncy = ny / by, ncz = nz / bz;
+  const unsigned long long ncell = (unsigned long long)ncx * ncy * ncz;
+  if (ncell > (unsigned long long)RT_NO_ALLOC_MAX_CELLS)
+    return no_alloc_fail(RT_EINVAL, "rt_majorant_no_alloc: %llu acceleration cells exceed RT_NO_ALLOC_MAX_CELLS = %llu "
+                         "(the scratch array is fixed; use rt_set_optics on a context)", ncell, RT_NO_ALLOC_MAX_CELLS);
+  auto pow2 = [](int v) { return v > 0 && !(v & (v - 1)); };
+  if (!pow2(mx) || !pow2(my) || !pow2(mz) || ncx % mx || ncy % my || ncz % mz || mx > 64 || my > 64 || mz > 64)
+    return no_alloc_fail(RT_EINVAL, "rt_majorant_no_alloc: merge factors must be powers of two <= 64 dividing the acceleration grid");
+  if (!(merge_ratio >= 1.0f) || !std::isfinite(merge_ratio))
+    return no_alloc_fail(RT_EINVAL, "rt_majorant_no_alloc: merge_ratio must be >= 1");
+  if (cuda_device < 0 || cuda_device >= kNoAllocMaxDevices)
+    return no_alloc_fail(RT_EINVAL, "rt_majorant_no_alloc: device %llu out of range", (unsigned long long)cuda_device);
+  DeviceGuard guard(cuda_device);
+  float* scratch = nullptr;
+  int sms = 0;
+  {
+    // set-up, once per device, with that device current: the DEVICE address of the scratch array
+    std::lock_guard<std::mutex> lock(g_no_alloc_mutex);
+    if (!g_no_alloc_ptr[cuda_device]) {
+      float* p = nullptr;
+      cudaError_t ce = cudaGetSymbolAddress((void**)&p, g_no_alloc_cell_min);
+      if (ce != cudaSuccess || !p) {
+        snprintf(g_no_alloc_err, sizeof g_no_alloc_err, "rt_majorant_no_alloc: cudaGetSymbolAddress: %s", cudaGetErrorString(ce));
+        return RT_ECUDA;
+      }
+      int n = 0;
+      ce = cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, cuda_device);
+      if (ce != cudaSuccess || n < 1) {
+        snprintf(g_no_alloc_err, sizeof g_no_alloc_err, "rt_majorant_no_alloc: cudaDeviceGetAttribute: %s", cudaGetErrorString(ce));
+        return RT_ECUDA;
+      }
+      g_no_alloc_sms[cuda_device] = n;
+      g_no_alloc_ptr[cuda_device] = p;
+    }
+    scratch = g_no_alloc_ptr[cuda_device];
+    sms = g_no_alloc_sms[cuda_device];
+  }
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaError_t ce = cudaSuccess;
+  if (bad_out) ce = cudaMemsetAsync(bad_out, 0, sizeof(int), st);
+  if (ce == cudaSuccess) {
+    const unsigned blocks = (unsigned)std::min<unsigned long long>((ncell + 255) / 256, (unsigned long long)sms * 8);
+    cell_extrema_no_alloc_kernel<<<blocks, 256, 0, st>>>(k_ext, khat_out, nx, ny, nz, bx, by, bz, bad_out);
+    if (mx * my * mz > 1) {
+      const unsigned long long nblk = ncell / ((unsigned long long)mx * my * mz);
+      rt::merge_cells_kernel<<<(unsigned)((nblk * 32 + 127) / 128), 128, 0, st>>>(khat_out, scratch, ncx, ncy, ncz, mx, my,
+                                                                                   mz, merge_ratio);
+    }
+    ce = cudaGetLastError();
+  }
+  if (ce != cudaSuccess) {
+    snprintf(g_no_alloc_err, sizeof g_no_alloc_err, "rt_majorant_no_alloc: %s", cudaGetErrorString(ce));
+    return RT_ECUDA;
+  }
+  return RT_OK;
 }
 
 }  // extern "C"
