@@ -115,9 +115,12 @@ int rt_trace_range(rt_ctx* ctx, double zenith_deg, double azimuth_deg, uint64_t 
 int rt_read_tallies(rt_ctx* ctx, int64_t* atm_abs, int64_t* sfc_dir, int64_t* sfc_dif, int64_t* sfc_abs,
                     int64_t* toa_up, rt_counters* counters);
 
-/* rt_read_tallies without the wait: the copies (and a one-thread kernel that assembles the counters) are queued
- * on `cuda_stream` after the work already queued there; the outputs are valid once the caller has synchronised
- * that stream.  HOST outputs should be pinned, or the copies serialise with the host.  Lets a caller upload the
+/* rt_read_tallies without the wait: copies only, queued on `cuda_stream` after the work already queued there (the
+ * counters go to pinned memory of the context as raw words and a host function queued on the stream,
+ * cudaLaunchHostFunc, fills *counters from them: `counters` must be a HOST pointer; no kernel is launched, because
+ * behind another context's persistent trace kernel a kernel of this stream would wait for that whole trace).  The
+ * outputs are valid once the caller has synchronised that stream; at most two read-outs of one context may be in
+ * flight.  HOST outputs should be pinned, or the copies serialise with the host.  Lets a caller upload the
  * next step's fields and download the last step's tallies while another context traces (bench.py's e2e leg). */
 int rt_read_tallies_async(rt_ctx* ctx, int64_t* atm_abs, int64_t* sfc_dir, int64_t* sfc_dif, int64_t* sfc_abs,
                           int64_t* toa_up, rt_counters* counters, void* cuda_stream);

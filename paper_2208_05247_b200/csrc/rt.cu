@@ -23,7 +23,11 @@ struct rt_ctx {
   float merge_ratio = 1.25f;
   int n_slots = 1;                        // rt_set_slots: optics / majorant / albedo slots (spectral points)
   std::vector<char> slot_ok = std::vector<char>(1, 0);
-  rt_counters* d_counters = nullptr;      // rt_read_tallies_async: counters assembled on the device
+  // rt_read_tallies_async: the raw counter words are copied to pinned host memory and a host function queued on the
+  // stream fills the caller's rt_counters from them (two buffers, used alternately: two read-outs may be in flight)
+  struct CounterJob { unsigned long long raw[rt::C_COUNT]; rt_counters* out; };
+  CounterJob* counter_jobs = nullptr;
+  unsigned counter_calls = 0;
   int optics_slots = 1;                   // slots the packed-optics array currently holds (grown on demand)
   float* cloud = nullptr;                 // rt_set_cloud: own copy of the cloud field, nvox
   float* cloud_max = nullptr;             // ... highest / lowest cloud extinction per cell and level-in-cell
@@ -90,6 +94,23 @@ int fail(rt_ctx* c, int code, const char* what, cudaError_t ce = cudaSuccess) {
     cudaError_t ce_ = (call);                                           \
     if (ce_ != cudaSuccess) return fail(ctx, ce_ == cudaErrorMemoryAllocation ? RT_ENOMEM : RT_ECUDA, #call, ce_); \
   } while (0)
+
+void fill_counters(const unsigned long long* h, rt_counters* out) {
+  out->n_null = h[rt::C_NULL]; out->n_rayleigh = h[rt::C_RAY]; out->n_hg = h[rt::C_HG];
+  out->n_atm_abs = h[rt::C_ATM_ABS]; out->n_sfc_hits = h[rt::C_SFC_HITS];
+  out->n_sfc_abs = h[rt::C_SFC_ABS]; out->n_toa = h[rt::C_TOA]; out->n_capped = h[rt::C_CAPPED];
+  out->n_cell_steps = h[rt::C_CELLS]; out->n_relevel = h[rt::C_RELEVEL];
+  out->n_roulette_killed = h[rt::C_ROUL_KILLED]; out->n_roulette_kept = h[rt::C_ROUL_KEPT];
+  out->roulette_lost = (int64_t)h[rt::C_ROUL_LOST]; out->roulette_gained = (int64_t)h[rt::C_ROUL_GAINED];
+  out->capped_energy = (int64_t)h[rt::C_CAPPED_E];
+  out->n_events = h[rt::C_NULL] + h[rt::C_RAY] + h[rt::C_HG] + h[rt::C_ATM_ABS];
+  out->n_photons = h[rt::C_ATM_ABS] + h[rt::C_SFC_ABS] + h[rt::C_TOA] + h[rt::C_CAPPED] + h[rt::C_ROUL_KILLED];
+}
+// Queued with cudaLaunchHostFunc behind the copy of the raw words; runs on a driver thread, calls no CUDA function.
+void CUDART_CB counters_host_fn(void* p) {
+  auto* job = static_cast<rt_ctx::CounterJob*>(p);
+  fill_counters(job->raw, job->out);
+}
 
 // Remember that `st` now carries work of this context (an event after it), for rt_read_tallies' wait.
 int mark(rt_ctx* c, cudaStream_t st) {
@@ -697,39 +718,9 @@ int rt_read_tallies(rt_ctx* c, int64_t* atm_abs, int64_t* sfc_dir, int64_t* sfc_
   unsigned long long h[rt::C_COUNT];
   if (counters) RT_CUDA(c, cudaMemcpyAsync(h, c->counters, sizeof h, cudaMemcpyDeviceToHost, c->copy_stream));
   RT_CUDA(c, cudaStreamSynchronize(c->copy_stream));
-  if (counters) {
-    counters->n_null = h[rt::C_NULL]; counters->n_rayleigh = h[rt::C_RAY]; counters->n_hg = h[rt::C_HG];
-    counters->n_atm_abs = h[rt::C_ATM_ABS]; counters->n_sfc_hits = h[rt::C_SFC_HITS];
-    counters->n_sfc_abs = h[rt::C_SFC_ABS]; counters->n_toa = h[rt::C_TOA]; counters->n_capped = h[rt::C_CAPPED];
-    counters->n_cell_steps = h[rt::C_CELLS]; counters->n_relevel = h[rt::C_RELEVEL];
-    counters->n_roulette_killed = h[rt::C_ROUL_KILLED]; counters->n_roulette_kept = h[rt::C_ROUL_KEPT];
-    counters->roulette_lost = (int64_t)h[rt::C_ROUL_LOST]; counters->roulette_gained = (int64_t)h[rt::C_ROUL_GAINED];
-    counters->capped_energy = (int64_t)h[rt::C_CAPPED_E];
-    counters->n_events = h[rt::C_NULL] + h[rt::C_RAY] + h[rt::C_HG] + h[rt::C_ATM_ABS];
-    counters->n_photons = h[rt::C_ATM_ABS] + h[rt::C_SFC_ABS] + h[rt::C_TOA] + h[rt::C_CAPPED] + h[rt::C_ROUL_KILLED];
-  }
+  if (counters) fill_counters(h, counters);
   return RT_OK;
 }
-
-}  // extern "C" (reopened below)
-
-namespace {
-__global__ void assemble_counters_kernel(const unsigned long long* __restrict__ h, rt_counters* __restrict__ out) {
-  rt_counters r;
-  r.n_null = h[rt::C_NULL]; r.n_rayleigh = h[rt::C_RAY]; r.n_hg = h[rt::C_HG];
-  r.n_atm_abs = h[rt::C_ATM_ABS]; r.n_sfc_hits = h[rt::C_SFC_HITS];
-  r.n_sfc_abs = h[rt::C_SFC_ABS]; r.n_toa = h[rt::C_TOA]; r.n_capped = h[rt::C_CAPPED];
-  r.n_cell_steps = h[rt::C_CELLS]; r.n_relevel = h[rt::C_RELEVEL];
-  r.n_roulette_killed = h[rt::C_ROUL_KILLED]; r.n_roulette_kept = h[rt::C_ROUL_KEPT];
-  r.roulette_lost = (int64_t)h[rt::C_ROUL_LOST]; r.roulette_gained = (int64_t)h[rt::C_ROUL_GAINED];
-  r.capped_energy = (int64_t)h[rt::C_CAPPED_E];
-  r.n_events = h[rt::C_NULL] + h[rt::C_RAY] + h[rt::C_HG] + h[rt::C_ATM_ABS];
-  r.n_photons = h[rt::C_ATM_ABS] + h[rt::C_SFC_ABS] + h[rt::C_TOA] + h[rt::C_CAPPED] + h[rt::C_ROUL_KILLED];
-  *out = r;
-}
-}  // namespace
-
-extern "C" {
 
 int rt_read_tallies_async(rt_ctx* c, int64_t* atm_abs, int64_t* sfc_dir, int64_t* sfc_dif, int64_t* sfc_abs,
                           int64_t* toa_up, rt_counters* counters, void* cuda_stream) {
@@ -741,10 +732,14 @@ int rt_read_tallies_async(rt_ctx* c, int64_t* atm_abs, int64_t* sfc_dir, int64_t
     if (outs[k])
       RT_CUDA(c, cudaMemcpyAsync(outs[k], tally_ptr(c, k), (k == 0 ? c->nvox : c->ncol) * sizeof(int64_t), cudaMemcpyDefault, st));
   if (counters) {
-    if (!c->d_counters) RT_CUDA(c, cudaMalloc(&c->d_counters, sizeof(rt_counters)));
-    assemble_counters_kernel<<<1, 1, 0, st>>>(c->counters, c->d_counters);
-    ++c->launches;
-    RT_CUDA(c, cudaMemcpyAsync(counters, c->d_counters, sizeof(rt_counters), cudaMemcpyDefault, st));
+    // No kernel here: behind a persistent trace kernel of ANOTHER context that already fills the SMs (it starts in the
+    // tail of this context's trace), a kernel of this stream would wait for that whole trace, and with it the caller's
+    // wait for this read-out and the upload of its next step (5.5 ms per step in bench.py's e2e leg).
+    if (!c->counter_jobs) RT_CUDA(c, cudaHostAlloc(&c->counter_jobs, 2 * sizeof(rt_ctx::CounterJob), cudaHostAllocDefault));
+    rt_ctx::CounterJob* job = c->counter_jobs + (c->counter_calls++ & 1u);
+    job->out = counters;
+    RT_CUDA(c, cudaMemcpyAsync(job->raw, c->counters, sizeof job->raw, cudaMemcpyDeviceToHost, st));
+    RT_CUDA(c, cudaLaunchHostFunc(st, counters_host_fn, job));
   }
   RT_CUDA(c, cudaGetLastError());
   return mark(c, st);
@@ -896,7 +891,7 @@ void rt_destroy(rt_ctx* c) {
     DeviceGuard guard(c->device);
     cudaDeviceSynchronize();
     cudaFree(c->optics); cudaFree(c->khat); cudaFree(c->kmin); cudaFree(c->atm_dir); cudaFree(c->albedo); cudaFree(c->tallies);
-    cudaFree(c->counters); cudaFree(c->d_counters); cudaFree(c->bad); cudaFree(c->gas_tab); cudaFree(c->point_par);
+    cudaFree(c->counters); if (c->counter_jobs) cudaFreeHost(c->counter_jobs); cudaFree(c->bad); cudaFree(c->gas_tab); cudaFree(c->point_par);
     cudaFree(c->cloud); cudaFree(c->cloud_max); cudaFree(c->cloud_min); cudaFree(c->batch_tab); cudaFree(c->sink); cudaFree(c->stage);
     cudaFree(c->blk_max); cudaFree(c->blk_min); cudaFree(c->blk_tab); cudaFree(c->gas_sum);
     if (c->ev0) cudaEventDestroy(c->ev0);
