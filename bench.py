@@ -249,7 +249,7 @@ def run_ours(args):
                                 counters=None)
     point_ms = []
 
-    def set_factored(kc, al):
+    def set_factored(kc, al, g=g):
         """All 112 points from their factors: kept factored in the trace (rt_set_cloud + rt_set_point; default) or
         packed into 16-byte records per voxel and point (rt_set_optics_factored; --packed-slots)."""
         if args.packed_slots:
@@ -405,19 +405,64 @@ def run_ours(args):
             if t.counters.n_photons != n or t.counters.n_capped != 0:
                 raise SystemExit("bench.py: e2e photon count mismatch (%d of %d)" % (t.counters.n_photons, n))
 
-        e2e_sweep(0)
-        barrier()
-        t0 = time.perf_counter()
-        for i in range(args.steps):
-            e2e_sweep(args.warmup + args.steps + i)
-        barrier()
-        e2e_s = max_over_ranks(time.perf_counter() - t0)
+        if args.e2e_serial or args.packed_slots:
+            e2e_sweep(0)
+            barrier()
+            t0 = time.perf_counter()
+            for i in range(args.steps):
+                e2e_sweep(args.warmup + args.steps + i)
+            barrier()
+            e2e_s = max_over_ranks(time.perf_counter() - t0)
+            how = "one context, synchronous read"
+        else:
+            # as the e2e leg of the other workloads: sweeps alternate over two contexts on two streams, so that one
+            # sweep's uploads and read-out overlap the other's trace
+            g2 = rt.Grid(*cfg.grid, device=local, **cfg.accel)
+            g2.set_mode(weighted=(args.mode == "weighted"))
+            g2.set_slots(len(pts))
+            ctxs, streams2 = [g, g2], [torch.cuda.Stream(dev), torch.cuda.Stream(dev)]
+            outs = [out_all, rt.Tallies(torch.empty((cfg.nz, cfg.ny, cfg.nx), dtype=torch.int64).pin_memory(),
+                                        *[torch.empty((cfg.ny, cfg.nx), dtype=torch.int64).pin_memory() for _ in range(4)],
+                                        counters=None)]
+            cbufs = [torch.zeros(ctypes.sizeof(rt.rt_counters), dtype=torch.uint8).pin_memory() for _ in range(2)]
+
+            def e2e_start(i, k):
+                with torch.cuda.stream(streams2[k]):
+                    set_factored(kc_host, al_host, ctxs[k])     # uploads first: they overlap the other context's trace
+                    ctxs[k].reset_tallies()
+                    ctxs[k].trace_batch(cfg.zenith_deg, cfg.azimuth_deg, counts,
+                                        first_photon_id=weak_range(rank, world, i, n)[0], seed=cfg.seed)
+                    ctxs[k].read_tallies_async(outs[k], cbufs[k])
+
+            def e2e_finish(k):
+                streams2[k].synchronize()
+                cnt = rt.counters_of(cbufs[k])
+                if cnt.n_photons != n or cnt.n_capped != 0:
+                    raise SystemExit("bench.py: e2e photon count mismatch (%d of %d)" % (cnt.n_photons, n))
+
+            for k in range(2):
+                e2e_start(k, k)
+            for k in range(2):
+                e2e_finish(k)
+            barrier()
+            t0 = time.perf_counter()
+            for i in range(args.steps):
+                k = i & 1
+                if i >= 2:
+                    e2e_finish(k)
+                e2e_start(args.warmup + args.steps + i, k)
+            for k in range(2):
+                e2e_finish(k)
+            barrier()
+            e2e_s = max_over_ranks(time.perf_counter() - t0)
+            how = "two contexts on two streams, sweeps alternating; copies overlap the other context's trace"
+            g2.close()
         h2d = kc_host.numel() * 4 + al_host.numel() * 4 + len(facs) * 2 * cfg.nz * 4
         d2h = (cfg.nvox + 4 * cfg.ncol) * 8 + ctypes.sizeof(rt.rt_counters)
         e2e = {"value": total_photons / e2e_s, "unit": UNIT, "ms_per_step": 1e3 * e2e_s / args.steps,
                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                "how": "factored inputs: cloud field + albedo from pinned host memory, 112 x 2 nz profile values; "
-                      "all tallies to pinned host memory; one context, synchronous read"}
+                      "all tallies to pinned host memory; " + how}
     if not spectral:
         import ctypes
         h2d = sum(x.numel() * x.element_size() for x in host)
