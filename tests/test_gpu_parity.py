@@ -467,4 +467,16 @@ def test_read_tallies_async_matches_synchronous_read():
     for name in ("atm_abs", "sfc_dir", "sfc_dif", "sfc_abs", "toa_up"):
         assert torch.equal(getattr(out, name), getattr(t, name)), name
     assert rt.counters_of(cbuf).asdict() == t.counters.asdict() and t.counters.n_photons == 1 << 16
+    # two read-outs of one context in flight (include/rt.h: at most two): each shows the counters as they stood when
+    # its turn came on the stream (tallies accumulate: 2 and 3 x 2^16 photons)
+    cbuf2 = torch.zeros(ctypes.sizeof(rt.rt_counters), dtype=torch.uint8).pin_memory()
+    with torch.cuda.stream(st):
+        g.trace(cfg.zenith_deg, cfg.azimuth_deg, 1 << 16, first_photon_id=1 << 16, seed=cfg.seed)
+        g.read_tallies_async(rt.Tallies(None, out.sfc_dir, out.sfc_dif, out.sfc_abs, out.toa_up, counters=None), cbuf)
+        g.trace(cfg.zenith_deg, cfg.azimuth_deg, 1 << 16, first_photon_id=2 << 16, seed=cfg.seed)
+        g.read_tallies_async(rt.Tallies(None, out.sfc_dir, out.sfc_dif, out.sfc_abs, out.toa_up, counters=None), cbuf2)
+    st.synchronize()
+    c1, c2 = rt.counters_of(cbuf), rt.counters_of(cbuf2)
+    assert c1.n_photons == 2 << 16 and c2.n_photons == 3 << 16 and c2.n_events > c1.n_events > t.counters.n_events
+    assert g.read_tallies().counters.asdict() == c2.asdict()
     g.close()
