@@ -216,7 +216,18 @@ int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photon
   A.records = records;
   A.n_photons = n_photons; A.first_id = first_id; A.ncol = c->ncol; A.index_base = index_base;
   A.n_full = (job_photons / c->ncol) * c->ncol;
-  const bool pow2 = !(c->ncx & (c->ncx - 1)) && !(c->ncy & (c->ncy - 1));
+  // the packed cell index of the kPow2 instantiations (rt_trace.cuh TraceArgs) needs every reachable index, one merged
+  // step beyond the top included, below 2^31
+  const bool pow2 = !(c->ncx & (c->ncx - 1)) && !(c->ncy & (c->ncy - 1)) &&
+                    (unsigned long long)c->ncell + 64ull * c->ncx * c->ncy < (1ull << 31);
+  if (pow2) {
+    auto log2i = [](int v) { int l = 0; while ((1 << l) < v) ++l; return l; };
+    A.lx = log2i(c->ncx); A.shz = A.lx + log2i(c->ncy);
+    A.xmask = (unsigned)c->ncx - 1u; A.ymask = ((unsigned)c->ncy - 1u) << A.lx; A.zmask = ~((1u << A.shz) - 1u);
+    A.omask = ~(((unsigned)c->mx - 1u) | (((unsigned)c->my - 1u) << A.lx) | (((unsigned)c->mz - 1u) << A.shz));
+  } else {
+    A.lx = A.shz = 0; A.xmask = A.ymask = A.zmask = A.omask = 0u;
+  }
   const int variant = (records ? 1 : 0) | (pow2 ? 2 : 0) | (c->weighted ? 4 : 0) | (n_points > 0 ? 8 : 0);
   const void* fn = pick_kernel(variant);
   int blocks = 0;

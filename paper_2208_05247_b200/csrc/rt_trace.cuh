@@ -57,6 +57,13 @@ struct TraceArgs {
   int mx, my, mz;
   float rmx, rmy, rmz, Lx1, Ly1, Lz1;
   unsigned vote_bias;                  // thresholds of the vote (vote_bias() above)
+  // kPow2: the cell index (cx, cy, cz) lives in ONE word, pc = cz << shz | cy << lx | cx, which for power-of-two ncx,
+  // ncy is the linear index of the cell in the majorant table; a crossing is one add and one masked merge, the
+  // periodic wrap is the field mask.  zmask = the bits from shz up; omask clears the in-block bits of the three
+  // fields (origin of a merged cell).  rt.cu uses these instantiations only when ncell + 64 ncx ncy < 2^31, so that
+  // a step beyond the top stays positive as an int and a step below the surface is negative.
+  int lx, shz;
+  unsigned xmask, ymask, zmask, omask;
   int move_steps;                      // MOVE steps between two votes: kMoveSteps or kMoveStepsUnit
   int unit;                            // bx = by = bz = 1: a level-0 acceleration cell IS a voxel (no position needed to
                                        // find the collision's voxel, and no null collisions outside merged cells)
@@ -141,7 +148,19 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
   uint32_t jpt = 0;                       // kBatch: the photon's point = its stream id and slot
   unsigned long long ig = 0;              // kBatch: index in the launch (records)
   uint32_t e = 0;
-  int cx = 0, cy = 0, cz = 0;
+  int cx = 0, cy = 0, cz = 0;             // the cell (generic grids)
+  uint32_t pc = 0;                        // ... packed (kPow2), see TraceArgs
+  uint32_t dpx = 0, dpy = 0, dpz = 0;     // kPow2: the index step per axis (+-1, or +-m in a merged cell) in its field's position
+  auto X = [&]() -> int { if constexpr (kPow2) return (int)(pc & A.xmask); else return cx; };
+  auto Y = [&]() -> int { if constexpr (kPow2) return (int)((pc & A.ymask) >> A.lx); else return cy; };
+  auto Z = [&]() -> int { if constexpr (kPow2) return (int)pc >> A.shz; else return cz; };   // arithmetic: < 0 below the surface
+  auto set_cell = [&](int x, int y, int z) {
+    if constexpr (kPow2) pc = ((uint32_t)z << A.shz) | ((uint32_t)y << A.lx) | (uint32_t)x;
+    else { cx = x; cy = y; cz = z; }
+  };
+  auto add_x = [&](int v) { if constexpr (kPow2) pc += (uint32_t)v; else cx += v; };          // within a block: no carry
+  auto add_y = [&](int v) { if constexpr (kPow2) pc += (uint32_t)v << A.lx; else cy += v; };
+  auto add_z = [&](int v) { if constexpr (kPow2) pc += (uint32_t)v << A.shz; else cz += v; };
   float da = 0, db = 0, dc = -1;          // unit direction
   float rx = 0, ry = 0, rz = 0;           // remaining distance to the cell's next face on each axis
   float delx = 0, dely = 0, delz = 0;     // distance between successive faces on each axis
@@ -152,8 +171,8 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
   bool direct = true;
   // §3.7b: kh holds the majorant table's word as stored, i.e. its sign bit says whether the photon travels
   // through a merged cell (then cx, cy, cz = that cell's origin); the majorant itself is |kh|
-  uint32_t stp = 0;                       // index step per axis as three signed bytes (+-1, or +-m in a merged
-                                          // cell), top byte: axis of the crossing that asked for a change of level
+  uint32_t stp = 0;                       // generic grids: index step per axis as three signed bytes (+-1, or +-m in a
+                                          // merged cell)
   // event counts: running totals of this thread; a photon's own counts are differences (records)
   uint32_t t_ev = 0, t_sc = 0, t_hg = 0, t_sfc = 0, t_cells = 0, t_relevel = 0;
   unsigned long long wq = kW0;            // weighted mode: the photon's weight in tally quanta
@@ -176,7 +195,8 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
   auto set_steps = [&](bool lev) {
     const int ax_ = (da > 0.0f) ? 1 : -1, ay_ = (db > 0.0f) ? 1 : -1, az_ = (dc > 0.0f) ? 1 : -1;
     const int sx = lev ? ax_ * A.mx : ax_, sy = lev ? ay_ * A.my : ay_, sz = lev ? az_ * A.mz : az_;
-    stp = ((uint32_t)sx & 0xffu) | (((uint32_t)sy & 0xffu) << 8) | (((uint32_t)sz & 0xffu) << 16);
+    if constexpr (kPow2) { dpx = (uint32_t)sx; dpy = (uint32_t)sy << A.lx; dpz = (uint32_t)sz << A.shz; }
+    else stp = ((uint32_t)sx & 0xffu) | (((uint32_t)sy & 0xffu) << 8) | (((uint32_t)sz & 0xffu) << 16);
   };
   auto place = [&](float qx, float qy, float qz) {
     const bool lev = __float_as_int(kh) < 0;
@@ -191,19 +211,27 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
     rz = ((vc > 0.0f ? Lz : 0.0f) - qz) * ic;
   };
   auto cell_of = [&]() {
-    const unsigned c = ((unsigned)cz * (unsigned)A.ncy + (unsigned)cy) * (unsigned)A.ncx + (unsigned)cx;
+    unsigned c;
+    if constexpr (kPow2) c = pc;
+    else c = ((unsigned)cz * (unsigned)A.ncy + (unsigned)cy) * (unsigned)A.ncx + (unsigned)cx;
     return kBatch ? c + jpt * A.ncell32 : c;
   };
   // the majorant table's word for the cell (cx, cy, cz): the table itself, or (fly) the block's word if the block is
   // merged, else the voxel's own extinction.  Both loads are issued at once; the indices are valid either way.
   auto voxel_word = [&]() {
-    const unsigned vox = ((unsigned)cz * (unsigned)A.ny + (unsigned)cy) * (unsigned)A.nx + (unsigned)cx;
-    return __ldg(A.gsum + jpt * (unsigned)A.nz + (unsigned)cz) + __ldg(A.cloud + vox);
+    unsigned vox;                          // voxel-sized cells: the cell index is the voxel index
+    if constexpr (kPow2) vox = pc;
+    else vox = ((unsigned)cz * (unsigned)A.ny + (unsigned)cy) * (unsigned)A.nx + (unsigned)cx;
+    return __ldg(A.gsum + jpt * (unsigned)A.nz + (unsigned)Z()) + __ldg(A.cloud + vox);
   };
   auto word_at = [&]() {
     if (kBatch && A.fly) {
-      const unsigned blk = ((unsigned)(cz >> A.lmz) * (unsigned)A.nby + (unsigned)(cy >> A.lmy)) * (unsigned)A.nbx +
-                           (unsigned)(cx >> A.lmx);
+      unsigned blk;
+      if constexpr (kPow2)                 // the three block coordinates straight from the packed index
+        blk = ((pc >> (A.shz + A.lmz)) * (unsigned)A.nby + ((pc >> (A.lx + A.lmy)) & ((unsigned)A.nby - 1u))) * (unsigned)A.nbx +
+              ((pc >> A.lmx) & ((unsigned)A.nbx - 1u));
+      else
+        blk = ((unsigned)(cz >> A.lmz) * (unsigned)A.nby + (unsigned)(cy >> A.lmy)) * (unsigned)A.nbx + (unsigned)(cx >> A.lmx);
       const float B = __ldg(A.btab + jpt * A.nblk32 + blk);
       const float k0 = voxel_word();   // (loading it only when the block is not merged was slower: 56.5 against 54.1 ms)
       return (__float_as_int(B) < 0) ? B : k0;
@@ -265,24 +293,24 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
     if (__float_as_int(kh) < 0) {
       // into a merged cell: distances to ITS faces (n whole cells further on the other two axes),
       // the index becomes its origin
-      const int ox = cx & (A.mx - 1), oy = cy & (A.my - 1), oz = cz & (A.mz - 1);   // powers of two
+      const int ox = X() & (A.mx - 1), oy = Y() & (A.my - 1), oz = Z() & (A.mz - 1);   // powers of two
       const float fx = (float)A.mx, fy = (float)A.my, fz = (float)A.mz;
       rx = (ax == 0) ? delx * fx : fmaf((float)(px ? A.mx - 1 - ox : ox), delx, rx);
       ry = (ax == 1) ? dely * fy : fmaf((float)(py ? A.my - 1 - oy : oy), dely, ry);
       rz = (ax == 2) ? delz * fz : fmaf((float)(pz ? A.mz - 1 - oz : oz), delz, rz);
       delx *= fx; dely *= fy; delz *= fz;       // exact: the factors are powers of two
-      cx -= ox; cy -= oy; cz -= oz;
+      if constexpr (kPow2) pc &= A.omask; else { cx -= ox; cy -= oy; cz -= oz; }
       set_steps(true);
     } else {
       // out of a merged cell into single cells: which cell of the entered block on the other two
       // axes (k whole cells before the block's face), and the distances to that cell's faces
       delx *= A.rmx; dely *= A.rmy; delz *= A.rmz;
-      if (ax == 0) { rx = delx; if (!px) cx += A.mx - 1; }
-      else { const int k = min(A.mx - 1, (int)(rx / delx)); rx = fmaxf(0.0f, fmaf(-(float)k, delx, rx)); cx += px ? A.mx - 1 - k : k; }
-      if (ax == 1) { ry = dely; if (!py) cy += A.my - 1; }
-      else { const int k = min(A.my - 1, (int)(ry / dely)); ry = fmaxf(0.0f, fmaf(-(float)k, dely, ry)); cy += py ? A.my - 1 - k : k; }
-      if (ax == 2) { rz = delz; if (!pz) cz += A.mz - 1; }
-      else { const int k = min(A.mz - 1, (int)(rz / delz)); rz = fmaxf(0.0f, fmaf(-(float)k, delz, rz)); cz += pz ? A.mz - 1 - k : k; }
+      if (ax == 0) { rx = delx; if (!px) add_x(A.mx - 1); }
+      else { const int k = min(A.mx - 1, (int)(rx / delx)); rx = fmaxf(0.0f, fmaf(-(float)k, delx, rx)); add_x(px ? A.mx - 1 - k : k); }
+      if (ax == 1) { ry = dely; if (!py) add_y(A.my - 1); }
+      else { const int k = min(A.my - 1, (int)(ry / dely)); ry = fmaxf(0.0f, fmaf(-(float)k, dely, ry)); add_y(py ? A.my - 1 - k : k); }
+      if (ax == 2) { rz = delz; if (!pz) add_z(A.mz - 1); }
+      else { const int k = min(A.mz - 1, (int)(rz / delz)); rz = fmaxf(0.0f, fmaf(-(float)k, delz, rz)); add_z(pz ? A.mz - 1 - k : k); }
       kh = (kBatch && A.fly) ? voxel_word() : __ldg(A.khat + cell_of());   // the single cell's own majorant (sign bit clear)
       set_steps(false);
     }
@@ -364,7 +392,7 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
           ix = min((int)(u24(X.z) * (float)A.nx), A.nx - 1);
           iy = min((int)(u24(X.w) * (float)A.ny), A.ny - 1);
         }
-        cx = ix / A.bx; cy = iy / A.by; cz = A.ncz - 1;
+        set_cell(ix / A.bx, iy / A.by, A.ncz - 1);
         da = A.sun_x; db = A.sun_y; dc = A.sun_z;
         // §3.5b: the sign bit of the stored majorant marks the cells of a merged cell
         kh = word_at();
@@ -373,7 +401,8 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
         int wx = A.bx, wy = A.by;             // cell extent in voxels at this level
         float Lx = A.Lx, Ly = A.Ly, Lz = A.Lz;
         if (lev) {
-          cx &= -A.mx; cy &= -A.my; cz &= -A.mz;      // merged-cell origin (factors are powers of two)
+          if constexpr (kPow2) pc &= A.omask;         // merged-cell origin (factors are powers of two)
+          else { cx &= -A.mx; cy &= -A.my; cz &= -A.mz; }
           wx *= A.mx; wy *= A.my; Lx = A.Lx1; Ly = A.Ly1; Lz = A.Lz1;
         }
         const float qx = ((float)(ix % wx) + e0) * A.dx, qy = ((float)(iy % wy) + e1) * A.dy;
@@ -414,10 +443,8 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
       // ---- MOVE: nearest face of the current cell (ties x < y < z), then cross or park (§3.7) -------
       // (rolled loop: one copy of the step and of the level change; the kernel is larger than the instruction cache)
 #pragma unroll 1
-      for (int rep = 0; rep < A.move_steps; ++rep) {
-      if (st == ST_MOVE) {
-        // index step per axis: +-1 cell, or +-m cells inside a merged cell
-        const int sx = (int)(stp << 24) >> 24, sy = (int)(stp << 16) >> 24, sz = (int)(stp << 8) >> 24;
+      for (int rep = A.move_steps; st == ST_MOVE && rep > 0; --rep) {   // a lane leaves the loop with its last MOVE step
+      {
         const bool ax0 = (rx <= ry) && (rx <= rz);
         const bool ax1 = !ax0 && (ry <= rz);
         const bool ax2 = !ax0 && !ax1;
@@ -433,15 +460,22 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
           ry = ax1 ? dely : ry - t;
           rz = ax2 ? delz : rz - t;
           // step the cell index; x and y wrap (periodic)
-          if (kPow2) {
-            if (ax0) cx = (cx + sx) & (A.ncx - 1);
-            if (ax1) cy = (cy + sy) & (A.ncy - 1);
+          bool outside;
+          if constexpr (kPow2) {
+            // one add in the crossed axis' field; the field mask is the periodic wrap in x and y, and in z (the top
+            // field) a step out of the domain gives an index >= ncell
+            const uint32_t d = ax0 ? dpx : (ax1 ? dpy : dpz);
+            const uint32_t m = ax0 ? A.xmask : (ax1 ? A.ymask : A.zmask);
+            pc = (pc & ~m) | ((pc + d) & m);
+            outside = pc >= A.ncell32;
           } else {
+            const int sx = (int)(stp << 24) >> 24, sy = (int)(stp << 16) >> 24, sz = (int)(stp << 8) >> 24;
             if (ax0) { cx += sx; cx = (cx >= A.ncx) ? cx - A.ncx : cx; cx = (cx < 0) ? cx + A.ncx : cx; }
             if (ax1) { cy += sy; cy = (cy >= A.ncy) ? cy - A.ncy : cy; cy = (cy < 0) ? cy + A.ncy : cy; }
+            if (ax2) cz += sz;
+            outside = (unsigned)cz >= (unsigned)A.ncz;
           }
-          if (ax2) cz += sz;
-          if ((unsigned)cz >= (unsigned)A.ncz) st = ST_BOUNDARY;   // surface (cz < 0) or domain top
+          if (outside) st = ST_BOUNDARY;             // surface (cz < 0) or domain top
           else {
             const float raw = word_at();
             const bool other = (__float_as_int(raw) ^ __float_as_int(kh)) < 0;   // §3.7b: the entered cell is at the other level
@@ -486,16 +520,17 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
         unsigned vox;
         int vz;
         if (A.unit && !lev) {                         // voxel-sized cell: the cell index is the voxel index
-          vz = cz;
-          vox = ((unsigned)cz * (unsigned)A.ny + (unsigned)cy) * (unsigned)A.nx + (unsigned)cx;
+          vz = Z();
+          if constexpr (kPow2) vox = pc;
+          else vox = ((unsigned)cz * (unsigned)A.ny + (unsigned)cy) * (unsigned)A.nx + (unsigned)cx;
         } else {
           const float qx = local(da, rx, lev ? A.Lx1 : A.Lx), qy = local(db, ry, lev ? A.Ly1 : A.Ly),
                       qz = local(dc, rz, lev ? A.Lz1 : A.Lz);
           const int lx = min((int)(qx * A.rdx), (lev ? A.mx * A.bx : A.bx) - 1);
           const int ly = min((int)(qy * A.rdy), (lev ? A.my * A.by : A.by) - 1);
           const int lz = min((int)(qz * A.rdz), (lev ? A.mz * A.bz : A.bz) - 1);
-          vz = cz * A.bz + lz;
-          vox = ((unsigned)vz * (unsigned)A.ny + (unsigned)(cy * A.by + ly)) * (unsigned)A.nx + (unsigned)(cx * A.bx + lx);
+          vz = Z() * A.bz + lz;
+          vox = ((unsigned)vz * (unsigned)A.ny + (unsigned)(Y() * A.by + ly)) * (unsigned)A.nx + (unsigned)(X() * A.bx + lx);
         }
         float4 v;
         if (kBatch && A.cloud) {
@@ -559,10 +594,10 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
       if (st == ST_BOUNDARY) {
         const bool lev = __float_as_int(kh) < 0;
         const float qx = local(da, rx, lev ? A.Lx1 : A.Lx), qy = local(db, ry, lev ? A.Ly1 : A.Ly);
-        const int hx = cx * A.bx + min((int)(qx * A.rdx), (lev ? A.mx * A.bx : A.bx) - 1);
-        const int hy = cy * A.by + min((int)(qy * A.rdy), (lev ? A.my * A.by : A.by) - 1);
+        const int hx = X() * A.bx + min((int)(qx * A.rdx), (lev ? A.mx * A.bx : A.bx) - 1);
+        const int hy = Y() * A.by + min((int)(qy * A.rdy), (lev ? A.my * A.by : A.by) - 1);
         const unsigned col = (unsigned)hy * (unsigned)A.nx + (unsigned)hx;
-        if (cz >= 0) {                              // left through the domain top
+        if (Z() >= 0) {                             // left through the domain top
           if (kWeighted) atomicAdd(A.toa_up + col, wq); else tally_a = A.toa_up + col;
           fate = 3; term = (uint32_t)col;
         } else {                                    // Lambertian surface
@@ -588,7 +623,8 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
             float sp, cp;
             sincos_2pi(u24(w3), sp, cp);
             da = sn * cp; db = sn * sp; dc = mu;
-            direct = false; cz = 0;                 // back in the cell it left: same level, same majorant
+            direct = false;                         // back in the cell it left (cz = 0): same level, same majorant
+            if constexpr (kPow2) pc &= ~A.zmask; else cz = 0;
             place(qx, qy, 0.0f);
             ++e;
             if (e > kEventCap) { fate = 4; term = 0; }   // §3.12
