@@ -288,16 +288,21 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
   //      kh already holds the ENTERED cell's word).  It used to be a parked phase of its own: 3 per photon, batches
   //      of 4-6 lanes, one visit running both directions and often the arrival code too (31 % of the kernel's
   //      instructions, profiles/r2_trace_kernel.md); inline it runs for the 1-2 lanes that need it at that step.
-  auto relevel = [&](int ax) {
+  auto relevel = [&](bool a0, bool a1, bool a2) {   // which axis was crossed
+    // The compiler otherwise lifts the cheap parts of both branches (the in-block offsets, the rescaled face
+    // spacings) into the MOVE step itself, where every lane pays for them at every crossing: an empty volatile asm
+    // that redefines the inputs keeps them in here (5 % of the kernel's instructions, profiles/r2_trace_kernel.md F).
+    asm volatile("" : "+f"(delx), "+f"(dely), "+f"(delz));
+    if constexpr (kPow2) asm volatile("" : "+r"(pc));
     const bool px = da > 0.0f, py = db > 0.0f, pz = dc > 0.0f;
     if (__float_as_int(kh) < 0) {
       // into a merged cell: distances to ITS faces (n whole cells further on the other two axes),
       // the index becomes its origin
       const int ox = X() & (A.mx - 1), oy = Y() & (A.my - 1), oz = Z() & (A.mz - 1);   // powers of two
       const float fx = (float)A.mx, fy = (float)A.my, fz = (float)A.mz;
-      rx = (ax == 0) ? delx * fx : fmaf((float)(px ? A.mx - 1 - ox : ox), delx, rx);
-      ry = (ax == 1) ? dely * fy : fmaf((float)(py ? A.my - 1 - oy : oy), dely, ry);
-      rz = (ax == 2) ? delz * fz : fmaf((float)(pz ? A.mz - 1 - oz : oz), delz, rz);
+      rx = a0 ? delx * fx : fmaf((float)(px ? A.mx - 1 - ox : ox), delx, rx);
+      ry = a1 ? dely * fy : fmaf((float)(py ? A.my - 1 - oy : oy), dely, ry);
+      rz = a2 ? delz * fz : fmaf((float)(pz ? A.mz - 1 - oz : oz), delz, rz);
       delx *= fx; dely *= fy; delz *= fz;       // exact: the factors are powers of two
       if constexpr (kPow2) pc &= A.omask; else { cx -= ox; cy -= oy; cz -= oz; }
       set_steps(true);
@@ -305,11 +310,11 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
       // out of a merged cell into single cells: which cell of the entered block on the other two
       // axes (k whole cells before the block's face), and the distances to that cell's faces
       delx *= A.rmx; dely *= A.rmy; delz *= A.rmz;
-      if (ax == 0) { rx = delx; if (!px) add_x(A.mx - 1); }
+      if (a0) { rx = delx; if (!px) add_x(A.mx - 1); }
       else { const int k = min(A.mx - 1, (int)(rx / delx)); rx = fmaxf(0.0f, fmaf(-(float)k, delx, rx)); add_x(px ? A.mx - 1 - k : k); }
-      if (ax == 1) { ry = dely; if (!py) add_y(A.my - 1); }
+      if (a1) { ry = dely; if (!py) add_y(A.my - 1); }
       else { const int k = min(A.my - 1, (int)(ry / dely)); ry = fmaxf(0.0f, fmaf(-(float)k, dely, ry)); add_y(py ? A.my - 1 - k : k); }
-      if (ax == 2) { rz = delz; if (!pz) add_z(A.mz - 1); }
+      if (a2) { rz = delz; if (!pz) add_z(A.mz - 1); }
       else { const int k = min(A.mz - 1, (int)(rz / delz)); rz = fmaxf(0.0f, fmaf(-(float)k, delz, rz)); add_z(pz ? A.mz - 1 - k : k); }
       kh = (kBatch && A.fly) ? voxel_word() : __ldg(A.khat + cell_of());   // the single cell's own majorant (sign bit clear)
       set_steps(false);
@@ -480,7 +485,7 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
             const float raw = word_at();
             const bool other = (__float_as_int(raw) ^ __float_as_int(kh)) < 0;   // §3.7b: the entered cell is at the other level
             kh = raw;
-            if (other) relevel(ax0 ? 0 : (ax1 ? 1 : 2));
+            if (other) relevel(ax0, ax1, ax2);
           }
         }
       }
