@@ -310,6 +310,7 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
   const int mxyz[3] = {P.mx, P.my, P.mz};
   const R Lv[2][3] = {{(R)bx * dx, (R)by * dy, (R)bz * dz},
                       {(R)(P.mx * bx) * dx, (R)(P.my * by) * dy, (R)(P.mz * bz) * dz}};
+  const R rL0[3] = {(R)1 / Lv[0][0], (R)1 / Lv[0][1], (R)1 / Lv[0][2]};   // §3.7b: reciprocal level-0 cell extents
   const int ncs[3] = {ncx, ncy, ncz};
   const R TINY = (R)1e-30f;
 
@@ -604,8 +605,10 @@ void trace_range(const Problem& P, const std::vector<float>& khat, uint64_t i_be
               for (int a = 0; a < 3; ++a) {
                 const int m = mxyz[a];
                 if (a != axis) {
-                  const int k = std::min(m - 1, (int)(r[a] / del[0][a]));
-                  if (track) note_floor(DK_RELEVEL, k, r[a] / del[0][a], m);
+                  // whole level-0 cells in r: r / del^0 with del^0 = L^0 |1/v|, taken as r (|v| (1/L^0))
+                  const R cells = r[a] * (std::fabs(v[a]) * rL0[a]);
+                  const int k = std::min(m - 1, (int)cells);
+                  if (track) note_floor(DK_RELEVEL, k, cells, m);
                   r[a] = std::max((R)0, E::fma(-(R)k, del[0][a], r[a]));
                   c[a] += (v[a] > 0) ? (m - 1 - k) : k;
                 } else {
