@@ -194,6 +194,7 @@ int do_trace(rt_ctx* c, double zenith_deg, double azimuth_deg, uint64_t n_photon
   A.dx = c->dx; A.dy = c->dy; A.dz = c->dz;
   A.rdx = 1.0f / c->dx; A.rdy = 1.0f / c->dy; A.rdz = 1.0f / c->dz;
   A.Lx = (float)c->bx * c->dx; A.Ly = (float)c->by * c->dy; A.Lz = (float)c->bz * c->dz;
+  A.rLx = 1.0f / A.Lx; A.rLy = 1.0f / A.Ly; A.rLz = 1.0f / A.Lz;
   A.mx = c->mx; A.my = c->my; A.mz = c->mz;
   A.unit = (c->bx == 1 && c->by == 1 && c->bz == 1) ? 1 : 0;
   A.vote_bias = rt::vote_bias(A.unit ? rt::kCollideBatchUnit : rt::kCollideBatch);

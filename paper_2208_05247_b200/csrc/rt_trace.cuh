@@ -38,7 +38,7 @@ constexpr int kRegenBatch = 6;         // refill when this many lanes are idle (
 constexpr int kScatterBatch = 8;       // SCATTER
 constexpr int kCollideBatch = 8, kCollideBatchUnit = 12;   // COLLIDE: cells of several voxels / voxel-sized cells
 constexpr int kBoundaryBatch = 8;      // BOUNDARY: surface and domain-top arrivals (1 per photon)
-constexpr int kMoveSteps = 3, kMoveStepsUnit = 4;           // MOVE steps between two votes
+constexpr int kMoveSteps = 3, kMoveStepsUnit = 5;           // MOVE steps between two votes
 constexpr int kMoveStepsFly = 6;       // ... in a sweep over spectral points kept factored (8 crossings per collision)
 constexpr unsigned vote_bias(int collide_batch) {
   return (32u - kRegenBatch) | ((32u - 1u) << 6) | ((32u - (unsigned)collide_batch) << 12) |
@@ -53,6 +53,7 @@ enum : uint32_t { ST_DEAD = 0, ST_MOVE = 1, ST_COLLIDE = 2, ST_SCATTER = 3, ST_B
 struct TraceArgs {
   int nx, ny, nz, bx, by, bz, ncx, ncy, ncz;
   float dx, dy, dz, rdx, rdy, rdz, Lx, Ly, Lz;
+  float rLx, rLy, rLz;                 // 1 / Lx ...: §3.7b counts the whole cells in a remaining distance without dividing
   // §3.5b merged cells: factors (powers of two), their reciprocals, merged-cell extents (m b) d
   int mx, my, mz;
   float rmx, rmy, rmz, Lx1, Ly1, Lz1;
@@ -308,14 +309,14 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
       set_steps(true);
     } else {
       // out of a merged cell into single cells: which cell of the entered block on the other two
-      // axes (k whole cells before the block's face), and the distances to that cell's faces
+      // axes (k whole cells before the block's face: r / del = r (|v| (1 / L)), §3.7b), and the distances to that cell's faces
       delx *= A.rmx; dely *= A.rmy; delz *= A.rmz;
       if (a0) { rx = delx; if (!px) add_x(A.mx - 1); }
-      else { const int k = min(A.mx - 1, (int)(rx / delx)); rx = fmaxf(0.0f, fmaf(-(float)k, delx, rx)); add_x(px ? A.mx - 1 - k : k); }
+      else { const int k = min(A.mx - 1, (int)(rx * (fabsf(da) * A.rLx))); rx = fmaxf(0.0f, fmaf(-(float)k, delx, rx)); add_x(px ? A.mx - 1 - k : k); }
       if (a1) { ry = dely; if (!py) add_y(A.my - 1); }
-      else { const int k = min(A.my - 1, (int)(ry / dely)); ry = fmaxf(0.0f, fmaf(-(float)k, dely, ry)); add_y(py ? A.my - 1 - k : k); }
+      else { const int k = min(A.my - 1, (int)(ry * (fabsf(db) * A.rLy))); ry = fmaxf(0.0f, fmaf(-(float)k, dely, ry)); add_y(py ? A.my - 1 - k : k); }
       if (a2) { rz = delz; if (!pz) add_z(A.mz - 1); }
-      else { const int k = min(A.mz - 1, (int)(rz / delz)); rz = fmaxf(0.0f, fmaf(-(float)k, delz, rz)); add_z(pz ? A.mz - 1 - k : k); }
+      else { const int k = min(A.mz - 1, (int)(rz * (fabsf(dc) * A.rLz))); rz = fmaxf(0.0f, fmaf(-(float)k, delz, rz)); add_z(pz ? A.mz - 1 - k : k); }
       kh = (kBatch && A.fly) ? voxel_word() : __ldg(A.khat + cell_of());   // the single cell's own majorant (sign bit clear)
       set_steps(false);
     }
