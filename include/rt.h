@@ -278,6 +278,14 @@ uint64_t rt_launch_count(const rt_ctx* ctx);
 int rt_philox_words(int cuda_device, const uint32_t* ctr, uint32_t key0, uint32_t key1, uint32_t* out,
                     uint64_t n);
 
+/* Self-test of the two places where the kernels replace an IEEE fp32 operation by the instruction sequence the compiler
+ * itself uses on the fast side of that operation's range check (rt_device.cuh: rcp_in_range for 1 / x, sqrt_in_range
+ * for sqrt(x); the operands there cannot leave the range): compares them with 1.0f / x and sqrtf(x)
+ * over EVERY float of their ranges (reciprocal: 2^-126 <= |x| < 2^125, both signs; root: 2^-101 <= x <= FLT_MAX) and
+ * writes the numbers of differing results, which must be 0 for the kernels to follow the stream definition bit for bit.
+ * About 0.1 s.  Errors: RT_EINVAL, RT_ENOMEM, RT_ECUDA. */
+int rt_selftest_ieee(int cuda_device, uint64_t* rcp_mismatches, uint64_t* sqrt_mismatches);
+
 /* The majorant table WITHOUT any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture,
  * tight serving loops, harnesses that forbid it).  Computes what rt_set_optics + rt_read_majorant give for the same
  * extinction field (the maximum of the extinction over each acceleration cell, and the merged

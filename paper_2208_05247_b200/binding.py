@@ -14,7 +14,7 @@ MODE_ANALOG, MODE_WEIGHTED = 0, 1
 
 EXPORTS = ("rt_create_grid", "rt_set_merge", "rt_set_mode", "rt_set_source", "rt_set_optics", "rt_set_slots", "rt_set_optics_slot", "rt_set_optics_factored", "rt_set_cloud", "rt_set_point", "rt_set_points", "rt_trace_batch", "rt_trace", "rt_trace_records", "rt_trace_range", "rt_read_tallies", "rt_read_tallies_async",
            "rt_reset_tallies", "rt_set_heating_split", "rt_read_heating_direct", "rt_tally_to_flux", "rt_read_majorant", "rt_read_packed_optics", "rt_gather_bench",
-           "rt_last_trace_ms", "rt_launch_count", "rt_philox_words", "rt_majorant_no_alloc", "rt_no_alloc_last_error", "rt_last_error", "rt_destroy")
+           "rt_last_trace_ms", "rt_launch_count", "rt_philox_words", "rt_selftest_ieee", "rt_majorant_no_alloc", "rt_no_alloc_last_error", "rt_last_error", "rt_destroy")
 
 COUNTER_FIELDS = ("n_photons", "n_events", "n_null", "n_rayleigh", "n_hg", "n_atm_abs", "n_sfc_hits",
                   "n_sfc_abs", "n_toa", "n_capped", "n_cell_steps", "n_relevel", "n_roulette_killed", "n_roulette_kept",
@@ -74,6 +74,7 @@ def lib():
     L.rt_launch_count.argtypes = [vp]
     L.rt_launch_count.restype = u64
     L.rt_philox_words.argtypes = [i32, vp, u32, u32, vp, u64]
+    L.rt_selftest_ieee.argtypes = [i32, C.POINTER(u64), C.POINTER(u64)]
     L.rt_majorant_no_alloc.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, i32, i32, i32, i32, f32, i32, vp]
     L.rt_no_alloc_last_error.argtypes = []
     L.rt_no_alloc_last_error.restype = C.c_char_p
@@ -341,6 +342,15 @@ def philox_words(ctr, key, device=0):
     if rc != 0:
         raise RtError("rt_philox_words failed (%d)" % rc)
     return out
+
+
+def selftest_ieee(device=0):
+    """include/rt.h rt_selftest_ieee: (reciprocal mismatches, square-root mismatches) over every float of the ranges."""
+    a, b = C.c_uint64(0), C.c_uint64(0)
+    rc = lib().rt_selftest_ieee(int(device), C.byref(a), C.byref(b))
+    if rc != 0:
+        raise RtError("rt_selftest_ieee failed (%d)" % rc)
+    return a.value, b.value
 
 
 NO_ALLOC_MAX_CELLS = 1 << 20

@@ -895,6 +895,25 @@ int rt_philox_words(int cuda_device, const uint32_t* ctr, uint32_t key0, uint32_
   return RT_OK;
 }
 
+int rt_selftest_ieee(int cuda_device, uint64_t* rcp_mismatches, uint64_t* sqrt_mismatches) {
+  if (!rcp_mismatches || !sqrt_mismatches) return RT_EINVAL;
+  DeviceGuard guard(cuda_device);
+  unsigned long long* d = nullptr;
+  if (cudaMalloc(&d, 2 * sizeof(unsigned long long)) != cudaSuccess) return RT_ENOMEM;
+  unsigned long long h[2] = {0, 0};
+  cudaError_t ce = cudaMemset(d, 0, sizeof h);
+  // reciprocal: biased exponents 1 .. 251 (2^-126 <= |x| < 2^125); square root: from 2^-101 to the largest finite float
+  if (ce == cudaSuccess) {
+    rt::ieee_selftest_kernel<<<1184, 256>>>(d, 1u << 23, 252u << 23, 0x0d000000u, 0x7f800000u);
+    ce = cudaGetLastError();
+  }
+  if (ce == cudaSuccess) ce = cudaMemcpy(h, d, sizeof h, cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  if (ce != cudaSuccess) return RT_ECUDA;
+  *rcp_mismatches = h[0]; *sqrt_mismatches = h[1];
+  return RT_OK;
+}
+
 const char* rt_last_error(const rt_ctx* c) { return c ? c->err.c_str() : "null context"; }
 
 void rt_destroy(rt_ctx* c) {

@@ -408,6 +408,26 @@ __global__ void gather_bench_kernel(const float4* __restrict__ optics, unsigned 
   if (acc == -1.2345f) sink[0] = acc;
 }
 
+// rt_selftest_ieee: rcp_in_range and sqrt_in_range (rt_device.cuh) against the IEEE operations they stand for, over
+// EVERY float of their ranges: bit patterns [lo, hi) of positive floats, the reciprocal also for the negated value.
+__global__ void ieee_selftest_kernel(unsigned long long* __restrict__ bad, uint32_t rcp_lo, uint32_t rcp_hi,
+                                     uint32_t sqrt_lo, uint32_t sqrt_hi) {
+  const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+  const unsigned long long t0 = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  unsigned long long nr = 0, ns = 0;
+  for (unsigned long long b = rcp_lo + t0; b < rcp_hi; b += stride) {
+    const float x = __uint_as_float((uint32_t)b);
+    if (__float_as_uint(rcp_in_range(x)) != __float_as_uint(1.0f / x)) ++nr;
+    if (__float_as_uint(rcp_in_range(-x)) != __float_as_uint(1.0f / -x)) ++nr;
+  }
+  for (unsigned long long b = sqrt_lo + t0; b < sqrt_hi; b += stride) {
+    const float x = __uint_as_float((uint32_t)b);
+    if (__float_as_uint(sqrt_in_range(x)) != __float_as_uint(sqrtf(x))) ++ns;
+  }
+  if (nr) atomicAdd(bad, nr);
+  if (ns) atomicAdd(bad + 1, ns);
+}
+
 __global__ void philox_words_kernel(const uint4* __restrict__ ctr, uint32_t k0, uint32_t k1,
                                     uint4* __restrict__ out, unsigned long long n) {
   const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;

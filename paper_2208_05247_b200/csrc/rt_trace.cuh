@@ -204,7 +204,7 @@ __global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const 
     da = nudge(da); db = nudge(db); dc = nudge(dc);   // Q20: the nudged components are the direction from here on
     set_steps(lev);
     const float va = da, vb = db, vc = dc;
-    const float ia = 1.0f / va, ib = 1.0f / vb, ic = 1.0f / vc;
+    const float ia = rcp_in_range(va), ib = rcp_in_range(vb), ic = rcp_in_range(vc);   // |v| in [1e-30, 1]
     const float Lx = lev ? A.Lx1 : A.Lx, Ly = lev ? A.Ly1 : A.Ly, Lz = lev ? A.Lz1 : A.Lz;
     delx = Lx * fabsf(ia); dely = Ly * fabsf(ib); delz = Lz * fabsf(ic);
     rx = ((va > 0.0f ? Lx : 0.0f) - qx) * ia;

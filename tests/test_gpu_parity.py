@@ -480,3 +480,11 @@ def test_read_tallies_async_matches_synchronous_read():
     assert c1.n_photons == 2 << 16 and c2.n_photons == 3 << 16 and c2.n_events > c1.n_events > t.counters.n_events
     assert g.read_tallies().counters.asdict() == c2.asdict()
     g.close()
+
+
+def test_in_range_reciprocal_and_root_equal_the_ieee_operations():
+    """rt_device.cuh replaces 1 / x and sqrt(x), where the operand cannot leave the normal range, by the compiler's own
+    fast-path sequence without its range check.  The stream definition says IEEE fp32 division and
+    square root, and the oracle uses them: the two must agree for EVERY float of the ranges, not for a sample."""
+    rt = _rt()
+    assert rt.selftest_ieee(0) == (0, 0)
