@@ -129,7 +129,11 @@ __device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
 // absorption: integer weight wq (tally quanta), deposits at every tentative collision, roulette ledger.
 // kBatch: several spectral points in one launch, each with its own optics and majorant slot (see TraceArgs).
 template <bool kRecords, bool kPow2, bool kWeighted, bool kBatch = false>
-__global__ void __launch_bounds__(kTraceThreads, kMinBlocks) trace_kernel(const TraceArgs A) {
+// Launch bounds: 4 blocks of 256 threads per SM (64 registers) for the weighted and the batch instantiations; the
+// analog single-point ones need 58 registers and run better squeezed to 48 with 5 blocks per SM (40 warps instead of
+// 32 hide more of the majorant load's latency: config 3 67.8 -> 67.2 ms, config 5 379 -> 368; weighted 74.4 -> 75.1 and
+// the batch kernel 49.9 -> 50.4 would lose).
+__global__ void __launch_bounds__(kTraceThreads, (!kBatch && !kWeighted) ? kMinBlocks + 1 : kMinBlocks) trace_kernel(const TraceArgs A) {
   __shared__ unsigned long long s_cnt[C_COUNT];
   // finished photons of this block per fate (1..5): 32-bit words, because a 64-bit shared-memory atomic is a
   // compare-and-swap loop; a launch holds fewer than 2^32 photons (rt.cu splits longer calls)
